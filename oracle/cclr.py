@@ -1,0 +1,261 @@
+"""O4-O9 — CC-LR on the CPU (TEST INFRASTRUCTURE; see oracle/__init__.py).
+
+sigma = A x, A = CCSD Jacobian (Eq. 14; Table 1), two ways:
+  * sigma_fd      : the definition A x = d/de Omega(t + e x)|0 by a 5-point stencil, exact because Omega is a
+                    polynomial of degree <= 4 in t;
+  * CCLR.sigma    : hand-coded from S-Eq. 11-12 with the intermediates S-Eq. 15-28
+                     in the readings listed in DESIGN.md ("Readings of the paper").
+Response equations (A - z) t = -xi, z = w + i*gamma (Eq. 19, 183-187 Eq. 20-21), xi / eta
+(S-Eq. 2-6), Lambda (Eq. 13), the F.x.y contraction as the second derivative of
+the Lagrangian, and the response functions Eq. 15-17.
+
+Conventions: V[p,q,r,s] = <pq||rs>, upper index = bra; t1[a,i], t2[a,b,i,j]; lam1[a,i] =
+lambda^i_a, lam2[a,b,i,j] = lambda^ij_ab; all tensors full (unpacked) complex128; dots over UNIQUE elements
+(singles + a<b,i<j).  P(pq) g = g - g(p<->q) (the minus sign is lost in the extracted text).
+"""
+import numpy as np
+from . import ccsd
+from .packing import flat, unflat
+
+
+def _Pab(x):
+    return x - x.transpose(1, 0, 2, 3)
+
+
+def _Pij(x):
+    return x - x.transpose(0, 1, 3, 2)
+
+
+# ------------------------------------------------------------------------------------------------------------
+# O4: sigma by the definition
+# ------------------------------------------------------------------------------------------------------------
+def sigma_fd(ints, t1, t2, x1, x2, h=None):
+    """A x = [Omega(t-2hx) - 8 Omega(t-hx) + 8 Omega(t+hx) - Omega(t+2hx)] / (12h); exact for a quartic."""
+    if h is None:
+        nx = np.sqrt(np.linalg.norm(x1) ** 2 + np.linalg.norm(x2) ** 2)
+        nt = np.sqrt(np.linalg.norm(t1) ** 2 + np.linalg.norm(t2) ** 2)
+        h = max(nt, 1e-1) / max(nx, 1e-300)
+    acc1 = acc2 = 0.0
+    for c, s in ((1.0, -2.0), (-8.0, -1.0), (8.0, 1.0), (-1.0, 2.0)):
+        o1, o2 = ccsd.residual(ints, t1 + s * h * x1, t2 + s * h * x2)
+        acc1 = acc1 + c * o1
+        acc2 = acc2 + c * o2
+    return acc1 / (12 * h), acc2 / (12 * h)
+
+
+# ------------------------------------------------------------------------------------------------------------
+# O5: intermediates and hand-coded sigma
+# ------------------------------------------------------------------------------------------------------------
+class CCLR:
+    """Intermediates of S-Eq. 15-28 for given integrals and ground-state amplitudes, and A x from S-Eq. 11-12."""
+
+    def __init__(self, ints, t1, t2):
+        I = self.I = ints
+        self.o, self.v = ints.o, ints.v
+        self.t1, self.t2 = t1, t2
+        tau = self.tau = ccsd.tau(t1, t2)                                          # S-Eq. 28
+        vovv = -I.ovvv.transpose(1, 0, 2, 3)                                       # <am||ef> = -<ma||ef>
+        oovo = -I.ooov.transpose(0, 1, 3, 2)                                       # <mn||ej> = -<mn||je>
+        # S-Eq. 17, 15, 16 (16 read as F^a_e with a = bra, DESIGN reading 2)
+        self.Fme = I.fov + np.einsum("mnef,fn->me", I.oovv, t1)
+        self.Fmi = (I.foo + np.einsum("me,ei->mi", I.fov, t1) + np.einsum("mnie,en->mi", I.ooov, t1)
+                    + 0.5 * np.einsum("mnef,efin->mi", I.oovv, tau))
+        self.Fae = (I.fvv - np.einsum("am,me->ae", t1, I.fov) + np.einsum("fm,amef->ae", t1, vovv)
+                    - 0.5 * np.einsum("afmn,mnef->ae", tau, I.oovv))
+        # S-Eq. 18
+        self.Wmnij = (I.oooo + _Pij(np.einsum("ej,mnie->mnij", t1, I.ooov))
+                      + 0.5 * np.einsum("efij,mnef->mnij", tau, I.oovv))
+        # S-Eq. 22
+        self.Wabef = (I.vvvv - _Pab(np.einsum("bm,amef->abef", t1, vovv))
+                      + 0.5 * np.einsum("abmn,mnef->abef", tau, I.oovv))
+        # S-Eq. 23, 19
+        self.Wbar = I.ovvo - np.einsum("bfnj,mnef->mbej", t2, I.oovv)
+        self.Wmbej = (I.ovvo + np.einsum("fj,mbef->mbej", t1, I.ovvv) - np.einsum("bn,mnej->mbej", t1, oovo)
+                      - np.einsum("fbjn,mnef->mbej", t2 + np.einsum("fj,bn->fbjn", t1, t1), I.oovv))
+        # S-Eq. 24, 25
+        self.Wmnie = I.ooov + np.einsum("fi,mnfe->mnie", t1, I.oovv)
+        self.Wamef = vovv - np.einsum("an,nmef->amef", t1, I.oovv)
+        # S-Eq. 20 (sign of the F.t2 term: reading 3)
+        self.Wmbij = (I.ovoo - np.einsum("me,beij->mbij", self.Fme, t2)
+                      - np.einsum("bn,mnij->mbij", t1, self.Wmnij)
+                      + 0.5 * np.einsum("mbef,efij->mbij", I.ovvv, tau)
+                      + _Pij(np.einsum("mnie,bejn->mbij", I.ooov, t2))
+                      + _Pij(np.einsum("ei,mbej->mbij", t1, self.Wbar)))
+        # S-Eq. 21 (sign of the P V t2 term and q -> g: reading 4)
+        self.Wabej = (I.vvvo - np.einsum("me,abmj->abej", self.Fme, t2)
+                      + np.einsum("fj,abef->abej", t1, self.Wabef)
+                      + 0.5 * np.einsum("mnej,abmn->abej", oovo, tau)
+                      - _Pab(np.einsum("mbef,afmj->abej", I.ovvv, t2))
+                      - _Pab(np.einsum("am,mbej->abej", t1, self.Wbar)))
+        self.D1, self.D2 = ccsd.denominators(ints)
+
+    # ---- S-Eq. 11-12 -------------------------------------------------------------------------------------
+    def sigma(self, r1, r2, z=0.0):
+        """(A - z) r for r1[a,i], r2[a,b,i,j] antisymmetric; z = omega + i*gamma."""
+        I, t2 = self.I, self.t2
+        s1 = (np.einsum("ae,ei->ai", self.Fae, r1) - np.einsum("mi,am->ai", self.Fmi, r1)      # S1-S2
+              + np.einsum("me,aeim->ai", self.Fme, r2)                                          # S3
+              + np.einsum("maei,em->ai", self.Wmbej, r1)                                        # S4 (reading 1)
+              + 0.5 * np.einsum("amef,efim->ai", self.Wamef, r2)                                # S5
+              - 0.5 * np.einsum("mnie,aemn->ai", self.Wmnie, r2))                               # S6
+        s2 = -_Pab(np.einsum("mbij,am->abij", self.Wmbij, r1))                                  # T1
+        s2 += _Pij(np.einsum("abej,ei->abij", self.Wabej, r1))                                  # T2
+        s2 += _Pab(np.einsum("bf,afij->abij", np.einsum("bmfe,em->bf", self.Wamef, r1), t2))    # T3
+        s2 -= _Pij(np.einsum("nj,abin->abij", np.einsum("nmje,em->nj", self.Wmnie, r1), t2))    # T4
+        s2 += _Pab(np.einsum("be,aeij->abij", self.Fae, r2))                                    # T5
+        s2 -= _Pij(np.einsum("mj,abim->abij", self.Fmi, r2))                                    # T6
+        s2 += 0.5 * np.einsum("mnij,abmn->abij", self.Wmnij, r2)                                # T7
+        ring = np.einsum("mbej,aeim->abij", self.Wmbej, r2)                                     # T8
+        s2 += _Pab(_Pij(ring))
+        s2 -= 0.5 * _Pab(np.einsum("fa,fbij->abij", np.einsum("nmfe,eamn->fa", I.oovv, r2), t2))   # T9
+        s2 -= 0.5 * _Pij(np.einsum("ni,bajn->abij", np.einsum("nmfe,feim->ni", I.oovv, r2), t2))   # T10
+        s2 += 0.5 * np.einsum("abef,efij->abij", self.Wabef, r2)                                # T11
+        return s1 - z * r1, s2 - z * r2
+
+    # ---- dense algebra over unique elements (small sizes) ---------------------------------------------------
+    def dim(self):
+        o, v = self.o, self.v
+        return o * v + (o * (o - 1) // 2) * (v * (v - 1) // 2)
+
+    def dense_jacobian(self):
+        n = self.dim()
+        A = np.zeros((n, n), complex)
+        e = np.zeros(n, complex)
+        for k in range(n):
+            e[k] = 1.0
+            A[:, k] = flat(*self.sigma(*unflat(e, self.o, self.v)))
+            e[k] = 0.0
+        return A
+
+    # ---- Lambda, xi, eta -----------------------------------------------------------------------------------
+    def eta0(self):
+        """eta0_nu = <R|[Hbar,tau_nu]|R> = (Fme[i,a], <ij||ab>)."""
+        return self.Fme.T.copy(), self.I.oovv.transpose(2, 3, 0, 1).copy()
+
+    def solve_lambda_dense(self, A=None):
+        """lambda A = -eta0 (Eq. 13) by dense LU over unique elements."""
+        A = self.dense_jacobian() if A is None else A
+        lam = np.linalg.solve(A.T, -flat(*self.eta0()))
+        return unflat(lam, self.o, self.v)
+
+    def xi(self, X):
+        """xi^X_mu = <mu|Xbar|R> = Omega[f := X, V := 0](t)  (S-Eq. 1)."""
+        return ccsd.residual(self.I.one_body_only(X), self.t1, self.t2)
+
+    def xi_printed(self, X):
+        """S-Eq. 2-3 as printed."""
+        o = self.o
+        t1, t2 = self.t1, self.t2
+        Xoo, Xov, Xvo, Xvv = X[:o, :o], X[:o, o:], X[o:, :o], X[o:, o:]
+        x1 = (Xvo + Xvv @ t1 - t1 @ Xoo - t1 @ (Xov @ t1) + np.einsum("me,aeim->ai", Xov, t2))
+        x2 = (_Pab(np.einsum("bf,afij->abij", Xvv, t2)) - _Pij(np.einsum("mj,abim->abij", Xoo, t2))
+              - _Pij(np.einsum("mi,abmj->abij", Xov @ t1, t2))
+              - _Pab(np.einsum("af,fbij->abij", t1 @ Xov, t2)))
+        return x1, x2
+
+    def eta(self, X, lam1, lam2):
+        """S-Eq. 5-6 as printed; X^p_q = X[p,q]; result laid out like amplitudes [a,i], [a,b,i,j]."""
+        o = self.o
+        t1, t2 = self.t1, self.t2
+        Xoo, Xov, Xvo, Xvv = X[:o, :o], X[:o, o:], X[o:, :o], X[o:, o:]
+        e1 = (Xov.T + np.einsum("ea,ei->ai", Xvv, lam1) - np.einsum("im,am->ai", Xoo, lam1)
+              - np.einsum("ma,em,ei->ai", Xov, t1, lam1) - np.einsum("ie,em,am->ai", Xov, t1, lam1)
+              - 0.5 * np.einsum("ni,na->ai", np.einsum("femn,femi->ni", t2, lam2), Xov)
+              - 0.5 * np.einsum("ea,ie->ai", np.einsum("fenm,fanm->ea", t2, lam2), Xov))
+        e2 = (_Pij(_Pab(np.einsum("ai,jb->abij", lam1, Xov)))
+              + _Pab(np.einsum("aeij,eb->abij", lam2, Xvv))
+              - _Pij(np.einsum("abim,jm->abij", lam2, Xoo))
+              - _Pab(np.einsum("aeij,em,mb->abij", lam2, t1, Xov))
+              - _Pij(np.einsum("abim,em,je->abij", lam2, t1, Xov)))
+        return e1, e2
+
+    def eta_eom(self, X, lam1, lam2):
+        """EOM-eta = eta + (lambda_2 . xi_1 on singles)  (S-Eq. 7)."""
+        e1, e2 = self.eta(X, lam1, lam2)
+        x1, _ = self.xi(X)
+        return e1 + np.einsum("abij,bj->ai", lam2, x1), e2
+
+    # ---- F.x.y as the second derivative of the Lagrangian (PAPER.md:861-879 is unusable) ----
+    def lagrangian(self, lam1, lam2, t1, t2):
+        e = ccsd.energy(self.I, t1, t2)
+        o1, o2 = ccsd.residual(self.I, t1, t2)
+        return e + dot(lam1, lam2, o1, o2)
+
+    def xFy(self, lam1, lam2, x1, x2, y1, y2):
+        """x.F.y = d2/da db [E + lambda.Omega](t + a x + b y)|0: mixed 4-point stencil + one Richardson step,
+        exact for a quartic."""
+        nt = max(np.sqrt(np.linalg.norm(self.t1) ** 2 + np.linalg.norm(self.t2) ** 2), 0.1)
+        hx = nt / max(np.sqrt(np.linalg.norm(x1) ** 2 + np.linalg.norm(x2) ** 2), 1e-300)
+        hy = nt / max(np.sqrt(np.linalg.norm(y1) ** 2 + np.linalg.norm(y2) ** 2), 1e-300)
+
+        def L(a, b):
+            return self.lagrangian(lam1, lam2, self.t1 + a * hx * x1 + b * hy * y1,
+                                   self.t2 + a * hx * x2 + b * hy * y2)
+
+        def D(h):
+            return (L(h, h) - L(h, -h) - L(-h, h) + L(-h, -h)) / (4 * h * h)
+
+        return (4 * D(0.5) - D(1.0)) / 3 / (hx * hy)
+
+    # ---- response equations and functions ---------------------------------------------------------------------
+    def solve_dense(self, A, xi1, xi2, z):
+        """t(z) = -(A - z)^-1 xi  (Eq. 19-21) by dense LU."""
+        n = A.shape[0]
+        t = np.linalg.solve(A - z * np.eye(n), -flat(xi1, xi2))
+        return unflat(t, self.o, self.v)
+
+    def solve_iterative(self, xi1, xi2, z, tol=1e-10, maxiter=200):
+        """Same by a plain preconditioned Krylov subspace method on CCLR.sigma (steps 1-5 of PAPER.md:952-967,
+        in the readings of DESIGN.md): trial space b, sigma_j = A b_j, reduced system
+        (b^H sigma - z b^H b) beta = -b^H xi, residual r = (sigma - z b) beta + xi, correction r/(z - D)."""
+        o, v = self.o, self.v
+        d = flat(self.D1 + 0j, self.D2 + 0j)
+        rhs = flat(xi1, xi2)
+        nrm_rhs = np.linalg.norm(rhs)
+        B, S = [], []
+        new = -rhs / (d - z)
+        for it in range(maxiter):
+            for _ in range(2):
+                for bj in B:
+                    new = new - bj * np.vdot(bj, new)
+            new = new / np.linalg.norm(new)
+            B.append(new)
+            S.append(flat(*self.sigma(*unflat(new, o, v))))
+            Bm, Sm = np.array(B).T, np.array(S).T
+            G = Bm.conj().T @ Sm - z * (Bm.conj().T @ Bm)
+            beta = np.linalg.solve(G, -Bm.conj().T @ rhs)
+            r = (Sm - z * Bm) @ beta + rhs
+            if np.linalg.norm(r) <= tol * nrm_rhs:
+                break
+            new = r / (z - d)
+        return unflat(Bm @ beta, o, v), dict(iterations=it + 1, residual=np.linalg.norm(r) / nrm_rhs)
+
+    def response_cc_cc(self, solve, X, Y, z, lam1, lam2):
+        """<<X;Y>>_z, symmetric CC-CC form, Eq. 15 + Eq. 17 in readings 7-8:
+        g(z) = eta^X.t^Y(z) + eta^Y.t^X(-z) + t^X(-z).F.t^Y(z);  <<X;Y>>_z = 1/2 [ g(z) + conj g(-conj z) ].
+        ``solve(xi1, xi2, z)`` returns t(z)."""
+        def g(zz):
+            tY = solve(*self.xi(Y), zz)
+            tX = solve(*self.xi(X), -zz)
+            return (dot(*self.eta(X, lam1, lam2), *tY) + dot(*self.eta(Y, lam1, lam2), *tX)
+                    + self.xFy(lam1, lam2, *tX, *tY))
+        return 0.5 * (g(z) + np.conj(g(-np.conj(z))))
+
+    def response_cc_ci(self, solve, X, Y, z, lam1, lam2):
+        """CC-CI (EOM-CC) form, Eq. 16: g(z) = EOMeta^X.t^Y(z) - (lam.t^X(-z))(lam.xi^Y) + (X<->Y, z<->-z)."""
+        def g(zz):
+            tY = solve(*self.xi(Y), zz)
+            tX = solve(*self.xi(X), -zz)
+            return (dot(*self.eta_eom(X, lam1, lam2), *tY) - dot(lam1, lam2, *tX) * dot(lam1, lam2, *self.xi(Y))
+                    + dot(*self.eta_eom(Y, lam1, lam2), *tX) - dot(lam1, lam2, *tY) * dot(lam1, lam2, *self.xi(X)))
+        return 0.5 * (g(z) + np.conj(g(-np.conj(z))))
+
+
+def dot(a1, a2, b1, b2):
+    """Bilinear (no conjugation) dot over unique elements: sum_ai a1 b1 + sum_{a<b,i<j} a2 b2 = ... + 1/4 full sum."""
+    return np.sum(a1 * b1) + 0.25 * np.sum(a2 * b2)
+
+
+def vdot(a1, a2, b1, b2):
+    """Sesquilinear dot over unique elements (used for projections / norms, Eq. 29)."""
+    return np.sum(np.conj(a1) * b1) + 0.25 * np.sum(np.conj(a2) * b2)
