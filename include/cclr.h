@@ -1,0 +1,141 @@
+/* cclr.h — C ABI of the B200-native CC-LR hot path (arXiv:2307.14296; PAPER.md).
+ *
+ * The library evaluates the CCSD Jacobian transform  sigma = (A - (omega + i*gamma)) X  of relativistic
+ * coupled-cluster linear response (Eq. 19, 183-187 Eq. 20-21; A = Hbar_N of PAPER.md:131 Eq. 14 and
+ * Table 1; programmable form: supplementary S-Eq. 11-12 PAPER.md:885-893 with the intermediates
+ * S-Eq. 15-28), solves the right response equations (A - z) t = -xi and
+ * contracts t with a perturbation vector (Eq. 15, 203).  Every step runs in hand-written sm_100a
+ * CUDA kernels of this library; there is no CPU fallback and no cuBLAS / cuTENSOR call.
+ *
+ * Conventions
+ *   - complex128, interleaved (re, im); every pointer is a DEVICE pointer unless its comment says "host".
+ *   - o occupied / v virtual spinors; i,j,m,n occupied, a,b,e,f virtual; n = o + v.
+ *   - <pq||rs> antisymmetrised, upper index = bra: V[pq,rs] = conj(V[rs,pq]).
+ *   - pair index P(p<q) = q(q-1)/2 + p; oo = o(o-1)/2, vv = v(v-1)/2.
+ *   - amplitudes x1[a][i] ([v][o], row-major), x2[P(a<b)][P(i<j)] ([vv][oo], row-major); nvec vectors are stored
+ *     vector-major ([nvec][v*o], [nvec][vv*oo]).  Antisymmetry is a property of the storage.
+ *   - all dots / norms run over UNIQUE elements (singles + a<b,i<j).
+ *   - every call returns 0 (CCLR_OK) or a negative error code; nothing aborts, throws or keeps global state.
+ *     Calls on one context are not re-entrant.  Work is enqueued on the context's stream; calls that return host
+ *     data (cclr_solve, cclr_property, *_host) synchronise that stream before returning.
+ */
+#ifndef CCLR_H
+#define CCLR_H
+#include <stddef.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct cclr_ctx cclr_ctx; /* opaque */
+typedef struct { double re, im; } cclr_c128;
+
+enum {
+  CCLR_OK = 0,
+  CCLR_EINVAL = -1,   /* bad argument (null pointer, o<2, v<2, nvec<1, ...) */
+  CCLR_ENOMEM = -2,   /* device allocation failed */
+  CCLR_ECUDA = -3,    /* a CUDA call or kernel failed; cclr_last_cuda_error() gives the CUDA code */
+  CCLR_ENOTCONV = -4, /* cclr_solve hit maxiter; the best iterate is still written and info filled */
+  CCLR_ENODEV = -5    /* no sm_100 device */
+};
+
+/* The six classes of MO integrals of PAPER.md:231, all <pq||rs>, packed over antisymmetric pairs. */
+typedef struct {
+  const cclr_c128 *oooo; /* [oo][oo]      <mn||ij>, m<n ; i<j   (Hermitian matrix)                     */
+  const cclr_c128 *ooov; /* [oo][o][v]    <mn||ie>, m<n                                                */
+  const cclr_c128 *oovv; /* [oo][vv]      <mn||ef>, m<n ; e<f                                          */
+  const cclr_c128 *ovvo; /* [o][v][v][o]  <mb||ej>                                                     */
+  const cclr_c128 *ovvv; /* [o][v][vv]    <mb||ef>, e<f                                                */
+  const cclr_c128 *vvvv; /* [vv][vv]      <ab||ef>, a<b ; e<f   (Hermitian matrix)                     */
+} cclr_eri_packed;
+
+/* flags for cclr_create */
+#define CCLR_ERI_INPLACE 1u /* the context adopts eri->vvvv and dresses it in place into W_vvvv (S-Eq. 22);
+                               the caller must keep the buffer alive until cclr_destroy and not read it again */
+
+/* Build the context: tau (S-Eq. 28), F_me/F_mi/F_ae (S-Eq. 15-17), W_oooo (S-Eq. 18
+ * :913), W_vvvv (S-Eq. 22 :929), W_ovvo and Wbar (S-Eq. 19, 23 :916, 932), W_ooov / W_vovv (S-Eq. 24-25 :934-936),
+ * W_ovoo (S-Eq. 20 :919) and W_vvvo (S-Eq. 21 :924) in the readings of DESIGN.md, and the orbital-energy
+ * denominators D1, D2.  fock is [n][n] row-major <p|f|q>.  t1 is [v][o], t2 is [vv][oo]; they need
+ * not be converged (sigma = dOmega/dt . x at any t).  Inputs are borrowed for the duration of the call (vvvv: see
+ * CCLR_ERI_INPLACE).  cuda_stream is a cudaStream_t (NULL = default stream); all later work of the context runs on it. */
+int cclr_create(int o, int v, const cclr_c128 *fock, const cclr_eri_packed *eri, const cclr_c128 *t1,
+                const cclr_c128 *t2, unsigned flags, void *cuda_stream, cclr_ctx **out);
+
+/* out = A x - (omega + i*gamma) x  for nvec trial vectors (S-Eq. 11-12; shift PAPER.md:163, 187).
+ * out1/out2 must not alias x1/x2. */
+int cclr_sigma(cclr_ctx *ctx, const cclr_c128 *x1, const cclr_c128 *x2, int nvec, double omega, double gamma,
+               cclr_c128 *out1, cclr_c128 *out2);
+
+typedef struct {
+  int iterations;       /* subspace expansions performed                                   */
+  int sigma_calls;      /* number of single-vector A.b products evaluated                  */
+  int subspace;         /* final subspace dimension                                        */
+  int converged;        /* 1 if every system met tol                                       */
+  double max_residual;  /* max over systems of ||(A-z)t+xi|| / ||xi|| (unique-element 2-norm) */
+  double seconds;       /* wall time of the call                                           */
+} cclr_solve_info;
+
+/* Solve (A - z_k) t = -xi_r, z_k = omegas[k] + i*gamma, for every right-hand side r < nrhs and shift k < nomega with
+ * one shared Krylov subspace (steps 1-5 of PAPER.md:952-967 in the readings of DESIGN.md; A is shift independent so
+ * one sigma serves every frequency).  Convergence: ||(A - z)t + xi||_2 <= tol * ||xi||_2 over unique elements.
+ * omegas (host) may be negative, gamma may be negative.  Outputs: t1_out [nrhs][nomega][v*o], t2_out
+ * [nrhs][nomega][vv*oo].  info (host) may be NULL. */
+int cclr_solve(cclr_ctx *ctx, const cclr_c128 *xi1, const cclr_c128 *xi2, int nrhs, const double *omegas,
+               int nomega, double gamma, double tol, int maxiter, cclr_c128 *t1_out, cclr_c128 *t2_out,
+               cclr_solve_info *info);
+
+/* result[k] = sum_ai eta1 x1_k + sum_{a<b,i<j} eta2 x2_k  (bilinear, no conjugation; PAPER.md:137 Eq. 15, :203) for
+ * nvec vectors x_k; result is a HOST array of nvec complex numbers. */
+int cclr_property(cclr_ctx *ctx, const cclr_c128 *eta1, const cclr_c128 *eta2, const cclr_c128 *x1,
+                  const cclr_c128 *x2, int nvec, cclr_c128 *result);
+
+void cclr_destroy(cclr_ctx *ctx);
+const char *cclr_strerror(int code);
+int cclr_last_cuda_error(void); /* CUDA error code behind the last CCLR_ECUDA of the calling thread */
+
+/* ---- host-buffer forms (end-to-end timing: host<->device copies are part of the call) ------------------------ */
+/* Same as cclr_sigma with HOST x1, x2, out1, out2 (pinned or pageable). */
+int cclr_sigma_host(cclr_ctx *ctx, const cclr_c128 *x1, const cclr_c128 *x2, int nvec, double omega, double gamma,
+                    cclr_c128 *out1, cclr_c128 *out2);
+
+/* ---- kernel-level entry points (unit tests, roofline measurement) ------------------------------------------------ */
+/* C[M][N] = alpha * opA(A)[M][K] * opB(B) + beta * C, complex128, row-major with leading dimensions in elements.
+ * A is always [M][K] (K contiguous).  b_is_kn = 0: B is [N][K] (K contiguous); 1: B is [K][N] (N contiguous).
+ * conj_a / conj_b conjugate the operand elementwise.  batch > 1 repeats with element strides sa, sb, sc.
+ * The 4M complex product runs on the FP64 tensor cores (DMMA) from TMA-staged shared-memory tiles.
+ * alpha, beta are host pointers to one complex number. */
+int cclr_zgemm(void *cuda_stream, int M, int N, int K, const cclr_c128 *alpha, const cclr_c128 *A, long lda,
+               int conj_a, const cclr_c128 *B, long ldb, int b_is_kn, int conj_b, const cclr_c128 *beta,
+               cclr_c128 *C, long ldc, int batch, long sa, long sb, long sc);
+
+/* The particle-particle ladder alone (term T11 of S-Eq. 12):
+ * out2[k][ab][ij] = sum_{e<f} W_vvvv[ab][ef] x2[k][ef][ij] for nvec vectors (no shift, no other term). */
+int cclr_ladder(cclr_ctx *ctx, const cclr_c128 *x2, int nvec, cclr_c128 *out2);
+
+/* The ring term alone (T8 of S-Eq. 12): out2[ab][ij] = P(ab)P(ij) sum_me W_mbej x2[ae][im], one vector. */
+int cclr_ring(cclr_ctx *ctx, const cclr_c128 *x2, cclr_c128 *out2);
+
+/* Copy a named intermediate to a device buffer of `capacity` elements (tests: block-by-block parity against the
+ * oracle).  Names and layouts: see DESIGN.md "Data layout".  Returns the element count, or a negative error. */
+long cclr_get_intermediate(cclr_ctx *ctx, const char *name, cclr_c128 *out, long capacity);
+
+/* Device bytes currently owned by the context. */
+size_t cclr_ctx_bytes(const cclr_ctx *ctx);
+
+/* Milliseconds (CUDA events on the context's stream) spent in each phase of the last cclr_sigma call:
+ * ms[0] total, ms[1] ladder GEMM, ms[2] ring GEMM, ms[3] other GEMMs, ms[4] layout / bandwidth kernels.
+ * Only filled when profiling was enabled with cclr_set_profiling(ctx, 1) (which adds event records). */
+int cclr_set_profiling(cclr_ctx *ctx, int on);
+int cclr_last_sigma_ms(const cclr_ctx *ctx, double ms[5]);
+
+/* FP64 tensor-core (DMMA m8n8k4) issue-rate probe: runs `iters` dependent-chain-free DMMA per warp on every SM
+ * and returns the measured TFLOP/s in *tflops (host).  This is the roofline denominator used by bench.py. */
+int cclr_fp64_tensor_peak(void *cuda_stream, int iters, double *tflops);
+
+/* Streaming-copy probe over `bytes` of device memory (read + write) -> GB/s in *gbs (host). */
+int cclr_hbm_copy_peak(void *cuda_stream, size_t bytes, double *gbs);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CCLR_H */

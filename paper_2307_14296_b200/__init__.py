@@ -1,0 +1,191 @@
+"""paper_2307_14296_b200 — thin Python binding of the B200-native CC-LR hot-path library (include/cclr.h).
+
+Same names as the C ABI; this layer only marshals arguments (torch tensors -> device pointers, the current CUDA
+stream).  Every step of the path runs in the library's own sm_100a kernels; PyTorch supplies device memory and
+streams only.  There is no CPU fallback: a missing ``libcclr.so`` or a non-CUDA tensor raises.
+"""
+import ctypes as C
+
+import torch
+
+from . import _lib
+from ._lib import CclrError, SolveInfo  # noqa: F401
+
+__all__ = ["Context", "cclr_create", "cclr_sigma", "cclr_solve", "cclr_property", "cclr_zgemm", "cclr_ladder",
+           "cclr_ring", "cclr_fp64_tensor_peak", "cclr_hbm_copy_peak", "CclrError"]
+
+
+def _dev(t, name, shape_numel=None):
+    if not isinstance(t, torch.Tensor) or not t.is_cuda or t.dtype != torch.complex128 or not t.is_contiguous():
+        raise TypeError("%s must be a contiguous complex128 CUDA tensor" % name)
+    if shape_numel is not None and t.numel() != shape_numel:
+        raise ValueError("%s has %d elements, expected %d" % (name, t.numel(), shape_numel))
+    return C.c_void_p(t.data_ptr())
+
+
+def _host(t, name, shape_numel=None):
+    if not isinstance(t, torch.Tensor) or t.is_cuda or t.dtype != torch.complex128 or not t.is_contiguous():
+        raise TypeError("%s must be a contiguous complex128 host tensor" % name)
+    if shape_numel is not None and t.numel() != shape_numel:
+        raise ValueError("%s has %d elements, expected %d" % (name, t.numel(), shape_numel))
+    return C.c_void_p(t.data_ptr())
+
+
+def _stream():
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+ERI_INPLACE = 1
+
+
+class Context:
+    """Owner of a ``cclr_ctx*``; created by :func:`cclr_create`."""
+
+    def __init__(self, handle, o, v, keep):
+        self.handle, self.o, self.v = handle, o, v
+        self._keep = keep  # buffers the C context may still reference (vvvv with ERI_INPLACE)
+        self.oo, self.vv = o * (o - 1) // 2, v * (v - 1) // 2
+        self.n1, self.n2 = o * v, self.oo * self.vv
+
+    def close(self):
+        if self.handle is not None:
+            _lib.load().cclr_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def bytes(self):
+        return int(_lib.load().cclr_ctx_bytes(self.handle))
+
+    def get_intermediate(self, name):
+        lib = _lib.load()
+        n = lib.cclr_get_intermediate(self.handle, name.encode(), None, 0)
+        if n < 0:
+            raise CclrError(int(n), "cclr_get_intermediate(%s)" % name)
+        out = torch.empty(int(n), dtype=torch.complex128, device="cuda")
+        m = lib.cclr_get_intermediate(self.handle, name.encode(), _dev(out, "out"), n)
+        if m < 0:
+            raise CclrError(int(m), "cclr_get_intermediate(%s)" % name)
+        torch.cuda.current_stream().synchronize()
+        return out
+
+    def set_profiling(self, on):
+        _lib.check(_lib.load().cclr_set_profiling(self.handle, int(bool(on))), "cclr_set_profiling")
+
+    def last_sigma_ms(self):
+        ms = (C.c_double * 5)()
+        _lib.check(_lib.load().cclr_last_sigma_ms(self.handle, ms), "cclr_last_sigma_ms")
+        return dict(zip(("total", "ladder", "ring", "other_gemm", "layout"), list(ms)))
+
+
+def cclr_create(o, v, fock, eri, t1, t2, flags=0):
+    """eri: dict with the six packed classes of include/cclr.h (device tensors)."""
+    lib = _lib.load()
+    oo, vv, n = o * (o - 1) // 2, v * (v - 1) // 2, o + v
+    sizes = dict(oooo=oo * oo, ooov=oo * o * v, oovv=oo * vv, ovvo=o * v * v * o, ovvv=o * v * vv, vvvv=vv * vv)
+    e = _lib.EriPacked()
+    for k, sz in sizes.items():
+        setattr(e, k, _dev(eri[k], "eri." + k, sz))
+    h = C.c_void_p()
+    rc = lib.cclr_create(o, v, _dev(fock, "fock", n * n), C.byref(e), _dev(t1, "t1", o * v), _dev(t2, "t2", vv * oo),
+                         flags, _stream(), C.byref(h))
+    _lib.check(rc, "cclr_create")
+    return Context(h, o, v, keep=[eri["vvvv"]] if flags & ERI_INPLACE else [])
+
+
+def cclr_sigma(ctx, x1, x2, omega=0.0, gamma=0.0, out1=None, out2=None):
+    """out = A x - (omega + i gamma) x.  x1: [nvec, v*o] (or [v*o]), x2: [nvec, vv*oo]."""
+    nvec = x1.numel() // ctx.n1
+    if out1 is None:
+        out1 = torch.empty_like(x1)
+    if out2 is None:
+        out2 = torch.empty_like(x2)
+    rc = _lib.load().cclr_sigma(ctx.handle, _dev(x1, "x1", nvec * ctx.n1), _dev(x2, "x2", nvec * ctx.n2), nvec,
+                                float(omega), float(gamma), _dev(out1, "out1", nvec * ctx.n1),
+                                _dev(out2, "out2", nvec * ctx.n2))
+    _lib.check(rc, "cclr_sigma")
+    return out1, out2
+
+
+def cclr_sigma_host(ctx, x1, x2, omega, gamma, out1, out2):
+    """Same through HOST tensors (copies inside the call)."""
+    nvec = x1.numel() // ctx.n1
+    rc = _lib.load().cclr_sigma_host(ctx.handle, _host(x1, "x1", nvec * ctx.n1), _host(x2, "x2", nvec * ctx.n2), nvec,
+                                     float(omega), float(gamma), _host(out1, "out1", nvec * ctx.n1),
+                                     _host(out2, "out2", nvec * ctx.n2))
+    _lib.check(rc, "cclr_sigma_host")
+    return out1, out2
+
+
+def cclr_solve(ctx, xi1, xi2, omegas, gamma=0.0, tol=1e-10, maxiter=200):
+    """Solve (A - (omega_k + i gamma)) t = -xi_r.  Returns t1 [nrhs, nomega, v*o], t2 [nrhs, nomega, vv*oo], info."""
+    nrhs = xi1.numel() // ctx.n1
+    om = (C.c_double * len(omegas))(*[float(w) for w in omegas])
+    t1 = torch.empty((nrhs, len(omegas), ctx.n1), dtype=torch.complex128, device="cuda")
+    t2 = torch.empty((nrhs, len(omegas), ctx.n2), dtype=torch.complex128, device="cuda")
+    info = SolveInfo()
+    rc = _lib.load().cclr_solve(ctx.handle, _dev(xi1, "xi1", nrhs * ctx.n1), _dev(xi2, "xi2", nrhs * ctx.n2), nrhs, om,
+                                len(omegas), float(gamma), float(tol), int(maxiter), _dev(t1, "t1"), _dev(t2, "t2"),
+                                C.byref(info))
+    if rc not in (0, -4):
+        _lib.check(rc, "cclr_solve")
+    return t1, t2, info
+
+
+def cclr_property(ctx, eta1, eta2, x1, x2):
+    """Bilinear eta . x_k for every vector k; returns a Python list of complex."""
+    nvec = x1.numel() // ctx.n1
+    res = (_lib.Complex * nvec)()
+    rc = _lib.load().cclr_property(ctx.handle, _dev(eta1, "eta1", ctx.n1), _dev(eta2, "eta2", ctx.n2),
+                                   _dev(x1, "x1", nvec * ctx.n1), _dev(x2, "x2", nvec * ctx.n2), nvec, res)
+    _lib.check(rc, "cclr_property")
+    return [complex(r.re, r.im) for r in res]
+
+
+def cclr_ladder(ctx, x2, out2=None):
+    nvec = x2.numel() // ctx.n2
+    if out2 is None:
+        out2 = torch.empty_like(x2)
+    _lib.check(_lib.load().cclr_ladder(ctx.handle, _dev(x2, "x2", nvec * ctx.n2), nvec, _dev(out2, "out2")),
+               "cclr_ladder")
+    return out2
+
+
+def cclr_ring(ctx, x2, out2=None):
+    if out2 is None:
+        out2 = torch.empty_like(x2)
+    _lib.check(_lib.load().cclr_ring(ctx.handle, _dev(x2, "x2", ctx.n2), _dev(out2, "out2", ctx.n2)), "cclr_ring")
+    return out2
+
+
+def cclr_zgemm(A, B, C_out, alpha=1.0, beta=0.0, conj_a=False, conj_b=False, b_is_kn=False, M=None, N=None, K=None,
+               lda=None, ldb=None, ldc=None, batch=1, sa=0, sb=0, sc=0):
+    """C = alpha opA(A) opB(B) + beta C on 2-D (or batched 3-D) row-major tensors; see include/cclr.h."""
+    if M is None:
+        M, K = A.shape[-2], A.shape[-1]
+        N = B.shape[-1] if b_is_kn else B.shape[-2]
+        lda, ldb, ldc = A.shape[-1], B.shape[-1], C_out.shape[-1]
+        if A.dim() == 3:
+            batch = A.shape[0]
+            sa, sb, sc = A.shape[1] * A.shape[2], B.shape[1] * B.shape[2], C_out.shape[1] * C_out.shape[2]
+    al, be = _lib.Complex(complex(alpha).real, complex(alpha).imag), _lib.Complex(complex(beta).real, complex(beta).imag)
+    rc = _lib.load().cclr_zgemm(_stream(), M, N, K, C.byref(al), _dev(A, "A"), lda, int(conj_a), _dev(B, "B"), ldb,
+                                int(b_is_kn), int(conj_b), C.byref(be), _dev(C_out, "C"), ldc, batch, sa, sb, sc)
+    _lib.check(rc, "cclr_zgemm")
+    return C_out
+
+
+def cclr_fp64_tensor_peak(iters=20000):
+    out = C.c_double()
+    _lib.check(_lib.load().cclr_fp64_tensor_peak(_stream(), iters, C.byref(out)), "cclr_fp64_tensor_peak")
+    return out.value
+
+
+def cclr_hbm_copy_peak(nbytes=4 << 30):
+    out = C.c_double()
+    _lib.check(_lib.load().cclr_hbm_copy_peak(_stream(), nbytes, C.byref(out)), "cclr_hbm_copy_peak")
+    return out.value

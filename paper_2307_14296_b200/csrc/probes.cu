@@ -1,0 +1,139 @@
+// probes.cu — roofline denominators measured by the library itself (include/cclr.h: cclr_fp64_tensor_peak,
+// cclr_hbm_copy_peak) and the C-ABI wrapper of the GEMM engine (cclr_zgemm).
+#include "common.cuh"
+#include "../../include/cclr.h"
+
+thread_local int g_last_cuda_error = 0;
+
+namespace {
+
+// 8 independent accumulator pairs per warp, no memory traffic: the DMMA issue-rate ceiling.
+__global__ void __launch_bounds__(256) dmma_peak_kernel(double *out, int iters, double seed) {
+  double c[16][2];
+  double a = seed * (threadIdx.x + 1), b = seed * 3.0;
+#pragma unroll
+  for (int j = 0; j < 16; ++j) c[j][0] = c[j][1] = 0.0;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int j = 0; j < 16; ++j)
+      asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                   : "+d"(c[j][0]), "+d"(c[j][1])
+                   : "d"(a), "d"(b));
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int j = 0; j < 16; ++j) s += c[j][0] + c[j][1];
+  out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+__global__ void copy_kernel(const double2 *__restrict__ src, double2 *__restrict__ dst, size_t n) {
+  for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+    dst[i] = src[i];
+}
+
+}  // namespace
+
+extern "C" int cclr_last_cuda_error(void) { return g_last_cuda_error; }
+
+extern "C" const char *cclr_strerror(int code) {
+  switch (code) {
+    case CCLR_OK: return "ok";
+    case CCLR_EINVAL: return "invalid argument";
+    case CCLR_ENOMEM: return "device allocation failed";
+    case CCLR_ECUDA: return "CUDA error (see cclr_last_cuda_error)";
+    case CCLR_ENOTCONV: return "solver did not converge within maxiter";
+    case CCLR_ENODEV: return "no sm_100 CUDA device";
+    default: return "unknown error";
+  }
+}
+
+extern "C" int cclr_fp64_tensor_peak(void *cuda_stream, int iters, double *tflops) {
+  if (!tflops || iters < 1) return CCLR_EINVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const int sms = zgemm_num_sms();
+  const int grid = sms * 2, threads = 256;
+  double *out = nullptr;
+  cudaError_t e = cudaMalloc(&out, sizeof(double) * grid * threads);
+  if (e != cudaSuccess) { g_last_cuda_error = e; return CCLR_ENOMEM; }
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0);
+  cudaEventCreate(&e1);
+  dmma_peak_kernel<<<grid, threads, 0, st>>>(out, iters / 4 + 1, 1e-9);  // warm-up
+  float best = 1e30f;
+  for (int rep = 0; rep < 3; ++rep) {
+    cudaEventRecord(e0, st);
+    dmma_peak_kernel<<<grid, threads, 0, st>>>(out, iters, 1e-9);
+    cudaEventRecord(e1, st);
+    e = cudaEventSynchronize(e1);
+    if (e != cudaSuccess) break;
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    if (ms < best) best = ms;
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(out);
+  if (e != cudaSuccess) { g_last_cuda_error = e; return CCLR_ECUDA; }
+  const double flops = (double)grid * (threads / 32) * (double)iters * 16.0 * (8.0 * 8.0 * 4.0 * 2.0);
+  *tflops = flops / (best * 1e-3) / 1e12;
+  return CCLR_OK;
+}
+
+extern "C" int cclr_hbm_copy_peak(void *cuda_stream, size_t bytes, double *gbs) {
+  if (!gbs || bytes < (1u << 20)) return CCLR_EINVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t n = bytes / 32;  // n double2 read + n double2 written = bytes
+  double2 *src = nullptr, *dst = nullptr;
+  cudaError_t e = cudaMalloc(&src, n * 16);
+  if (e == cudaSuccess) e = cudaMalloc(&dst, n * 16);
+  if (e != cudaSuccess) { cudaFree(src); g_last_cuda_error = e; return CCLR_ENOMEM; }
+  cudaMemsetAsync(src, 0, n * 16, st);
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0);
+  cudaEventCreate(&e1);
+  const int grid = zgemm_num_sms() * 16;
+  copy_kernel<<<grid, 512, 0, st>>>(src, dst, n);
+  float best = 1e30f;
+  for (int rep = 0; rep < 5; ++rep) {
+    cudaEventRecord(e0, st);
+    copy_kernel<<<grid, 512, 0, st>>>(src, dst, n);
+    cudaEventRecord(e1, st);
+    e = cudaEventSynchronize(e1);
+    if (e != cudaSuccess) break;
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    if (ms < best) best = ms;
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(src);
+  cudaFree(dst);
+  if (e != cudaSuccess) { g_last_cuda_error = e; return CCLR_ECUDA; }
+  *gbs = (double)(2 * n * 16) / (best * 1e-3) / 1e9;
+  return CCLR_OK;
+}
+
+extern "C" int cclr_zgemm(void *cuda_stream, int M, int N, int K, const cclr_c128 *alpha, const cclr_c128 *A,
+                          long lda, int conj_a, const cclr_c128 *B, long ldb, int b_is_kn, int conj_b,
+                          const cclr_c128 *beta, cclr_c128 *C, long ldc, int batch, long sa, long sb, long sc) {
+  if (!alpha || !beta || !C || M < 0 || N < 0 || K < 0 || batch < 1) return CCLR_EINVAL;
+  if (K > 0 && (!A || !B)) return CCLR_EINVAL;
+  if (lda < K || ldc < N || (b_is_kn ? ldb < N : ldb < K)) return CCLR_EINVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  // split-K workspace for this stand-alone entry point (the context keeps its own)
+  ZgemmWorkspace ws;
+  const long tiles = (long)((M + 127) / 128) * ((N + 63) / 64) * batch;
+  if (tiles < zgemm_num_sms() && K >= 256) {
+    ws.elems = (size_t)M * N * batch * 64;
+    if (cudaMalloc(&ws.buf, ws.elems * sizeof(c128)) != cudaSuccess) { ws.buf = nullptr; ws.elems = 0; cudaGetLastError(); }
+  }
+  cudaError_t e = zgemm(st, M, N, K, make_double2(alpha->re, alpha->im), (const c128 *)A, lda, conj_a != 0,
+                        (const c128 *)B, ldb, b_is_kn != 0, conj_b != 0, make_double2(beta->re, beta->im), (c128 *)C,
+                        ldc, batch, sa, sb, sc, ws.buf ? &ws : nullptr);
+  if (ws.buf) {
+    cudaStreamSynchronize(st);
+    cudaFree(ws.buf);
+  }
+  if (e != cudaSuccess) { g_last_cuda_error = e; return CCLR_ECUDA; }
+  return CCLR_OK;
+}
