@@ -52,6 +52,9 @@ typedef struct {
 #define CCLR_ERI_INPLACE 1u /* the context adopts eri->vvvv and dresses it in place into W_vvvv (S-Eq. 22);
                                the caller must keep the buffer alive until cclr_destroy and not read it again */
 
+#define CCLR_SMALL_CHUNKS 2u /* testing aid: run the chunked intermediate builds with chunks of 3 indices so that small
+                               inputs exercise several chunks and a ragged last one (results are unchanged) */
+
 /* Build the context: tau (S-Eq. 28), F_me/F_mi/F_ae (S-Eq. 15-17), W_oooo (S-Eq. 18
  * :913), W_vvvv (S-Eq. 22 :929), W_ovvo and Wbar (S-Eq. 19, 23 :916, 932), W_ooov / W_vovv (S-Eq. 24-25 :934-936),
  * W_ovoo (S-Eq. 20 :919) and W_vvvo (S-Eq. 21 :924) in the readings of DESIGN.md, and the orbital-energy
@@ -92,6 +95,7 @@ int cclr_property(cclr_ctx *ctx, const cclr_c128 *eta1, const cclr_c128 *eta2, c
 void cclr_destroy(cclr_ctx *ctx);
 const char *cclr_strerror(int code);
 int cclr_last_cuda_error(void); /* CUDA error code behind the last CCLR_ECUDA of the calling thread */
+const char *cclr_last_error_message(void); /* text of the last failure of the calling thread ("" if none) */
 
 /* ---- host-buffer forms (end-to-end timing: host<->device copies are part of the call) ------------------------ */
 /* Same as cclr_sigma with HOST x1, x2, out1, out2 (pinned or pageable). */

@@ -35,6 +35,7 @@ SIGNATURES = {
     "cclr_destroy": (None, [C.c_void_p]),
     "cclr_strerror": (C.c_char_p, [C.c_int]),
     "cclr_last_cuda_error": (C.c_int, []),
+    "cclr_last_error_message": (C.c_char_p, []),
     "cclr_sigma_host": (C.c_int, [C.c_void_p, c128_p, c128_p, C.c_int, C.c_double, C.c_double, c128_p, c128_p]),
     "cclr_zgemm": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.POINTER(Complex), c128_p, C.c_long, C.c_int,
                              c128_p, C.c_long, C.c_int, C.c_int, C.POINTER(Complex), c128_p, C.c_long, C.c_int,
@@ -72,6 +73,9 @@ class CclrError(RuntimeError):
         lib = load()
         msg = lib.cclr_strerror(code).decode()
         extra = " (cuda error %d)" % lib.cclr_last_cuda_error() if code == -3 else ""
+        detail = lib.cclr_last_error_message().decode()
+        if detail:
+            extra += ": " + detail
         super().__init__("%s: %s%s" % (where, msg, extra))
         self.code = code
 

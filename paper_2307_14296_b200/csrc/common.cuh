@@ -36,3 +36,49 @@ cudaError_t zgemm(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *
                   const c128 *B, long ldb, bool b_is_kn, bool conjB, c128 beta, c128 *C, long ldc, int batch = 1,
                   long sa = 0, long sb = 0, long sc = 0, const ZgemmWorkspace *ws = nullptr);
 int zgemm_num_sms();
+
+// ---- permute.cu: generic index-permutation / pair (un)packing / antisymmetrising gather-scatter kernel ---------
+// dst(iteration index) (+)= sum_k coef_k * sign_k * [conj] src_k(slots(letters)); see plans.inc for the semantics.
+constexpr int PERM_MAX_AXES = 6, PERM_MAX_SLOTS = 5, PERM_MAX_SRC = 10, PERM_MAX_LETTERS = 12;
+struct PermAxis {
+  int kind;      // 0 = plain letter, 1 = packed pair (p<q), 2 = unit extent
+  int ext;       // extent of the axis (pair axes: n(n-1)/2)
+  int l0, l1;    // letter ids written by this axis (l1 for pairs)
+  int off;       // global offset added to a plain letter (chunk loops)
+};
+struct PermSlot {
+  int kind;      // 0 = plain, 1 = antisymmetric pair, 2 = unit
+  int l0, l1;    // letter ids read by this slot
+  int sub;       // subtracted from a plain letter's global value (buffer declared over a chunk)
+  long stride;   // elements
+};
+struct PermOperand {
+  const c128 *ptr;
+  c128 coef;
+  int conj, nslot;
+  PermSlot slot[PERM_MAX_SLOTS];
+};
+struct PermArgs {
+  int naxis, nsrc, accumulate, cond;   // cond: 0 = all, 1 = only dst-pair p<q, 2 = only p>q
+  int cond_l0, cond_l1, dst_linear, ndslot;
+  long total;
+  c128 *dst;
+  PermAxis axis[PERM_MAX_AXES];
+  PermSlot dslot[PERM_MAX_SLOTS];
+  PermOperand src[PERM_MAX_SRC];
+};
+cudaError_t permute(cudaStream_t st, const PermArgs &args);
+
+// ---- vecops.cu: bandwidth kernels of the solver / property contraction ------------------------------------------
+// out[ia*nb+ib] = sum_i op(A[ia][i]) * B[ib][i]  (op = conj if conjA); diag != 0: out[ia] = sum_i op(A[ia][i]) B[ia][i].
+// partial is a device scratch of at least dots_scratch_elems(na*nb) complex numbers; out is a DEVICE array.
+size_t dots_scratch_elems(int npairs);
+cudaError_t multi_dot(cudaStream_t st, const c128 *A, long lda, int na, const c128 *B, long ldb, int nb, long n,
+                      bool conjA, bool diag, c128 *partial, c128 *out);
+// y[i] = beta * y[i] + sum_{j<m} coef[j] * V[j*ldv + i]   (coef: DEVICE array of m complex numbers)
+cudaError_t lincomb(cudaStream_t st, c128 *y, c128 beta, const c128 *coef, const c128 *V, long ldv, int m, long n);
+// y[i] = alpha * x[i] / (z - D[i])      (orbital-energy preconditioner)
+cudaError_t precondition(cudaStream_t st, c128 *y, const c128 *x, const double *D, c128 z, c128 alpha, long n);
+cudaError_t scale_vec(cudaStream_t st, c128 *y, c128 alpha, long n);
+// D1[a,i] = eps_a - eps_i, D2[(ab),(ij)] = eps_a + eps_b - eps_i - eps_j from the diagonal of fock ([n][n])
+cudaError_t denominators(cudaStream_t st, const c128 *fock, int o, int v, double *D);

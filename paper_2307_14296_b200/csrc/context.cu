@@ -1,0 +1,356 @@
+// context.cu — C ABI of the CC-LR hot path (include/cclr.h): cclr_create / cclr_sigma / cclr_property and the
+// kernel-level entry points.  Every arithmetic step is a launch of zgemm.cu (DMMA GEMM), permute.cu (layout) or
+// vecops.cu (bandwidth kernels); this file only orchestrates them through the plans of plans.inc.
+#include "context.cuh"
+#include "plans.inc"
+#include <cstring>
+#include <new>
+
+extern thread_local int g_last_cuda_error;   // probes.cu
+static thread_local std::string g_last_message;
+
+void cclr_set_error(const std::string &msg, cudaError_t e) {
+  g_last_message = msg;
+  if (e != cudaSuccess) g_last_cuda_error = (int)e;
+}
+
+int cclr_fail(const PlanError &e) {
+  cclr_set_error(e.what(), e.cuda);
+  cudaGetLastError();   // clear the sticky-free error state
+  return e.code;
+}
+
+extern "C" const char *cclr_last_error_message(void) { return g_last_message.c_str(); }
+
+namespace {
+
+// the ring term alone and the ladder alone, on the buffers of the sigma plan
+const char *const PLAN_LADDER = R"PLAN(
+@ladder
+gemm out2[(ab);(ij)] = 1 Wabef[(ab);(ef)] x2[(ef);(ij)] kn
+)PLAN";
+const char *const PLAN_RING = R"PLAN(
+@layout
+perm R[aiem] = 1 x2[(ae)(im)]
+@ring
+gemm Z[bj;ai] = 1 Wring[bj;em] R[ai;em] nk
+@layout
+perm out2[(ab)(ij)] = 1 Z[bjai] -1 Z[ajbi] -1 Z[biaj] 1 Z[aibj]
+)PLAN";
+
+void check(cudaError_t e, const char *where) {
+  if (e != cudaSuccess)
+    throw PlanError(e == cudaErrorMemoryAllocation ? CCLR_ENOMEM : CCLR_ECUDA, std::string(where) + ": " + cudaGetErrorString(e), e);
+}
+
+void run_ops(cclr_ctx *ctx, const std::vector<ResolvedOp> &ops, bool profile) {
+  if (!profile) {
+    for (const ResolvedOp &op : ops) ctx->plan->launch(op);
+    return;
+  }
+  while (ctx->events.size() < ops.size() + 1) {
+    cudaEvent_t ev;
+    check(cudaEventCreate(&ev), "cudaEventCreate");
+    ctx->events.push_back(ev);
+  }
+  check(cudaEventRecord(ctx->events[0], ctx->st), "cudaEventRecord");
+  for (size_t k = 0; k < ops.size(); ++k) {
+    ctx->plan->launch(ops[k]);
+    check(cudaEventRecord(ctx->events[k + 1], ctx->st), "cudaEventRecord");
+  }
+  check(cudaEventSynchronize(ctx->events[ops.size()]), "cudaEventSynchronize");
+  for (size_t k = 0; k < ops.size(); ++k) {
+    float ms = 0.f;
+    check(cudaEventElapsedTime(&ms, ctx->events[k], ctx->events[k + 1]), "cudaEventElapsedTime");
+    ctx->ms[0] += ms;
+    const int ph = ops[k].phase;
+    if (ph >= PHASE_LADDER && ph <= PHASE_LAYOUT) ctx->ms[ph] += ms;
+  }
+}
+
+void bind_vectors(cclr_ctx *ctx, const c128 *x1, const c128 *x2, c128 *out1, c128 *out2) {
+  ctx->plan->rebind(ctx->x1_id, const_cast<c128 *>(x1));
+  ctx->plan->rebind(ctx->x2_id, const_cast<c128 *>(x2));
+  ctx->plan->rebind(ctx->out1_id, out1);
+  ctx->plan->rebind(ctx->out2_id, out2);
+}
+
+void destroy(cclr_ctx *ctx) {
+  if (!ctx) return;
+  if (ctx->st) cudaStreamSynchronize(ctx->st);
+  delete ctx->plan;
+  if (ctx->ws.buf) cudaFree(ctx->ws.buf);
+  if (ctx->D) cudaFree(ctx->D);
+  if (ctx->dot_partial) cudaFree(ctx->dot_partial);
+  if (ctx->dot_out) cudaFree(ctx->dot_out);
+  if (ctx->host_stage) cudaFree(ctx->host_stage);
+  for (cudaEvent_t ev : ctx->events) cudaEventDestroy(ev);
+  delete ctx;
+}
+
+}  // namespace
+
+void cclr_sigma_one(cclr_ctx *ctx, const c128 *x1, const c128 *x2, c128 z, c128 *out1, c128 *out2, bool profile) {
+  bind_vectors(ctx, x1, x2, out1, out2);
+  ctx->plan->set_scalar(0, make_double2(-z.x, -z.y));
+  run_ops(ctx, ctx->sigma_ops, profile);
+}
+
+void cclr_ensure_dot_scratch(cclr_ctx *ctx, int npairs) {
+  if (npairs <= ctx->dot_pairs_cap) return;
+  check(cudaStreamSynchronize(ctx->st), "sync");
+  if (ctx->dot_partial) { cudaFree(ctx->dot_partial); ctx->extra_bytes -= dots_scratch_elems(ctx->dot_pairs_cap) * sizeof(c128); }
+  if (ctx->dot_out) { cudaFree(ctx->dot_out); ctx->extra_bytes -= (size_t)ctx->dot_pairs_cap * sizeof(c128); }
+  ctx->dot_partial = ctx->dot_out = nullptr;
+  ctx->dot_pairs_cap = 0;
+  int cap = 256;
+  while (cap < npairs) cap *= 2;
+  check(cudaMalloc(&ctx->dot_partial, dots_scratch_elems(cap) * sizeof(c128)), "cudaMalloc(dot scratch)");
+  check(cudaMalloc(&ctx->dot_out, (size_t)cap * sizeof(c128)), "cudaMalloc(dot out)");
+  ctx->dot_pairs_cap = cap;
+  ctx->extra_bytes += dots_scratch_elems(cap) * sizeof(c128) + (size_t)cap * sizeof(c128);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+extern "C" int cclr_create(int o, int v, const cclr_c128 *fock, const cclr_eri_packed *eri, const cclr_c128 *t1,
+                           const cclr_c128 *t2, unsigned flags, void *cuda_stream, cclr_ctx **out) {
+  if (!out) return CCLR_EINVAL;
+  *out = nullptr;
+  if (o < 2 || v < 2 || !fock || !eri || !t1 || !t2 || !eri->oooo || !eri->ooov || !eri->oovv || !eri->ovvo ||
+      !eri->ovvv || !eri->vvvv) {
+    cclr_set_error("cclr_create: null pointer or o < 2 or v < 2", cudaSuccess);
+    return CCLR_EINVAL;
+  }
+  int dev = 0;
+  cudaDeviceProp prop;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess || prop.major != 10) {
+    cudaGetLastError();
+    cclr_set_error("cclr_create: no sm_100 device", cudaSuccess);
+    return CCLR_ENODEV;
+  }
+  cclr_ctx *ctx = new (std::nothrow) cclr_ctx();
+  if (!ctx) return CCLR_ENOMEM;
+  try {
+    ctx->o = o; ctx->v = v;
+    ctx->oo = npair(o); ctx->vv = npair(v);
+    ctx->n1 = (long)o * v; ctx->n2 = ctx->oo * ctx->vv;
+    ctx->st = (cudaStream_t)cuda_stream;
+    ctx->plan = new Plan(o, v, ctx->st);
+    Plan &P = *ctx->plan;
+    if (flags & CCLR_SMALL_CHUNKS) P.set_chunk_override(3);
+
+    // split-K workspace of the GEMM engine
+    ctx->ws.elems = (size_t)8 << 20;
+    check(cudaMalloc(&ctx->ws.buf, ctx->ws.elems * sizeof(c128)), "cudaMalloc(split-K workspace)");
+    ctx->extra_bytes += ctx->ws.elems * sizeof(c128);
+    P.set_workspace(&ctx->ws);
+
+    // borrowed inputs
+    P.bind("oooo", "(mn)(ij)", (c128 *)eri->oooo);
+    P.bind("ooov", "(mn)ie", (c128 *)eri->ooov);
+    P.bind("oovv", "(mn)(ef)", (c128 *)eri->oovv);
+    P.bind("ovvo", "mbej", (c128 *)eri->ovvo);
+    P.bind("ovvv", "mb(ef)", (c128 *)eri->ovvv);
+    P.bind("t1", "ai", (c128 *)t1);
+    P.bind("t2", "(ab)(ij)", (c128 *)t2);
+
+    // Fock blocks f_oo, f_ov, f_vv out of the [n][n] matrix
+    const size_t nf = (size_t)o + v;
+    const c128 *F = (const c128 *)fock;
+    struct { const char *name, *spec; size_t r0, c0, rows, cols; } blocks[3] = {
+        {"foo", "mi", 0, 0, (size_t)o, (size_t)o}, {"fov", "me", 0, (size_t)o, (size_t)o, (size_t)v},
+        {"fvv", "ae", (size_t)o, (size_t)o, (size_t)v, (size_t)v}};
+    for (auto &b : blocks) {
+      c128 *p = nullptr;
+      check(cudaMalloc(&p, b.rows * b.cols * sizeof(c128)), "cudaMalloc(fock block)");
+      P.adopt(b.name, b.spec, p, BUF_TEMP, true);
+      check(cudaMemcpy2DAsync(p, b.cols * sizeof(c128), F + b.r0 * nf + b.c0, nf * sizeof(c128), b.cols * sizeof(c128),
+                              b.rows, cudaMemcpyDeviceToDevice, ctx->st),
+            "copy fock block");
+    }
+
+    // <ab||ef>: adopted and dressed in place, or copied
+    const size_t nvvvv = (size_t)ctx->vv * (size_t)ctx->vv;
+    if (flags & CCLR_ERI_INPLACE) {
+      P.adopt("Wabef", "(ab)(ef)", (c128 *)eri->vvvv, BUF_PERSIST, false);
+    } else {
+      c128 *p = nullptr;
+      check(cudaMalloc(&p, nvvvv * sizeof(c128)), "cudaMalloc(Wabef)");
+      P.adopt("Wabef", "(ab)(ef)", p, BUF_PERSIST, true);
+      check(cudaMemcpyAsync(p, eri->vvvv, nvvvv * sizeof(c128), cudaMemcpyDeviceToDevice, ctx->st), "copy vvvv");
+    }
+
+    P.execute(CCLR_PLAN_CREATE);
+    P.free_class(BUF_TEMP);
+
+    check(cudaMalloc(&ctx->D, (size_t)(ctx->n1 + ctx->n2) * sizeof(double)), "cudaMalloc(D)");
+    ctx->extra_bytes += (size_t)(ctx->n1 + ctx->n2) * sizeof(double);
+    check(denominators(ctx->st, F, o, v, ctx->D), "denominators");
+
+    // the borrowed inputs end here
+    check(cudaStreamSynchronize(ctx->st), "cclr_create sync");
+    for (const char *name : {"oooo", "ooov", "oovv", "ovvo", "ovvv", "t1", "t2"}) P.rebind(P.find(name), nullptr);
+
+    // resolve the sigma plan once (allocates its workspace)
+    P.bind("x1", "ai", nullptr);
+    P.bind("x2", "(ab)(ij)", nullptr);
+    P.bind("out1", "ai", nullptr);
+    P.bind("out2", "(ab)(ij)", nullptr);
+    ctx->x1_id = P.find("x1"); ctx->x2_id = P.find("x2");
+    ctx->out1_id = P.find("out1"); ctx->out2_id = P.find("out2");
+    P.compile(CCLR_PLAN_SIGMA, ctx->sigma_ops);
+    P.compile(PLAN_LADDER, ctx->ladder_ops);
+    P.compile(PLAN_RING, ctx->ring_ops);
+    cclr_ensure_dot_scratch(ctx, 256);
+  } catch (const PlanError &e) {
+    destroy(ctx);
+    return cclr_fail(e);
+  } catch (const std::exception &e) {
+    destroy(ctx);
+    cclr_set_error(e.what(), cudaSuccess);
+    return CCLR_EINVAL;
+  }
+  *out = ctx;
+  return CCLR_OK;
+}
+
+extern "C" void cclr_destroy(cclr_ctx *ctx) { destroy(ctx); }
+
+extern "C" size_t cclr_ctx_bytes(const cclr_ctx *ctx) {
+  return ctx ? ctx->plan->owned_bytes() + ctx->extra_bytes : 0;
+}
+
+extern "C" int cclr_sigma(cclr_ctx *ctx, const cclr_c128 *x1, const cclr_c128 *x2, int nvec, double omega,
+                          double gamma, cclr_c128 *out1, cclr_c128 *out2) {
+  if (!ctx || !x1 || !x2 || !out1 || !out2 || nvec < 1 || x1 == out1 || x2 == out2) {
+    cclr_set_error("cclr_sigma: null pointer, nvec < 1 or aliased output", cudaSuccess);
+    return CCLR_EINVAL;
+  }
+  try {
+    if (ctx->profiling)
+      for (double &m : ctx->ms) m = 0.0;
+    for (int k = 0; k < nvec; ++k)
+      cclr_sigma_one(ctx, (const c128 *)x1 + (size_t)k * ctx->n1, (const c128 *)x2 + (size_t)k * ctx->n2,
+                     make_double2(omega, gamma), (c128 *)out1 + (size_t)k * ctx->n1, (c128 *)out2 + (size_t)k * ctx->n2,
+                     ctx->profiling);
+  } catch (const PlanError &e) {
+    return cclr_fail(e);
+  }
+  return CCLR_OK;
+}
+
+extern "C" int cclr_sigma_host(cclr_ctx *ctx, const cclr_c128 *x1, const cclr_c128 *x2, int nvec, double omega,
+                               double gamma, cclr_c128 *out1, cclr_c128 *out2) {
+  if (!ctx || !x1 || !x2 || !out1 || !out2 || nvec < 1) {
+    cclr_set_error("cclr_sigma_host: null pointer or nvec < 1", cudaSuccess);
+    return CCLR_EINVAL;
+  }
+  try {
+    const size_t n = (size_t)(ctx->n1 + ctx->n2), need = 2 * n * (size_t)nvec;
+    if (ctx->host_stage_elems < need) {
+      check(cudaStreamSynchronize(ctx->st), "sync");
+      if (ctx->host_stage) { cudaFree(ctx->host_stage); ctx->extra_bytes -= ctx->host_stage_elems * sizeof(c128); }
+      ctx->host_stage = nullptr;
+      ctx->host_stage_elems = 0;
+      check(cudaMalloc(&ctx->host_stage, need * sizeof(c128)), "cudaMalloc(host staging)");
+      ctx->host_stage_elems = need;
+      ctx->extra_bytes += need * sizeof(c128);
+    }
+    c128 *dx1 = ctx->host_stage, *dx2 = dx1 + (size_t)nvec * ctx->n1;
+    c128 *do1 = dx2 + (size_t)nvec * ctx->n2, *do2 = do1 + (size_t)nvec * ctx->n1;
+    check(cudaMemcpyAsync(dx1, x1, (size_t)nvec * ctx->n1 * sizeof(c128), cudaMemcpyHostToDevice, ctx->st), "H2D x1");
+    check(cudaMemcpyAsync(dx2, x2, (size_t)nvec * ctx->n2 * sizeof(c128), cudaMemcpyHostToDevice, ctx->st), "H2D x2");
+    const int rc = cclr_sigma(ctx, (cclr_c128 *)dx1, (cclr_c128 *)dx2, nvec, omega, gamma, (cclr_c128 *)do1, (cclr_c128 *)do2);
+    if (rc != CCLR_OK) return rc;
+    check(cudaMemcpyAsync(out1, do1, (size_t)nvec * ctx->n1 * sizeof(c128), cudaMemcpyDeviceToHost, ctx->st), "D2H out1");
+    check(cudaMemcpyAsync(out2, do2, (size_t)nvec * ctx->n2 * sizeof(c128), cudaMemcpyDeviceToHost, ctx->st), "D2H out2");
+    check(cudaStreamSynchronize(ctx->st), "cclr_sigma_host sync");
+  } catch (const PlanError &e) {
+    return cclr_fail(e);
+  }
+  return CCLR_OK;
+}
+
+extern "C" int cclr_ladder(cclr_ctx *ctx, const cclr_c128 *x2, int nvec, cclr_c128 *out2) {
+  if (!ctx || !x2 || !out2 || nvec < 1 || x2 == out2) return CCLR_EINVAL;
+  try {
+    for (int k = 0; k < nvec; ++k) {
+      bind_vectors(ctx, nullptr, (const c128 *)x2 + (size_t)k * ctx->n2, nullptr, (c128 *)out2 + (size_t)k * ctx->n2);
+      run_ops(ctx, ctx->ladder_ops, false);
+    }
+  } catch (const PlanError &e) {
+    return cclr_fail(e);
+  }
+  return CCLR_OK;
+}
+
+extern "C" int cclr_ring(cclr_ctx *ctx, const cclr_c128 *x2, cclr_c128 *out2) {
+  if (!ctx || !x2 || !out2 || x2 == out2) return CCLR_EINVAL;
+  try {
+    bind_vectors(ctx, nullptr, (const c128 *)x2, nullptr, (c128 *)out2);
+    run_ops(ctx, ctx->ring_ops, false);
+  } catch (const PlanError &e) {
+    return cclr_fail(e);
+  }
+  return CCLR_OK;
+}
+
+extern "C" long cclr_get_intermediate(cclr_ctx *ctx, const char *name, cclr_c128 *out, long capacity) {
+  if (!ctx || !name) return CCLR_EINVAL;
+  long n = 0;
+  const void *src = nullptr;
+  const int id = ctx->plan->find(name);
+  if (id >= 0 && ctx->plan->buf(id).ptr && ctx->plan->buf(id).cls != BUF_EXTERNAL) {
+    n = (long)ctx->plan->buf_elems(id);
+    src = ctx->plan->buf(id).ptr;
+  } else if (id >= 0 && std::strcmp(name, "Wabef") == 0 && ctx->plan->buf(id).ptr) {
+    n = (long)ctx->plan->buf_elems(id);
+    src = ctx->plan->buf(id).ptr;
+  }
+  if (!src) {
+    cclr_set_error(std::string("cclr_get_intermediate: unknown intermediate ") + name, cudaSuccess);
+    return CCLR_EINVAL;
+  }
+  if (!out) return n;
+  if (capacity < n) return CCLR_EINVAL;
+  cudaError_t e = cudaMemcpyAsync(out, src, (size_t)n * sizeof(c128), cudaMemcpyDeviceToDevice, ctx->st);
+  if (e != cudaSuccess) { cclr_set_error("cclr_get_intermediate copy", e); return CCLR_ECUDA; }
+  return n;
+}
+
+extern "C" int cclr_set_profiling(cclr_ctx *ctx, int on) {
+  if (!ctx) return CCLR_EINVAL;
+  ctx->profiling = on != 0;
+  return CCLR_OK;
+}
+
+extern "C" int cclr_last_sigma_ms(const cclr_ctx *ctx, double ms[5]) {
+  if (!ctx || !ms) return CCLR_EINVAL;
+  for (int k = 0; k < 5; ++k) ms[k] = ctx->ms[k];
+  return CCLR_OK;
+}
+
+extern "C" int cclr_property(cclr_ctx *ctx, const cclr_c128 *eta1, const cclr_c128 *eta2, const cclr_c128 *x1,
+                             const cclr_c128 *x2, int nvec, cclr_c128 *result) {
+  if (!ctx || !eta1 || !eta2 || !x1 || !x2 || !result || nvec < 1 || nvec > 16384) return CCLR_EINVAL;
+  try {
+    cclr_ensure_dot_scratch(ctx, 2 * nvec);
+    // bilinear dots over unique elements: singles then packed doubles (Eq. 15)
+    check(multi_dot(ctx->st, (const c128 *)eta1, ctx->n1, 1, (const c128 *)x1, ctx->n1, nvec, ctx->n1, false, false,
+                    ctx->dot_partial, ctx->dot_out),
+          "multi_dot(singles)");
+    check(multi_dot(ctx->st, (const c128 *)eta2, ctx->n2, 1, (const c128 *)x2, ctx->n2, nvec, ctx->n2, false, false,
+                    ctx->dot_partial + dots_scratch_elems(nvec), ctx->dot_out + nvec),
+          "multi_dot(doubles)");
+    std::vector<c128> host(2 * (size_t)nvec);
+    check(cudaMemcpyAsync(host.data(), ctx->dot_out, host.size() * sizeof(c128), cudaMemcpyDeviceToHost, ctx->st), "D2H dots");
+    check(cudaStreamSynchronize(ctx->st), "cclr_property sync");
+    for (int k = 0; k < nvec; ++k) {
+      result[k].re = host[k].x + host[nvec + k].x;
+      result[k].im = host[k].y + host[nvec + k].y;
+    }
+  } catch (const PlanError &e) {
+    return cclr_fail(e);
+  }
+  return CCLR_OK;
+}

@@ -1,0 +1,36 @@
+// context.cuh — the opaque cclr_ctx of include/cclr.h (shared by context.cu and solver.cu).
+#pragma once
+#include "plan.cuh"
+#include "../../include/cclr.h"
+#include <string>
+#include <vector>
+
+struct cclr_ctx {
+  int o = 0, v = 0;
+  long oo = 0, vv = 0, n1 = 0, n2 = 0;
+  cudaStream_t st = nullptr;
+  Plan *plan = nullptr;
+  ZgemmWorkspace ws;
+  std::vector<ResolvedOp> sigma_ops, ladder_ops, ring_ops;
+  int x1_id = -1, x2_id = -1, out1_id = -1, out2_id = -1;
+  double *D = nullptr;            // orbital-energy denominators over unique elements, [n1 + n2]
+  // small device scratch for dot products (vecops.cu)
+  c128 *dot_partial = nullptr, *dot_out = nullptr;
+  int dot_pairs_cap = 0;
+  // profiling of the last cclr_sigma call
+  bool profiling = false;
+  double ms[5] = {0, 0, 0, 0, 0};
+  std::vector<cudaEvent_t> events;
+  // staging buffers of cclr_sigma_host
+  c128 *host_stage = nullptr;
+  size_t host_stage_elems = 0;
+  size_t extra_bytes = 0;         // device bytes owned outside the plan
+};
+
+// thread-local error reporting (context.cu)
+void cclr_set_error(const std::string &msg, cudaError_t e);
+int cclr_fail(const PlanError &e);
+
+// out = A x for one vector on the context's stream (no shift when z == 0); throws PlanError
+void cclr_sigma_one(cclr_ctx *ctx, const c128 *x1, const c128 *x2, c128 z, c128 *out1, c128 *out2, bool profile);
+void cclr_ensure_dot_scratch(cclr_ctx *ctx, int npairs);

@@ -1,0 +1,235 @@
+"""GPU parity tests: the CUDA path (through the C ABI of include/cclr.h and its ctypes binding) against the CPU
+oracle on the same seeded synthetic inputs, element by element.
+
+Tolerances (BASELINE.json north_star): sigma vectors ||gpu - oracle||_2 / ||oracle||_2 <= 1e-10
+per vector, singles and doubles separately; intermediates max-norm 1e-11 relative; response functions 1e-8.
+"""
+import numpy as np
+import pytest
+import torch
+
+import synth
+from oracle import ccsd, cclr, packing
+
+pytestmark = pytest.mark.gpu
+
+
+def _lib():
+    import paper_2307_14296_b200 as cc
+    return cc
+
+
+def make_system(o, v, seed=0, t_scale=None, diag_fock=False, eri_scale=None):
+    """Synthetic packed inputs (host torch tensors) + the oracle objects built from the same numbers."""
+    eri = synth.eri_packed(o, v, seed=seed, scale=eri_scale)
+    f = synth.fock(o, v, seed=seed)
+    if not diag_fock:
+        f = f + 0.05 * torch.from_numpy(synth.hermitian_operator(o + v, seed, 7))
+    ts = synth.sigma_v(v) * 2 if t_scale is None else t_scale
+    t1, t2 = synth.amplitudes(o, v, seed=seed, scale=ts)
+    full = packing.unpack_eri(o, v, {k: x.numpy() for k, x in eri.items()})
+    ints = ccsd.Integrals(o, v, f.numpy(), **full)
+    t1f, t2f = packing.unpack_amplitudes(t1[0].numpy(), t2[0].numpy(), o, v)
+    return dict(o=o, v=v, eri=eri, fock=f, t1=t1[0], t2=t2[0], ints=ints, t1f=t1f, t2f=t2f)
+
+
+def gpu_context(s, flags=0):
+    cc = _lib()
+    dev = {k: x.cuda() for k, x in s["eri"].items()}
+    ctx = cc.cclr_create(s["o"], s["v"], s["fock"].contiguous().cuda(), dev, s["t1"].cuda(), s["t2"].cuda(), flags)
+    return ctx
+
+
+def rel(a, b):
+    return np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("M,N,K,kn,ca,cb,beta", [
+    (1, 1, 1, False, False, False, 0.0), (5, 3, 2, True, True, False, 0.5), (128, 64, 16, False, False, False, 0.0),
+    (129, 65, 17, False, False, True, 1.0), (200, 150, 333, True, False, False, 0.0), (37, 190, 190, True, True, True, -1.0),
+    (300, 34, 5000, False, False, False, 1.0),     # tall K -> split-K path
+    (20, 1, 80, False, False, False, 1.0),         # GEMV shapes of the singles terms
+    (1000, 9, 34, True, False, False, 0.0),
+])
+def test_zgemm_matches_numpy(M, N, K, kn, ca, cb, beta):
+    cc = _lib()
+    rng = np.random.default_rng(M * 1000 + N * 10 + K)
+    A = rng.normal(size=(M, K)) + 1j * rng.normal(size=(M, K))
+    B = rng.normal(size=(K, N) if kn else (N, K)) + 1j * rng.normal(size=(K, N) if kn else (N, K))
+    C0 = rng.normal(size=(M, N)) + 1j * rng.normal(size=(M, N))
+    alpha = 0.7 - 0.3j
+    opA = A.conj() if ca else A
+    opB = B.conj() if cb else B
+    ref = alpha * (opA @ (opB if kn else opB.T)) + beta * C0
+    Cd = torch.from_numpy(C0.copy()).cuda()
+    cc.cclr_zgemm(torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda(), Cd, alpha=alpha, beta=beta, conj_a=ca,
+                  conj_b=cb, b_is_kn=kn)
+    torch.cuda.synchronize()
+    assert rel(Cd.cpu().numpy(), ref) < 1e-13
+
+
+def test_zgemm_batched_and_strided():
+    cc = _lib()
+    rng = np.random.default_rng(5)
+    A = rng.normal(size=(3, 70, 40)) + 1j * rng.normal(size=(3, 70, 40))
+    B = rng.normal(size=(3, 40, 50)) + 1j * rng.normal(size=(3, 40, 50))
+    C = torch.zeros((3, 70, 50), dtype=torch.complex128, device="cuda")
+    cc.cclr_zgemm(torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda(), C, b_is_kn=True)
+    torch.cuda.synchronize()
+    assert rel(C.cpu().numpy(), A @ B) < 1e-13
+
+
+# ---------------------------------------------------------------------------------------------------------------
+INTERMEDIATES = {
+    # name -> oracle array in the library's layout
+    "Fme": lambda c: c.Fme, "Fmi": lambda c: c.Fmi, "Fae": lambda c: c.Fae,
+    "Wmnij": lambda c: packing.pack_pair_axes(packing.pack_pair_axes(c.Wmnij, 2), 0),
+    "Wabef": lambda c: packing.pack_pair_axes(packing.pack_pair_axes(c.Wabef, 2), 0),
+    "Wring": lambda c: c.Wmbej.transpose(1, 3, 2, 0),
+    "Wie": lambda c: packing.pack_pair_axes(c.Wmnie, 0).transpose(1, 2, 0),
+    "Wnjem": lambda c: c.Wmnie.transpose(0, 2, 3, 1),
+    "Wamef": lambda c: packing.pack_pair_axes(c.Wamef, 2),
+    "Wx": lambda c: c.Wamef.transpose(0, 2, 3, 1),
+    "Wmbij": lambda c: packing.pack_pair_axes(c.Wmbij, 2),
+    "Wabej": lambda c: packing.pack_pair_axes(c.Wabej, 0).transpose(0, 2, 1),
+}
+
+
+@pytest.mark.parametrize("o,v,flags", [(3, 5, 0), (4, 7, 2), (4, 20, 0), (5, 33, 2)])
+def test_create_intermediates_match_oracle(o, v, flags):
+    s = make_system(o, v, seed=o * 100 + v)
+    ctx = gpu_context(s, flags)
+    c = cclr.CCLR(s["ints"], s["t1f"], s["t2f"])
+    bad = []
+    for name, fn in INTERMEDIATES.items():
+        got = ctx.get_intermediate(name).cpu().numpy()
+        want = np.ascontiguousarray(fn(c)).reshape(-1)
+        err = np.abs(got - want).max() / max(1.0, np.abs(want).max())
+        if not err < 1e-11:
+            bad.append((name, err))
+    ctx.close()
+    assert not bad, bad
+
+
+@pytest.mark.parametrize("o,v,flags,nvec", [(3, 5, 0, 1), (4, 7, 2, 2), (4, 20, 0, 3), (6, 40, 0, 1)])
+def test_sigma_matches_oracle(o, v, flags, nvec):
+    cc = _lib()
+    s = make_system(o, v, seed=o * 100 + v + 1)
+    ctx = gpu_context(s, flags)
+    c = cclr.CCLR(s["ints"], s["t1f"], s["t2f"])
+    x1, x2 = synth.amplitudes(o, v, seed=3, cls1="x1", cls2="x2", nvec=nvec)
+    for (w, g) in [(0.0, 0.0), (0.0773, 0.0045)]:
+        o1, o2 = cc.cclr_sigma(ctx, x1.cuda(), x2.cuda(), w, g)
+        torch.cuda.synchronize()
+        for k in range(nvec):
+            r1, r2 = c.sigma(*packing.unpack_amplitudes(x1[k].numpy(), x2[k].numpy(), o, v), z=w + 1j * g)
+            r1p, r2p = packing.pack_amplitudes(r1, r2)
+            assert rel(o1[k].cpu().numpy(), r1p.reshape(-1)) < 1e-10, ("sigma1", k, w, g)
+            assert rel(o2[k].cpu().numpy(), r2p.reshape(-1)) < 1e-10, ("sigma2", k, w, g)
+    ctx.close()
+
+
+def test_ladder_and_ring_terms_match_oracle():
+    cc = _lib()
+    o, v = 4, 20
+    s = make_system(o, v, seed=11)
+    ctx = gpu_context(s)
+    c = cclr.CCLR(s["ints"], s["t1f"], s["t2f"])
+    x1, x2 = synth.amplitudes(o, v, seed=4, cls1="x1", cls2="x2", nvec=2)
+    lad = cc.cclr_ladder(ctx, x2.cuda()).cpu().numpy()
+    ring = cc.cclr_ring(ctx, x2[0].contiguous().cuda()).cpu().numpy()
+    for k in range(2):
+        _, r2 = packing.unpack_amplitudes(x1[k].numpy(), x2[k].numpy(), o, v)
+        want = 0.5 * np.einsum("abef,efij->abij", c.Wabef, r2)                       # T11
+        assert rel(lad[k], packing.pack_amplitudes(x1[k].numpy(), want)[1].reshape(-1)) < 1e-12
+    _, r2 = packing.unpack_amplitudes(x1[0].numpy(), x2[0].numpy(), o, v)
+    t8 = np.einsum("mbej,aeim->abij", c.Wmbej, r2)                                   # T8
+    t8 = t8 - t8.transpose(1, 0, 2, 3)
+    t8 = t8 - t8.transpose(0, 1, 3, 2)
+    assert rel(ring, packing.pack_amplitudes(x1[0].numpy(), t8)[1].reshape(-1)) < 1e-12
+    ctx.close()
+
+
+def test_sigma_host_entry_point_and_inplace_vvvv():
+    cc = _lib()
+    o, v = 4, 20
+    s = make_system(o, v, seed=12)
+    dev = {k: x.cuda() for k, x in s["eri"].items()}
+    ctx = cc.cclr_create(o, v, s["fock"].contiguous().cuda(), dev, s["t1"].cuda(), s["t2"].cuda(), cc.ERI_INPLACE)
+    c = cclr.CCLR(s["ints"], s["t1f"], s["t2f"])
+    x1, x2 = synth.amplitudes(o, v, seed=5, cls1="x1", cls2="x2", nvec=2)
+    o1, o2 = torch.empty_like(x1), torch.empty_like(x2)
+    cc.cclr_sigma_host(ctx, x1, x2, 0.1, -0.02, o1, o2)
+    for k in range(2):
+        r1, r2 = packing.pack_amplitudes(*c.sigma(*packing.unpack_amplitudes(x1[k].numpy(), x2[k].numpy(), o, v), z=0.1 - 0.02j))
+        assert rel(o1[k].numpy(), r1.reshape(-1)) < 1e-10 and rel(o2[k].numpy(), r2.reshape(-1)) < 1e-10
+    ctx.close()
+
+
+def test_property_is_bilinear_dot_over_unique_elements():
+    cc = _lib()
+    o, v = 4, 20
+    s = make_system(o, v, seed=13)
+    ctx = gpu_context(s)
+    e1, e2 = synth.amplitudes(o, v, seed=6, cls1="x1", cls2="x2")
+    x1, x2 = synth.amplitudes(o, v, seed=7, cls1="x1", cls2="x2", nvec=3)
+    got = cc.cclr_property(ctx, e1[0].cuda(), e2[0].cuda(), x1.cuda(), x2.cuda())
+    for k in range(3):
+        want = (e1[0].numpy() * x1[k].numpy()).sum() + (e2[0].numpy() * x2[k].numpy()).sum()
+        assert abs(got[k] - want) < 1e-12 * abs(want)
+    ctx.close()
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# invariants of the GPU path alone (no oracle): special cases with closed forms
+def test_gpu_V_zero_gives_orbital_energy_diagonal():
+    cc = _lib()
+    o, v = 5, 24
+    s = make_system(o, v, seed=14, diag_fock=True, eri_scale=0.0)
+    ctx = gpu_context(s)
+    x1, x2 = synth.amplitudes(o, v, seed=8, cls1="x1", cls2="x2")
+    o1, o2 = cc.cclr_sigma(ctx, x1.cuda(), x2.cuda())
+    eps = s["fock"].numpy().diagonal().real
+    eo, ev = eps[:o], eps[o:]
+    D1 = (ev[:, None] - eo[None, :]).reshape(-1)
+    pa, pb = packing.pairs(v)
+    pi, pj = packing.pairs(o)
+    D2 = ((ev[pa] + ev[pb])[:, None] - (eo[pi] + eo[pj])[None, :]).reshape(-1)
+    assert rel(o1[0].cpu().numpy(), D1 * x1[0].numpy()) < 1e-13
+    assert rel(o2[0].cpu().numpy(), D2 * x2[0].numpy()) < 1e-13
+    ctx.close()
+
+
+def test_gpu_T_zero_jacobian_is_hermitian():
+    cc = _lib()
+    o, v = 4, 12
+    s = make_system(o, v, seed=15, diag_fock=True, t_scale=0.0)
+    ctx = gpu_context(s)
+    x1, x2 = synth.amplitudes(o, v, seed=9, cls1="x1", cls2="x2", nvec=2)
+    o1, o2 = cc.cclr_sigma(ctx, x1.cuda(), x2.cuda())
+    X = torch.cat([x1, x2], dim=1).numpy()
+    S = torch.cat([o1.cpu(), o2.cpu()], dim=1).numpy()
+    lhs, rhs = np.vdot(X[0], S[1]), np.conj(np.vdot(X[1], S[0]))      # x^H A y = conj(y^H A x)
+    assert abs(lhs - rhs) < 1e-12 * abs(lhs)
+    ctx.close()
+
+
+def test_gpu_linearity_and_shift_identity():
+    cc = _lib()
+    o, v = 4, 20
+    s = make_system(o, v, seed=16)
+    ctx = gpu_context(s)
+    x1, x2 = synth.amplitudes(o, v, seed=10, cls1="x1", cls2="x2", nvec=2)
+    a, b = 0.3 - 1.1j, -0.7 + 0.2j
+    y1 = (a * x1[0] + b * x1[1])[None].contiguous()
+    y2 = (a * x2[0] + b * x2[1])[None].contiguous()
+    o1, o2 = cc.cclr_sigma(ctx, x1.cuda(), x2.cuda())
+    p1, p2 = cc.cclr_sigma(ctx, y1.cuda(), y2.cuda())
+    assert rel(p2[0].cpu().numpy(), (a * o2[0] + b * o2[1]).cpu().numpy()) < 1e-13
+    assert rel(p1[0].cpu().numpy(), (a * o1[0] + b * o1[1]).cpu().numpy()) < 1e-13
+    z1, z2 = cc.cclr_sigma(ctx, x1.cuda(), x2.cuda(), 0.0773, 0.0045)
+    zz = 0.0773 + 0.0045j
+    assert rel(z2.cpu().numpy(), (o2.cpu() - zz * x2).numpy()) < 1e-14
+    assert rel(z1.cpu().numpy(), (o1.cpu() - zz * x1).numpy()) < 1e-14
+    ctx.close()

@@ -1,0 +1,59 @@
+"""Host-logic check of the contraction plans (csrc/plans.inc): the plan text the GPU library executes is run by a
+numpy interpreter (tests/plan_interp.py) and compared with the oracle -- every intermediate of S-Eq. 15-28
+ and the sigma vector of S-Eq. 11-12.  A wrong sign, index order, pair
+unpacking or GEMM shape anywhere in the plan fails here, on the CPU, before any kernel runs."""
+import numpy as np
+import pytest
+from conftest import random_system, random_amplitudes
+from oracle import ccsd, cclr, packing
+import plan_interp
+
+
+def _setup(o, v, seed, chunk_override=None):
+    f, V = random_system(o, v, seed=seed, diag_fock=False)
+    t1, t2 = random_amplitudes(o, v, seed=seed + 1)
+    ints = ccsd.Integrals.from_full(f, V, o)
+    full = dict(oooo=ints.oooo, ooov=ints.ooov, oovv=ints.oovv, ovvo=ints.ovvo, ovvv=ints.ovvv, vvvv=ints.vvvv)
+    packed = packing.pack_eri(full)
+    t1p, t2p = packing.pack_amplitudes(t1, t2)
+    it = plan_interp.run_create(o, v, f, packed, t1p, t2p, chunk_override)
+    return it, cclr.CCLR(ints, t1, t2)
+
+
+def _close(a, b, tol=1e-12):
+    return np.abs(a - b).max() <= tol * max(1.0, np.abs(b).max())
+
+
+@pytest.mark.parametrize("o,v,chunk", [(3, 5, None), (4, 6, 2), (2, 7, 3)])
+def test_create_plan_reproduces_oracle_intermediates(o, v, chunk):
+    it, c = _setup(o, v, seed=40 + v, chunk_override=chunk)
+    P = packing
+    assert _close(it.get("Fme"), c.Fme)
+    assert _close(it.get("FmeT"), c.Fme.T)
+    assert _close(it.get("Fmi"), c.Fmi)
+    assert _close(it.get("Fae"), c.Fae)
+    assert _close(it.get("Wmnij"), P.pack_pair_axes(P.pack_pair_axes(c.Wmnij, 2), 0))
+    assert _close(it.get("Wabef"), P.pack_pair_axes(P.pack_pair_axes(c.Wabef, 2), 0))
+    assert _close(it.get("Wring"), c.Wmbej.transpose(1, 3, 2, 0))                    # [b j e m]
+    assert _close(it.get("Wie"), P.pack_pair_axes(c.Wmnie, 0).transpose(1, 2, 0))    # [i e (mn)]
+    assert _close(it.get("Wnjem"), c.Wmnie.transpose(0, 2, 3, 1))                    # [n j e m] = W[nm,je]
+    assert _close(it.get("Wamef"), P.pack_pair_axes(c.Wamef, 2))                     # [a m (ef)]
+    assert _close(it.get("Wx"), c.Wamef.transpose(0, 2, 3, 1))                       # [b f e m] = W[bm,fe]
+    assert _close(it.get("Wmbij"), P.pack_pair_axes(c.Wmbij, 2))
+    assert _close(it.get("Wabej"), P.pack_pair_axes(c.Wabej, 0).transpose(0, 2, 1))  # [(ab) j e]
+    assert _close(it.get("Vnm"), P.pack_pair_axes(c.I.oovv, 2))
+    assert _close(it.get("Vx"), P.pack_pair_axes(c.I.oovv, 0).transpose(1, 2, 0))    # [f e (mn)]
+    assert _close(it.get("Ut"), P.pack_pair_axes(c.t2, 2))
+    assert _close(it.get("To"), P.pack_pair_axes(c.t2, 0))
+
+
+@pytest.mark.parametrize("o,v,chunk", [(3, 5, None), (4, 6, 2)])
+def test_sigma_plan_reproduces_oracle_sigma(o, v, chunk):
+    it, c = _setup(o, v, seed=50 + v, chunk_override=chunk)
+    for k, z in enumerate([0.0, 0.0773 + 0.0045j]):
+        x1, x2 = random_amplitudes(o, v, seed=60 + k, scale=1.0)
+        x1p, x2p = packing.pack_amplitudes(x1, x2)
+        s1, s2 = plan_interp.run_sigma(it, x1p, x2p, z)
+        r1, r2 = packing.pack_amplitudes(*c.sigma(x1, x2, z))
+        assert np.linalg.norm(s1 - r1) <= 1e-12 * np.linalg.norm(r1)
+        assert np.linalg.norm(s2 - r2) <= 1e-12 * np.linalg.norm(r2)
