@@ -92,6 +92,10 @@ int cclr_solve(cclr_ctx *ctx, const cclr_c128 *xi1, const cclr_c128 *xi2, int nr
 int cclr_property(cclr_ctx *ctx, const cclr_c128 *eta1, const cclr_c128 *eta2, const cclr_c128 *x1,
                   const cclr_c128 *x2, int nvec, cclr_c128 *result);
 
+/* Cap the trial-space dimension of cclr_solve (memory = 2 * dim * (v*o + vv*oo) * 16 bytes); 0 = sized from the free
+ * device memory.  When the space is full it is collapsed onto the current solutions and the iteration continues. */
+int cclr_set_max_subspace(cclr_ctx *ctx, int dim);
+
 void cclr_destroy(cclr_ctx *ctx);
 const char *cclr_strerror(int code);
 int cclr_last_cuda_error(void); /* CUDA error code behind the last CCLR_ECUDA of the calling thread */
@@ -131,6 +135,10 @@ size_t cclr_ctx_bytes(const cclr_ctx *ctx);
  * Only filled when profiling was enabled with cclr_set_profiling(ctx, 1) (which adds event records). */
 int cclr_set_profiling(cclr_ctx *ctx, int on);
 int cclr_last_sigma_ms(const cclr_ctx *ctx, double ms[5]);
+
+/* HOST-only: the reduced-space step of cclr_solve: beta[k] = (G - z[k] I)^{-1} rhs for nz shifts sharing one
+ * L x L row-major matrix G, through one Hessenberg reduction.  All pointers are host pointers; beta is [nz][L]. */
+int cclr_host_shifted_solve(int L, const cclr_c128 *G, const cclr_c128 *rhs, int nz, const cclr_c128 *z, cclr_c128 *beta);
 
 /* FP64 tensor-core (DMMA m8n8k4) issue-rate probe: runs `iters` dependent-chain-free DMMA per warp on every SM
  * and returns the measured TFLOP/s in *tflops (host).  This is the roofline denominator used by bench.py. */

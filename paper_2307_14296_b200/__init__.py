@@ -73,6 +73,9 @@ class Context:
         torch.cuda.current_stream().synchronize()
         return out
 
+    def set_max_subspace(self, dim):
+        _lib.check(_lib.load().cclr_set_max_subspace(self.handle, int(dim)), "cclr_set_max_subspace")
+
     def set_profiling(self, on):
         _lib.check(_lib.load().cclr_set_profiling(self.handle, int(bool(on))), "cclr_set_profiling")
 

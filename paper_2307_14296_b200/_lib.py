@@ -32,6 +32,7 @@ SIGNATURES = {
     "cclr_solve": (C.c_int, [C.c_void_p, c128_p, c128_p, C.c_int, C.POINTER(C.c_double), C.c_int, C.c_double,
                              C.c_double, C.c_int, c128_p, c128_p, C.POINTER(SolveInfo)]),
     "cclr_property": (C.c_int, [C.c_void_p, c128_p, c128_p, c128_p, c128_p, C.c_int, C.POINTER(Complex)]),
+    "cclr_set_max_subspace": (C.c_int, [C.c_void_p, C.c_int]),
     "cclr_destroy": (None, [C.c_void_p]),
     "cclr_strerror": (C.c_char_p, [C.c_int]),
     "cclr_last_cuda_error": (C.c_int, []),
@@ -40,6 +41,7 @@ SIGNATURES = {
     "cclr_zgemm": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.POINTER(Complex), c128_p, C.c_long, C.c_int,
                              c128_p, C.c_long, C.c_int, C.c_int, C.POINTER(Complex), c128_p, C.c_long, C.c_int,
                              C.c_long, C.c_long, C.c_long]),
+    "cclr_host_shifted_solve": (C.c_int, [C.c_int, c128_p, c128_p, C.c_int, c128_p, c128_p]),
     "cclr_ladder": (C.c_int, [C.c_void_p, c128_p, C.c_int, c128_p]),
     "cclr_ring": (C.c_int, [C.c_void_p, c128_p, c128_p]),
     "cclr_get_intermediate": (C.c_long, [C.c_void_p, C.c_char_p, c128_p, C.c_long]),

@@ -318,6 +318,12 @@ extern "C" long cclr_get_intermediate(cclr_ctx *ctx, const char *name, cclr_c128
   return n;
 }
 
+extern "C" int cclr_set_max_subspace(cclr_ctx *ctx, int dim) {
+  if (!ctx || dim < 0) return CCLR_EINVAL;
+  ctx->max_subspace = dim;
+  return CCLR_OK;
+}
+
 extern "C" int cclr_set_profiling(cclr_ctx *ctx, int on) {
   if (!ctx) return CCLR_EINVAL;
   ctx->profiling = on != 0;

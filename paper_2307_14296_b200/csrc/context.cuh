@@ -24,6 +24,7 @@ struct cclr_ctx {
   // staging buffers of cclr_sigma_host
   c128 *host_stage = nullptr;
   size_t host_stage_elems = 0;
+  int max_subspace = 0;           // cclr_set_max_subspace (0 = automatic)
   size_t extra_bytes = 0;         // device bytes owned outside the plan
 };
 
