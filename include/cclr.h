@@ -127,6 +127,11 @@ int cclr_ring(cclr_ctx *ctx, const cclr_c128 *x2, cclr_c128 *out2);
  * oracle).  Names and layouts: see DESIGN.md "Data layout".  Returns the element count, or a negative error. */
 long cclr_get_intermediate(cclr_ctx *ctx, const char *name, cclr_c128 *out, long capacity);
 
+/* Number of CUDA kernels this library has launched in the calling process so far (every GEMM, layout and vector
+ * kernel is counted at its launch site; memcpy / memset are not).  bench.py reports the difference over its timed
+ * region as "gpu_launches". */
+unsigned long long cclr_kernel_launches(void);
+
 /* Device bytes currently owned by the context. */
 size_t cclr_ctx_bytes(const cclr_ctx *ctx);
 

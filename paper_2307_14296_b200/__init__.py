@@ -182,6 +182,10 @@ def cclr_zgemm(A, B, C_out, alpha=1.0, beta=0.0, conj_a=False, conj_b=False, b_i
     return C_out
 
 
+def cclr_kernel_launches():
+    return int(_lib.load().cclr_kernel_launches())
+
+
 def cclr_fp64_tensor_peak(iters=20000):
     out = C.c_double()
     _lib.check(_lib.load().cclr_fp64_tensor_peak(_stream(), iters, C.byref(out)), "cclr_fp64_tensor_peak")

@@ -45,6 +45,7 @@ SIGNATURES = {
     "cclr_ladder": (C.c_int, [C.c_void_p, c128_p, C.c_int, c128_p]),
     "cclr_ring": (C.c_int, [C.c_void_p, c128_p, c128_p]),
     "cclr_get_intermediate": (C.c_long, [C.c_void_p, C.c_char_p, c128_p, C.c_long]),
+    "cclr_kernel_launches": (C.c_ulonglong, []),
     "cclr_ctx_bytes": (C.c_size_t, [C.c_void_p]),
     "cclr_set_profiling": (C.c_int, [C.c_void_p, C.c_int]),
     "cclr_last_sigma_ms": (C.c_int, [C.c_void_p, C.POINTER(C.c_double)]),

@@ -26,6 +26,9 @@ CCLR_HOST_DEVICE void cfma(c128 &a, c128 b, c128 c) {
 CCLR_HOST_DEVICE long pair_index(long p, long q) { return q * (q - 1) / 2 + p; }
 CCLR_HOST_DEVICE long npair(long n) { return n * (n - 1) / 2; }
 
+// process-wide count of kernels launched by the library (include/cclr.h: cclr_kernel_launches)
+void cclr_count_launch(int n = 1);
+
 // ---- zgemm.cu -------------------------------------------------------------------------------------------------
 struct ZgemmWorkspace {
   c128 *buf = nullptr;   // split-K partial sums

@@ -106,5 +106,6 @@ cudaError_t permute(cudaStream_t st, const PermArgs &args) {
     permute_kernel<unsigned><<<(unsigned)blocks, threads, 0, st>>>(args);
   else
     permute_kernel<unsigned long long><<<(unsigned)blocks, threads, 0, st>>>(args);
+  cclr_count_launch();
   return cudaGetLastError();
 }

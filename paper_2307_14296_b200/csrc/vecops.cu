@@ -142,8 +142,10 @@ cudaError_t multi_dot(cudaStream_t st, const c128 *A, long lda, int na, const c1
     const c128 *Ap = diag ? A + (size_t)p0 * lda : A, *Bp = diag ? B + (size_t)p0 * ldb : B;
     dot_partial_kernel<<<grid, DOT_THREADS, 0, st>>>(Ap, lda, Bp, ldb, nb, n, conjA ? 1 : 0, diag ? 1 : 0, chunk_len,
                                                      partial + (size_t)p0 * chunks);
+    cclr_count_launch();
   }
   dot_final_kernel<<<(npairs + 127) / 128, 128, 0, st>>>(partial, chunks, npairs, out);
+  cclr_count_launch();
   return cudaGetLastError();
 }
 
@@ -151,23 +153,27 @@ cudaError_t lincomb(cudaStream_t st, c128 *y, c128 beta, const c128 *coef, const
   if (n <= 0) return cudaSuccess;
   if ((size_t)m * sizeof(c128) > 48 * 1024) return cudaErrorInvalidValue;
   lincomb_kernel<<<stream_grid(n), 256, (size_t)m * sizeof(c128), st>>>(y, beta, coef, V, ldv, m, n);
+  cclr_count_launch();
   return cudaGetLastError();
 }
 
 cudaError_t precondition(cudaStream_t st, c128 *y, const c128 *x, const double *D, c128 z, c128 alpha, long n) {
   if (n <= 0) return cudaSuccess;
   precondition_kernel<<<stream_grid(n), 256, 0, st>>>(y, x, D, z, alpha, n);
+  cclr_count_launch();
   return cudaGetLastError();
 }
 
 cudaError_t scale_vec(cudaStream_t st, c128 *y, c128 alpha, long n) {
   if (n <= 0) return cudaSuccess;
   scale_kernel<<<stream_grid(n), 256, 0, st>>>(y, alpha, n);
+  cclr_count_launch();
   return cudaGetLastError();
 }
 
 cudaError_t denominators(cudaStream_t st, const c128 *fock, int o, int v, double *D) {
   const long n = (long)o * v + npair(o) * npair(v);
   denominators_kernel<<<stream_grid(n), 256, 0, st>>>(fock, o, v, D);
+  cclr_count_launch();
   return cudaGetLastError();
 }

@@ -307,6 +307,7 @@ cudaError_t launch(cudaStream_t st, const CUtensorMap &tmA, const CUtensorMap &t
   }
   dim3 grid((args.N + BN - 1) / BN, (args.M + BM - 1) / BM, batch * args.splits);
   kern<<<grid, threads, smem, st>>>(tmA, tmB, args);
+  cclr_count_launch();
   return cudaGetLastError();
 }
 
@@ -330,6 +331,7 @@ cudaError_t zgemm(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *
   constexpr int BM = 128, BN = 64, BK = 16, WM = 32, WN = 32, STAGES = 4;
   if (K <= 0) {  // C = beta * C
     zgemm_reduce_kernel<<<256, 256, 0, st>>>(nullptr, 0, M, N, alpha, beta, C, ldc, sc, batch);
+    cclr_count_launch();
     return cudaGetLastError();
   }
   ZgemmArgs args{};
@@ -368,6 +370,7 @@ cudaError_t zgemm(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *
     int blocks = (int)((total + 255) / 256);
     if (blocks > 4 * sms) blocks = 4 * sms;
     zgemm_reduce_kernel<<<blocks, 256, 0, st>>>(ws->buf, splits, M, N, alpha, beta, C, ldc, sc, batch);
+    cclr_count_launch();
     e = cudaGetLastError();
   }
   return e;
