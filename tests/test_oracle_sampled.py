@@ -1,0 +1,39 @@
+"""Pins for oracle/sampled.py (the element-by-element definitions used by the full-size GPU parity tests): every element
+against oracle.cclr.CCLR (pinned by the determinant-space definitions) at small sizes."""
+import numpy as np
+import pytest
+
+import synth
+from oracle import ccsd, cclr, packing, sampled
+
+
+@pytest.mark.parametrize("o,v", [(3, 5), (4, 7)])
+def test_sigma_T0_elements_match_full_oracle(o, v):
+    eri = {k: x.numpy() for k, x in synth.eri_packed(o, v, seed=o + v, scale=0.3).items()}
+    f = synth.fock(o, v, seed=1).numpy() + 0.1 * synth.hermitian_operator(o + v, 2, 5)     # f_ov != 0 on purpose
+    ints = ccsd.Integrals(o, v, f, **packing.unpack_eri(o, v, eri))
+    c = cclr.CCLR(ints, np.zeros((v, o), complex), np.zeros((v, v, o, o), complex))
+    x1, x2 = synth.amplitudes(o, v, seed=3, cls1="x1", cls2="x2")
+    x1, x2 = x1[0].numpy(), x2[0].numpy()
+    z = 0.0773 + 0.0045j
+    w1, w2 = c.sigma(*packing.unpack_amplitudes(x1, x2, o, v), z=z)
+    vvvv = eri["vvvv"].reshape(packing.npair(v), -1)
+    singles = [(a, i) for a in range(v) for i in range(o)]
+    doubles = [(a, b, i, j) for b in range(v) for a in range(b) for j in range(o) for i in range(j)]
+    g1, g2 = sampled.sigma_T0_elements(o, v, f, eri, lambda ab: vvvv[ab], x1, x2, singles, doubles, z=z)
+    assert np.abs(np.array(g1) - np.array([w1[a, i] for a, i in singles])).max() < 1e-13
+    assert np.abs(np.array(g2) - np.array([w2[a, b, i, j] for a, b, i, j in doubles])).max() < 1e-13
+
+
+def test_ladder_rows_is_term_T11():
+    o, v = 3, 6
+    eri = {k: x.numpy() for k, x in synth.eri_packed(o, v, seed=4, scale=0.3).items()}
+    _, x2 = synth.amplitudes(o, v, seed=5, cls1="x1", cls2="x2")
+    x2p = x2[0].numpy().reshape(packing.npair(v), packing.npair(o))
+    full = packing.unpack_eri(o, v, eri)
+    r2 = packing.unpack_pair_axis(packing.unpack_pair_axis(x2p, o, 1), v, 0)
+    want = 0.5 * np.einsum("abef,efij->abij", full["vvvv"], r2)                       # T11 as printed
+    want = packing.pack_pair_axes(packing.pack_pair_axes(want, 2), 0)
+    rows = [0, 3, 14]
+    got = sampled.ladder_rows(eri["vvvv"].reshape(15, 15)[rows], x2p)
+    assert np.abs(got - want[rows]).max() < 1e-14
