@@ -138,3 +138,24 @@ def hermitian_operator(n, seed, component, imaginary_antisymmetric=False):
         return 1j * (K - K.T) / math.sqrt(2.0)
     K = (rng.normal(size=(n, n)) + 1j * rng.normal(size=(n, n))) / math.sqrt(2.0)
     return (K + K.conj().T) / math.sqrt(2.0)
+
+
+def first_order_amplitudes(o, v, fock_matrix, oovv):
+    """Ground-state amplitudes of the SHAPE a converged CCSD has, for sizes where no converged T is available: t1 = 0 and
+    t2[(ab),(ij)] = conj(<ij||ab>) / (eps_i + eps_j - eps_a - eps_b), the first-order (perturbative) doubles, from the packed
+    oovv class ([oo][vv]) and the diagonal of the Fock matrix.  Input recipe only (elementwise on the synthetic inputs);
+    sigma = dOmega/dt . x holds at any t, so parity does not depend on it."""
+    dev = oovv.device
+    eps = torch.diagonal(fock_matrix).real.to(dev)
+    eo, ev = eps[:o], eps[o:]
+    # pair order P = q(q-1)/2 + p: q outer, p inner
+    def pair_sums(e, n):
+        q = torch.arange(n, device=dev)[:, None].expand(n, n)
+        p = torch.arange(n, device=dev)[None, :].expand(n, n)
+        m = p < q
+        return e[p[m]] + e[q[m]]
+
+    d = pair_sums(eo, o)[None, :] - pair_sums(ev, v)[:, None]              # [vv][oo]
+    t2 = oovv.view(npair(o), npair(v)).conj().transpose(0, 1) / d
+    t1 = torch.zeros(o * v, dtype=torch.complex128, device=dev)
+    return t1, t2.contiguous().view(-1)
