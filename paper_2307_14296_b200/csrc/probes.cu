@@ -125,13 +125,10 @@ extern "C" int cclr_zgemm(void *cuda_stream, int M, int N, int K, const cclr_c12
   if (K > 0 && (!A || !B)) return CCLR_EINVAL;
   if (lda < K || ldc < N || (b_is_kn ? ldb < N : ldb < K)) return CCLR_EINVAL;
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  // split-K workspace for this stand-alone entry point (the context keeps its own)
+  // K-split workspace for this stand-alone entry point (the context keeps its own): room for 3 partial tiles per SM
   ZgemmWorkspace ws;
-  const long tiles = (long)((M + 127) / 128) * ((N + 63) / 64) * batch;
-  if (tiles < zgemm_num_sms() && K >= 256) {
-    ws.elems = (size_t)M * N * batch * 64;
-    if (cudaMalloc(&ws.buf, ws.elems * sizeof(c128)) != cudaSuccess) { ws.buf = nullptr; ws.elems = 0; cudaGetLastError(); }
-  }
+  ws.elems = (size_t)3 * zgemm_num_sms() * 128 * 64;
+  if (cudaMalloc(&ws.buf, ws.elems * sizeof(c128)) != cudaSuccess) { ws.buf = nullptr; ws.elems = 0; cudaGetLastError(); }
   cudaError_t e = zgemm(st, M, N, K, make_double2(alpha->re, alpha->im), (const c128 *)A, lda, conj_a != 0,
                         (const c128 *)B, ldb, b_is_kn != 0, conj_b != 0, make_double2(beta->re, beta->im), (c128 *)C,
                         ldc, batch, sa, sb, sc, ws.buf ? &ws : nullptr);

@@ -26,6 +26,8 @@
 
 namespace {
 
+constexpr int ZG_BM = 128, ZG_BK = 16, ZG_STAGES = 4;   // CTA tile rows, K chunk, TMA ring depth; BN = 8*NG, NG = 4..8
+
 // ---------------------------------------------------------------------------------------------------------------
 // PTX wrappers
 // ---------------------------------------------------------------------------------------------------------------
@@ -76,9 +78,14 @@ struct ZgemmArgs {
   long ldc, sc;
   c128 alpha, beta;
   int conjA, conjB;
-  int splits;          // >= 1
-  int chunks_per_split;
-  c128 *partial;       // [batch*splits][M][N] when splits > 1
+  // launch geometry: a 1-D grid of CTAs over the (batch, tile_m, tile_n) tiles, tile_n fastest.  The first `main_tiles`
+  // tiles are computed whole by one CTA each; every remaining ("tail") tile is split along K over `tail_splits` CTAs
+  // which write partial tiles to `partial` ([tail tile][split][BM*BN]) for zgemm_tail_reduce_kernel.  This removes the
+  // wave-quantisation loss of the last partial wave (and is the split-K path of tall-K / tiny-MN contractions when
+  // main_tiles == 0).
+  int tiles_m, tiles_n;
+  int main_tiles, tail_splits, chunks_per_split;
+  c128 *partial;
 };
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -90,7 +97,7 @@ zgemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CU
   constexpr int WARPS_M = BM / WM, WARPS_N = BN / WN, NCW = WARPS_M * WARPS_N;
   constexpr int MI = WM / 8, NG = WN / 4;          // DMMA tiles per warp: MI row groups x NG column groups
   constexpr int A_BYTES = BM * BK * 16, B_BYTES = BN * BK * 16, STAGE_BYTES = A_BYTES + B_BYTES;
-  static_assert(BK % 8 == 0 && BM % 8 == 0 && BN % 8 == 0 && WM % 8 == 0 && WN % 8 == 0, "tile shape");
+  static_assert(BK % 8 == 0 && BM % 8 == 0 && BN % 8 == 0 && WM % 8 == 0 && WN % 4 == 0, "tile shape");
   static_assert(NCW % 4 == 0, "consumer warps must form whole warpgroups (setmaxnreg)");
   constexpr int CONSUMER_REGS = (NCW == 8) ? 232 : 200;
 
@@ -100,13 +107,24 @@ zgemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CU
   const uint32_t bar_base = smem_base + STAGES * STAGE_BYTES;   // full[STAGES], empty[STAGES], 8 B each
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int tile_n = blockIdx.x, tile_m = blockIdx.y;
-  const int batch = blockIdx.z / p.splits, split = blockIdx.z % p.splits;
+  int tile = (int)blockIdx.x, split = 0;
+  const bool is_tail = tile >= p.main_tiles;
+  if (is_tail) {
+    const int r = tile - p.main_tiles;
+    tile = p.main_tiles + r / p.tail_splits;
+    split = r % p.tail_splits;
+  }
+  const int tiles_mn = p.tiles_m * p.tiles_n;
+  const int batch = tile / tiles_mn;
+  const int tile_m = (tile - batch * tiles_mn) / p.tiles_n, tile_n = (tile - batch * tiles_mn) % p.tiles_n;
   const int nchunks_total = (p.K + BK - 1) / BK;
-  const int chunk0 = split * p.chunks_per_split;
-  int nchunks = nchunks_total - chunk0;
-  if (nchunks > p.chunks_per_split) nchunks = p.chunks_per_split;
-  if (nchunks < 0) nchunks = 0;
+  int chunk0 = 0, nchunks = nchunks_total;
+  if (is_tail) {
+    chunk0 = split * p.chunks_per_split;
+    nchunks = nchunks_total - chunk0;
+    if (nchunks > p.chunks_per_split) nchunks = p.chunks_per_split;
+    if (nchunks < 0) nchunks = 0;
+  }
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < STAGES; ++s) {
@@ -152,6 +170,7 @@ zgemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CU
   const int rmap = ((gid & 1) << 2) | (gid >> 1);   // row permutation inside an 8-row group (bank-conflict free)
   const int par = gid & 1, nb4 = gid >> 1;
   const int wm = warp / WARPS_N, wn = warp % WARPS_N;
+  const int wpar = ((wn * WN) >> 2) & 1;            // WN may be an odd multiple of 4: parity of the warp's first 4-row group
   // sign masks (see header comment): f1 = m1 ^ (par ? b.im : b.re), f2 = m2 ^ (par ? b.re : b.im)
   const uint32_t sa = p.conjA ? 0x80000000u : 0u, sb = p.conjB ? 0x80000000u : 0u;
   const uint32_t m1 = par ? sb : 0u;
@@ -194,7 +213,7 @@ zgemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CU
         for (int g = 0; g < NG; ++g) {
           uint32_t addr;
           if (!BKN) {
-            const int n7 = ((g & 1) << 2) | nb4;
+            const int n7 = (((g & 1) ^ wpar) << 2) | nb4;   // (row & 7) of row = wn*WN + 4g + nb4
             addr = sB + kb * (BN * 128) + g * 512 + (b_off[s4] ^ (uint32_t)(n7 << 4));
           } else {
             const int n = wn * WN + 4 * g + nb4;
@@ -216,9 +235,12 @@ zgemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CU
   }
 
   // ===== epilogue =====
-  const bool partial = p.splits > 1;
-  c128 *Cb = partial ? p.partial + (size_t)blockIdx.z * (size_t)p.M * (size_t)p.N : p.C + (size_t)batch * p.sc;
-  const long ldc = partial ? (long)p.N : p.ldc;
+  // tail tiles: raw partial sums into the workspace tile [BM][BN] of (tail tile, split); main tiles: C directly
+  const bool partial = is_tail;
+  c128 *Cb = partial ? p.partial + ((size_t)(blockIdx.x - p.main_tiles)) * (size_t)(BM * BN) -
+                           ((size_t)tile_m * BM * BN + (size_t)tile_n * BN)
+                     : p.C + (size_t)batch * p.sc;
+  const long ldc = partial ? (long)BN : p.ldc;
   const c128 alpha = partial ? make_double2(1.0, 0.0) : p.alpha;
   const c128 beta = partial ? make_double2(0.0, 0.0) : p.beta;
   const bool has_beta = (beta.x != 0.0) || (beta.y != 0.0);
@@ -295,7 +317,7 @@ bool make_map(CUtensorMap *tm, const c128 *base, long inner_complex, long rows, 
 }
 
 template <int BM, int BN, int BK, int WM, int WN, int STAGES, bool BKN>
-cudaError_t launch(cudaStream_t st, const CUtensorMap &tmA, const CUtensorMap &tmB, const ZgemmArgs &args, int batch) {
+cudaError_t launch(cudaStream_t st, const CUtensorMap &tmA, const CUtensorMap &tmB, const ZgemmArgs &args, int ctas) {
   constexpr int threads = (BM / WM) * (BN / WN) * 32 + 128;
   constexpr int smem = STAGES * (BM + BN) * BK * 16 + 2 * STAGES * 8 + 1024;
   auto kern = zgemm_kernel<BM, BN, BK, WM, WN, STAGES, BKN>;
@@ -305,10 +327,76 @@ cudaError_t launch(cudaStream_t st, const CUtensorMap &tmA, const CUtensorMap &t
     if (e != cudaSuccess) return e;
     configured = true;
   }
-  dim3 grid((args.N + BN - 1) / BN, (args.M + BM - 1) / BM, batch * args.splits);
-  kern<<<grid, threads, smem, st>>>(tmA, tmB, args);
+  kern<<<ctas, threads, smem, st>>>(tmA, tmB, args);
   cclr_count_launch();
   return cudaGetLastError();
+}
+
+// one instantiation per N-tile width BN = 8*NG (NG DMMA column groups per warp), for both B layouts
+template <int NG>
+cudaError_t launch_ng(cudaStream_t st, const CUtensorMap &tmA, const CUtensorMap &tmB, const ZgemmArgs &args, int ctas,
+                      bool kn) {
+  return kn ? launch<ZG_BM, 8 * NG, ZG_BK, 32, 4 * NG, ZG_STAGES, true>(st, tmA, tmB, args, ctas)
+            : launch<ZG_BM, 8 * NG, ZG_BK, 32, 4 * NG, ZG_STAGES, false>(st, tmA, tmB, args, ctas);
+}
+
+// C tile = alpha * sum_splits partial + beta * C for the K-split tail tiles
+__global__ void __launch_bounds__(256) zgemm_tail_reduce_kernel(const ZgemmArgs p, int BN) {
+  const int t = p.main_tiles + (int)blockIdx.x;                 // tile id
+  const int tiles_mn = p.tiles_m * p.tiles_n;
+  const int batch = t / tiles_mn;
+  const int tile_m = (t - batch * tiles_mn) / p.tiles_n, tile_n = (t - batch * tiles_mn) % p.tiles_n;
+  const c128 *part = p.partial + (size_t)blockIdx.x * p.tail_splits * (size_t)(ZG_BM * BN);
+  const bool has_beta = p.beta.x != 0.0 || p.beta.y != 0.0;
+  for (int e = threadIdx.x; e < ZG_BM * BN; e += blockDim.x) {
+    const int r = e / BN, c = e % BN;
+    const int row = tile_m * ZG_BM + r, col = tile_n * BN + c;
+    if (row >= p.M || col >= p.N) continue;
+    c128 s = czero();
+    for (int k = 0; k < p.tail_splits; ++k) s = cadd(s, part[(size_t)k * (ZG_BM * BN) + e]);
+    c128 *dst = p.C + (size_t)batch * p.sc + (size_t)row * p.ldc + col;
+    c128 out = cmul(p.alpha, s);
+    if (has_beta) out = cadd(out, cmul(p.beta, *dst));
+    *dst = out;
+  }
+}
+
+// y[m] = alpha * sum_k opA(A[m][k]) * opB(b[k]) + beta * y[m]: the N = 1 contractions (S3, S4, G3, G4, F_me) are
+// bandwidth-bound GEMVs; one warp per row, 16-byte loads, shuffle reduction (HBM roofline, not the tensor pipe).
+__global__ void __launch_bounds__(256) zgemv_kernel(int M, int K, c128 alpha, const c128 *__restrict__ A, long lda,
+                                                    int conjA, const c128 *__restrict__ b, long incb, int conjB,
+                                                    c128 beta, c128 *C, long ldc) {
+  const int lane = threadIdx.x & 31;
+  const int warps = (gridDim.x * blockDim.x) >> 5;
+  const double sa = conjA ? -1.0 : 1.0, sb = conjB ? -1.0 : 1.0;
+  for (int m = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; m < M; m += warps) {
+    const c128 *a = A + (size_t)m * lda;
+    double x0 = 0.0, y0 = 0.0, x1 = 0.0, y1 = 0.0;
+    int k = lane;
+    for (; k + 32 < K; k += 64) {
+      c128 u = a[k], w = b[(size_t)k * incb], u2 = a[k + 32], w2 = b[(size_t)(k + 32) * incb];
+      u.y *= sa; w.y *= sb; u2.y *= sa; w2.y *= sb;
+      x0 = fma(u.x, w.x, x0); x0 = fma(-u.y, w.y, x0); y0 = fma(u.x, w.y, y0); y0 = fma(u.y, w.x, y0);
+      x1 = fma(u2.x, w2.x, x1); x1 = fma(-u2.y, w2.y, x1); y1 = fma(u2.x, w2.y, y1); y1 = fma(u2.y, w2.x, y1);
+    }
+    if (k < K) {
+      c128 u = a[k], w = b[(size_t)k * incb];
+      u.y *= sa; w.y *= sb;
+      x0 = fma(u.x, w.x, x0); x0 = fma(-u.y, w.y, x0); y0 = fma(u.x, w.y, y0); y0 = fma(u.y, w.x, y0);
+    }
+    x0 += x1; y0 += y1;
+#pragma unroll
+    for (int s = 16; s > 0; s >>= 1) {
+      x0 += __shfl_xor_sync(0xffffffffu, x0, s);
+      y0 += __shfl_xor_sync(0xffffffffu, y0, s);
+    }
+    if (lane == 0) {
+      c128 out = cmul(alpha, make_double2(x0, y0));
+      c128 *dst = C + (size_t)m * ldc;
+      if (beta.x != 0.0 || beta.y != 0.0) out = cadd(out, cmul(beta, *dst));
+      *dst = out;
+    }
+  }
 }
 
 }  // namespace
@@ -328,32 +416,70 @@ cudaError_t zgemm(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *
                   const c128 *B, long ldb, bool b_is_kn, bool conjB, c128 beta, c128 *C, long ldc, int batch, long sa,
                   long sb, long sc, const ZgemmWorkspace *ws) {
   if (M <= 0 || N <= 0 || batch <= 0) return cudaSuccess;
-  constexpr int BM = 128, BN = 64, BK = 16, WM = 32, WN = 32, STAGES = 4;
+  constexpr int BM = ZG_BM, BK = ZG_BK;
+  const int sms = zgemm_num_sms();
   if (K <= 0) {  // C = beta * C
     zgemm_reduce_kernel<<<256, 256, 0, st>>>(nullptr, 0, M, N, alpha, beta, C, ldc, sc, batch);
     cclr_count_launch();
     return cudaGetLastError();
   }
+  // ---- N = 1 or M = 1: bandwidth-bound matrix-vector products ----
+  if (batch == 1 && (N == 1 || (M == 1 && !b_is_kn)) && K >= 32) {
+    const int rows = N == 1 ? M : N;
+    int blocks = (rows + 7) / 8;
+    if (blocks > sms * 8) blocks = sms * 8;
+    if (N == 1)
+      zgemv_kernel<<<blocks, 256, 0, st>>>(M, K, alpha, A, lda, conjA, B, b_is_kn ? ldb : 1, conjB, beta, C, ldc);
+    else
+      zgemv_kernel<<<blocks, 256, 0, st>>>(N, K, alpha, B, ldb, conjB, A, 1, conjA, beta, C, 1);
+    cclr_count_launch();
+    return cudaGetLastError();
+  }
+  // ---- N-tile width: the least padded N, widest tile on ties ----
+  int NG = 8;
+  long best = -1;
+  for (int ng = 8; ng >= 4; --ng) {
+    const long bn = 8 * ng, padded = (N + bn - 1) / bn * bn;
+    if (best < 0 || padded < best) { best = padded; NG = ng; }
+  }
+  const int BN = 8 * NG;
   ZgemmArgs args{};
   args.M = M; args.N = N; args.K = K;
   args.C = C; args.ldc = ldc; args.sc = sc;
   args.alpha = alpha; args.beta = beta;
   args.conjA = conjA; args.conjB = conjB;
+  args.tiles_m = (M + BM - 1) / BM;
+  args.tiles_n = (N + BN - 1) / BN;
+  const long tiles = (long)args.tiles_m * args.tiles_n * batch;
+  if (tiles > 0x7fffffffL / 2) return cudaErrorInvalidValue;
   const int nchunks = (K + BK - 1) / BK;
-  // split-K when the MN tile grid cannot fill the chip and K is long
-  int splits = 1;
-  const long tiles = (long)((M + BM - 1) / BM) * ((N + BN - 1) / BN) * batch;
-  const int sms = zgemm_num_sms();
-  if (ws && ws->buf && tiles < sms && nchunks >= 16) {
-    splits = (int)((2L * sms + tiles - 1) / tiles);
-    if (splits > nchunks / 4) splits = nchunks / 4;
-    const size_t per = (size_t)M * N * batch;
-    if ((size_t)splits * per > ws->elems) splits = (int)(ws->elems / per);
-    if (splits < 1) splits = 1;
+  // ---- launch geometry (see ZgemmArgs): whole tiles, then the K-split tail ----
+  int main_tiles = (int)tiles, splits = 1;
+  const size_t tile_elems = (size_t)BM * BN;
+  if (ws && ws->buf) {
+    if (tiles < sms && nchunks >= 16) {
+      // the MN grid cannot fill the chip: split every tile along K
+      splits = (int)((2L * sms + tiles - 1) / tiles);
+      if (splits > nchunks / 4) splits = nchunks / 4;
+      if ((size_t)splits * tiles * tile_elems > ws->elems) splits = (int)(ws->elems / (tiles * tile_elems));
+      if (splits > 1) main_tiles = 0; else splits = 1;
+    } else if (tiles > sms) {
+      // last partial wave: split its tiles so that it lasts 1/splits of a wave instead of a whole one
+      const int rem = (int)(tiles % sms);
+      if (rem > 0 && 2 * rem <= sms) {
+        splits = sms / rem;
+        if (splits > nchunks / 4) splits = nchunks / 4;
+        if ((size_t)splits * rem * tile_elems > ws->elems) splits = (int)(ws->elems / (rem * tile_elems));
+        if (splits > 1) main_tiles = (int)tiles - rem; else splits = 1;
+      }
+    }
   }
-  args.splits = splits;
+  args.main_tiles = main_tiles;
+  args.tail_splits = splits;
   args.chunks_per_split = (nchunks + splits - 1) / splits;
   args.partial = splits > 1 ? ws->buf : nullptr;
+  const int tail_tiles = (int)tiles - main_tiles;
+  const int ctas = main_tiles + tail_tiles * splits;
 
   CUtensorMap tmA, tmB;
   if (!make_map(&tmA, A, K, M, lda, batch, sa, BM)) return cudaErrorInvalidValue;
@@ -362,14 +488,17 @@ cudaError_t zgemm(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *
   } else {
     if (!make_map(&tmB, B, N, K, ldb, batch, sb, BK)) return cudaErrorInvalidValue;
   }
-  cudaError_t e = b_is_kn ? launch<BM, BN, BK, WM, WN, STAGES, true>(st, tmA, tmB, args, batch)
-                          : launch<BM, BN, BK, WM, WN, STAGES, false>(st, tmA, tmB, args, batch);
+  cudaError_t e;
+  switch (NG) {
+    case 4: e = launch_ng<4>(st, tmA, tmB, args, ctas, b_is_kn); break;
+    case 5: e = launch_ng<5>(st, tmA, tmB, args, ctas, b_is_kn); break;
+    case 6: e = launch_ng<6>(st, tmA, tmB, args, ctas, b_is_kn); break;
+    case 7: e = launch_ng<7>(st, tmA, tmB, args, ctas, b_is_kn); break;
+    default: e = launch_ng<8>(st, tmA, tmB, args, ctas, b_is_kn); break;
+  }
   if (e != cudaSuccess) return e;
-  if (splits > 1) {
-    const size_t total = (size_t)M * N * batch;
-    int blocks = (int)((total + 255) / 256);
-    if (blocks > 4 * sms) blocks = 4 * sms;
-    zgemm_reduce_kernel<<<blocks, 256, 0, st>>>(ws->buf, splits, M, N, alpha, beta, C, ldc, sc, batch);
+  if (tail_tiles > 0 && splits > 1) {
+    zgemm_tail_reduce_kernel<<<tail_tiles, 256, 0, st>>>(args, BN);
     cclr_count_launch();
     e = cudaGetLastError();
   }

@@ -51,6 +51,16 @@ def rel(a, b):
     (300, 34, 5000, False, False, False, 1.0),     # tall K -> split-K path
     (20, 1, 80, False, False, False, 1.0),         # GEMV shapes of the singles terms
     (1000, 9, 34, True, False, False, 0.0),
+    # every N-tile width (BN = 32, 40, 48, 56, 64) in both B layouts, ragged edges
+    (300, 34, 70, True, False, False, 1.0), (300, 34, 70, False, True, False, 0.0),
+    (257, 45, 100, True, False, True, 0.5), (257, 45, 100, False, False, False, 0.0),
+    (130, 153, 64, True, False, False, 0.0), (130, 153, 64, False, False, True, 1.0),
+    (260, 276, 48, True, True, False, 0.0), (260, 276, 48, False, False, False, -1.0),
+    # more tiles than SMs with a short last wave -> K-split tail tiles (40 x 5 = 200 tiles on 148 SMs)
+    (5120, 276, 200, True, False, False, 1.0), (5120, 276, 200, False, True, True, 0.0),
+    (19000, 30, 130, True, False, False, 0.5),
+    # matrix-vector products (N = 1 in both layouts, M = 1)
+    (4000, 1, 481, False, True, False, 1.0), (4000, 1, 481, True, False, True, 0.0), (1, 700, 333, False, False, True, 0.5),
 ])
 def test_zgemm_matches_numpy(M, N, K, kn, ca, cb, beta):
     cc = _lib()
@@ -232,4 +242,27 @@ def test_gpu_linearity_and_shift_identity():
     zz = 0.0773 + 0.0045j
     assert rel(z2.cpu().numpy(), (o2.cpu() - zz * x2).numpy()) < 1e-14
     assert rel(z1.cpu().numpy(), (o1.cpu() - zz * x1).numpy()) < 1e-14
+    ctx.close()
+
+
+def test_sigma_matches_full_oracle_at_config2():
+    """BASELINE.json configs[1] (o=10, v=80, damped gamma=0.0045) at full size against the full-tensor oracle, norm-wise
+    1e-10.  Amplitudes: first-order doubles (synth.first_order_amplitudes) -- sigma = dOmega/dt . x holds at any t."""
+    cc = _lib()
+    o, v = 10, 80
+    eri = synth.eri_packed(o, v, seed=0)
+    f = synth.fock(o, v, seed=0)
+    t1, t2 = synth.first_order_amplitudes(o, v, f, eri["oovv"])
+    full = packing.unpack_eri(o, v, {k: x.numpy() for k, x in eri.items()})
+    ints = ccsd.Integrals(o, v, f.numpy(), **full)
+    c = cclr.CCLR(ints, *packing.unpack_amplitudes(t1.numpy(), t2.numpy(), o, v))
+    ctx = cc.cclr_create(o, v, f.cuda(), {k: x.cuda() for k, x in eri.items()}, t1.cuda(), t2.cuda())
+    x1, x2 = synth.amplitudes(o, v, seed=3, cls1="x1", cls2="x2")
+    z = 0.0773 + 0.0045j
+    o1, o2 = cc.cclr_sigma(ctx, x1.cuda(), x2.cuda(), z.real, z.imag)
+    torch.cuda.synchronize()
+    r1, r2 = c.sigma(*packing.unpack_amplitudes(x1[0].numpy(), x2[0].numpy(), o, v), z=z)
+    r1p, r2p = packing.pack_amplitudes(r1, r2)
+    assert rel(o1[0].cpu().numpy(), r1p.reshape(-1)) < 1e-10
+    assert rel(o2[0].cpu().numpy(), r2p.reshape(-1)) < 1e-10
     ctx.close()
