@@ -226,6 +226,7 @@ def run_ours(args):
             phases[k] += val
     e1.record()
     torch.cuda.nvtx.range_pop()
+    ops_last = ctx.last_sigma_ops()
     barrier()
     launches = cc.cclr_kernel_launches() - launches0
     ms = e0.elapsed_time(e1)
@@ -272,6 +273,8 @@ def run_ours(args):
             "traffic": None, "algorithmic_bytes": 16.0 * (npair(v) ** 2 + 2 * n2), "ms_per_launch": lad_ms,
         }
         tot = max(phases["total"], 1e-9)
+        if args.ops:
+            line["ops_ms_last_step"] = [(t, round(m, 4)) for t, m in ops_last]
         line["phases_ms_per_step"] = {k: val / args.steps for k, val in phases.items()}
         line["phase_share"] = {k: val / tot for k, val in phases.items() if k != "total"}
         ring_ms = phases["ring"] / (args.steps * nvec)
@@ -312,6 +315,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--tol", type=float, default=1e-10)
     ap.add_argument("--no-solve", action="store_true")
+    ap.add_argument("--ops", action="store_true", help="add the per-operation times of the last sigma step to the line")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

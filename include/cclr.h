@@ -92,6 +92,23 @@ int cclr_solve(cclr_ctx *ctx, const cclr_c128 *xi1, const cclr_c128 *xi2, int nr
 int cclr_property(cclr_ctx *ctx, const cclr_c128 *eta1, const cclr_c128 *eta2, const cclr_c128 *x1,
                   const cclr_c128 *x2, int nvec, cclr_c128 *result);
 
+typedef struct {
+  int iterations;        /* residual evaluations that were followed by an amplitude update          */
+  int converged;         /* 1 if ||Omega|| <= tol                                                    */
+  int sigma_calls;       /* cclr_create + cclr_sigma pairs spent (two per residual)                  */
+  double residual;       /* final ||Omega||_2 over the FULL tensors (= sqrt(|O1|^2 + 4 |O2 unique|^2)) */
+  double energy_re, energy_im; /* CCSD correlation energy  sum f[i,a] t1[a,i] + 1/4 sum <ij||ab> tau[ab,ij]  */
+  double seconds;
+} cclr_ccsd_info;
+
+/* Ground-state CCSD amplitudes (paper step 1): solves Omega(t) = 0 by quasi-Newton steps
+ * t -= Omega / D with DIIS, where the residual is assembled from this library's own Jacobian transform through the exact
+ * identity  Omega(t) = Omega(0) + 1/2 sum_k A(s_k t) . t,  s_k = 1/2 -+ 1/(2 sqrt 3).
+ * t1 [v][o], t2 [vv][oo] are IN/OUT device arrays: the start amplitudes on entry (zeros are fine), the solution on exit.
+ * The integrals are only read.  Returns CCLR_OK, or CCLR_ENOTCONV (best iterate written, info filled). */
+int cclr_ccsd(int o, int v, const cclr_c128 *fock, const cclr_eri_packed *eri, cclr_c128 *t1, cclr_c128 *t2, double tol,
+              int maxiter, void *cuda_stream, cclr_ccsd_info *info);
+
 /* Cap the trial-space dimension of cclr_solve (memory = 2 * dim * (v*o + vv*oo) * 16 bytes); 0 = sized from the free
  * device memory.  When the space is full it is collapsed onto the current solutions and the iteration continues. */
 int cclr_set_max_subspace(cclr_ctx *ctx, int dim);
@@ -140,6 +157,12 @@ size_t cclr_ctx_bytes(const cclr_ctx *ctx);
  * Only filled when profiling was enabled with cclr_set_profiling(ctx, 1) (which adds event records). */
 int cclr_set_profiling(cclr_ctx *ctx, int on);
 int cclr_last_sigma_ms(const cclr_ctx *ctx, double ms[5]);
+/* Per operation of the sigma plan (csrc/plans.inc, CCLR_PLAN_SIGMA): the number of operations, the plan statement of
+ * operation k (a string owned by the context), and the milliseconds each took in the last profiled cclr_sigma call
+ * (summed over its nvec vectors); cclr_last_sigma_op_ms returns the count, or CCLR_EINVAL if capacity is too small. */
+int cclr_sigma_op_count(const cclr_ctx *ctx);
+const char *cclr_sigma_op_text(const cclr_ctx *ctx, int k);
+int cclr_last_sigma_op_ms(const cclr_ctx *ctx, double *ms, int capacity);
 
 /* HOST-only: the reduced-space step of cclr_solve: beta[k] = (G - z[k] I)^{-1} rhs for nz shifts sharing one
  * L x L row-major matrix G, through one Hessenberg reduction.  All pointers are host pointers; beta is [nz][L]. */

@@ -11,7 +11,7 @@ import torch
 from . import _lib
 from ._lib import CclrError, SolveInfo  # noqa: F401
 
-__all__ = ["Context", "cclr_create", "cclr_sigma", "cclr_solve", "cclr_property", "cclr_zgemm", "cclr_ladder",
+__all__ = ["Context", "cclr_create", "cclr_ccsd", "cclr_sigma", "cclr_solve", "cclr_property", "cclr_zgemm", "cclr_ladder",
            "cclr_ring", "cclr_fp64_tensor_peak", "cclr_hbm_copy_peak", "CclrError"]
 
 
@@ -85,6 +85,15 @@ class Context:
         return dict(zip(("total", "ladder", "ring", "other_gemm", "layout"), list(ms)))
 
 
+    def last_sigma_ops(self):
+        """[(plan statement, ms)] of the last profiled cclr_sigma call."""
+        lib = _lib.load()
+        n = lib.cclr_sigma_op_count(self.handle)
+        ms = (C.c_double * n)()
+        _lib.check(min(lib.cclr_last_sigma_op_ms(self.handle, ms, n), 0), "cclr_last_sigma_op_ms")
+        return [(lib.cclr_sigma_op_text(self.handle, k).decode(), ms[k]) for k in range(n)]
+
+
 def cclr_create(o, v, fock, eri, t1, t2, flags=0):
     """eri: dict with the six packed classes of include/cclr.h (device tensors)."""
     lib = _lib.load()
@@ -98,6 +107,32 @@ def cclr_create(o, v, fock, eri, t1, t2, flags=0):
                          flags, _stream(), C.byref(h))
     _lib.check(rc, "cclr_create")
     return Context(h, o, v, keep=[eri["vvvv"]] if flags & ERI_INPLACE else [])
+
+
+def _eri_struct(o, v, eri):
+    oo, vv = o * (o - 1) // 2, v * (v - 1) // 2
+    sizes = dict(oooo=oo * oo, ooov=oo * o * v, oovv=oo * vv, ovvo=o * v * v * o, ovvv=o * v * vv, vvvv=vv * vv)
+    e = _lib.EriPacked()
+    for k, sz in sizes.items():
+        setattr(e, k, _dev(eri[k], "eri." + k, sz))
+    return e
+
+
+def cclr_ccsd(o, v, fock, eri, t1=None, t2=None, tol=1e-10, maxiter=100):
+    """Ground-state CCSD amplitudes on the device; returns (t1 [v*o], t2 [vv*oo], info).  t1/t2: start amplitudes (updated
+    in place) or None for zeros."""
+    oo, vv, n = o * (o - 1) // 2, v * (v - 1) // 2, o + v
+    if t1 is None:
+        t1 = torch.zeros(o * v, dtype=torch.complex128, device="cuda")
+    if t2 is None:
+        t2 = torch.zeros(vv * oo, dtype=torch.complex128, device="cuda")
+    e = _eri_struct(o, v, eri)
+    info = _lib.CcsdInfo()
+    rc = _lib.load().cclr_ccsd(o, v, _dev(fock, "fock", n * n), C.byref(e), _dev(t1, "t1", o * v), _dev(t2, "t2", vv * oo),
+                               float(tol), int(maxiter), _stream(), C.byref(info))
+    if rc not in (0, -4):
+        _lib.check(rc, "cclr_ccsd")
+    return t1, t2, info
 
 
 def cclr_sigma(ctx, x1, x2, omega=0.0, gamma=0.0, out1=None, out2=None):

@@ -63,6 +63,10 @@ void run_ops(cclr_ctx *ctx, const std::vector<ResolvedOp> &ops, bool profile) {
     float ms = 0.f;
     check(cudaEventElapsedTime(&ms, ctx->events[k], ctx->events[k + 1]), "cudaEventElapsedTime");
     ctx->ms[0] += ms;
+    if (&ops == &ctx->sigma_ops) {
+      if (ctx->op_ms.size() != ops.size()) ctx->op_ms.assign(ops.size(), 0.0);
+      ctx->op_ms[k] += ms;
+    }
     const int ph = ops[k].phase;
     if (ph >= PHASE_LADDER && ph <= PHASE_LAYOUT) ctx->ms[ph] += ms;
   }
@@ -227,8 +231,10 @@ extern "C" int cclr_sigma(cclr_ctx *ctx, const cclr_c128 *x1, const cclr_c128 *x
     return CCLR_EINVAL;
   }
   try {
-    if (ctx->profiling)
+    if (ctx->profiling) {
       for (double &m : ctx->ms) m = 0.0;
+      ctx->op_ms.assign(ctx->sigma_ops.size(), 0.0);
+    }
     for (int k = 0; k < nvec; ++k)
       cclr_sigma_one(ctx, (const c128 *)x1 + (size_t)k * ctx->n1, (const c128 *)x2 + (size_t)k * ctx->n2,
                      make_double2(omega, gamma), (c128 *)out1 + (size_t)k * ctx->n1, (c128 *)out2 + (size_t)k * ctx->n2,
@@ -334,6 +340,19 @@ extern "C" int cclr_last_sigma_ms(const cclr_ctx *ctx, double ms[5]) {
   if (!ctx || !ms) return CCLR_EINVAL;
   for (int k = 0; k < 5; ++k) ms[k] = ctx->ms[k];
   return CCLR_OK;
+}
+
+extern "C" int cclr_sigma_op_count(const cclr_ctx *ctx) { return ctx ? (int)ctx->sigma_ops.size() : CCLR_EINVAL; }
+
+extern "C" const char *cclr_sigma_op_text(const cclr_ctx *ctx, int k) {
+  if (!ctx || k < 0 || k >= (int)ctx->sigma_ops.size()) return "";
+  return ctx->sigma_ops[k].text.c_str();
+}
+
+extern "C" int cclr_last_sigma_op_ms(const cclr_ctx *ctx, double *ms, int capacity) {
+  if (!ctx || !ms || capacity < (int)ctx->sigma_ops.size()) return CCLR_EINVAL;
+  for (size_t k = 0; k < ctx->sigma_ops.size(); ++k) ms[k] = k < ctx->op_ms.size() ? ctx->op_ms[k] : 0.0;
+  return (int)ctx->sigma_ops.size();
 }
 
 extern "C" int cclr_property(cclr_ctx *ctx, const cclr_c128 *eta1, const cclr_c128 *eta2, const cclr_c128 *x1,

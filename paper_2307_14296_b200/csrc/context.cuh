@@ -20,6 +20,7 @@ struct cclr_ctx {
   // profiling of the last cclr_sigma call
   bool profiling = false;
   double ms[5] = {0, 0, 0, 0, 0};
+  std::vector<double> op_ms;      // per operation of the sigma plan, summed over the vectors of the last call
   std::vector<cudaEvent_t> events;
   // staging buffers of cclr_sigma_host
   c128 *host_stage = nullptr;

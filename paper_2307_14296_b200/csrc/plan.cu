@@ -238,6 +238,7 @@ void Plan::run(const std::vector<PlanStmt> &stmts, std::vector<ResolvedOp> *coll
     } else if (op == "gemm" || op == "perm" || op == "scat") {
       ResolvedOp r = op == "gemm" ? resolve_gemm(s) : resolve_perm(s);
       r.phase = s.phase;
+      for (auto &t : s.tok) r.text += (r.text.empty() ? "" : " ") + t;
       if (collect)
         collect->push_back(r);
       else

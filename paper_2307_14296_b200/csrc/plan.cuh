@@ -40,6 +40,7 @@ struct PlanStmt {
 struct ResolvedOp {
   int type = 0;                 // 0 = gemm, 1 = permute
   int phase = PHASE_OTHER;
+  std::string text;             // the plan statement (profiling output)
   // gemm
   int M = 0, N = 0, K = 0, a = -1, b = -1, c = -1;
   size_t aoff = 0, boff = 0, coff = 0;

@@ -26,7 +26,7 @@
 
 namespace {
 
-constexpr int ZG_BM = 128, ZG_BK = 16, ZG_STAGES = 4;   // CTA tile rows, K chunk, TMA ring depth; BN = 8*NG, NG = 4..8
+constexpr int ZG_BK = 16, ZG_STAGES = 4;   // K chunk, TMA ring depth; CTA tile BM x BN with BM = 128 | 64, BN = 8*NG, NG = 4..8
 
 // ---------------------------------------------------------------------------------------------------------------
 // PTX wrappers
@@ -335,25 +335,28 @@ cudaError_t launch(cudaStream_t st, const CUtensorMap &tmA, const CUtensorMap &t
 // one instantiation per N-tile width BN = 8*NG (NG DMMA column groups per warp), for both B layouts
 template <int NG>
 cudaError_t launch_ng(cudaStream_t st, const CUtensorMap &tmA, const CUtensorMap &tmB, const ZgemmArgs &args, int ctas,
-                      bool kn) {
-  return kn ? launch<ZG_BM, 8 * NG, ZG_BK, 32, 4 * NG, ZG_STAGES, true>(st, tmA, tmB, args, ctas)
-            : launch<ZG_BM, 8 * NG, ZG_BK, 32, 4 * NG, ZG_STAGES, false>(st, tmA, tmB, args, ctas);
+                      bool kn, int BM) {
+  if (BM == 128)
+    return kn ? launch<128, 8 * NG, ZG_BK, 32, 4 * NG, ZG_STAGES, true>(st, tmA, tmB, args, ctas)
+              : launch<128, 8 * NG, ZG_BK, 32, 4 * NG, ZG_STAGES, false>(st, tmA, tmB, args, ctas);
+  return kn ? launch<64, 8 * NG, ZG_BK, 16, 4 * NG, ZG_STAGES, true>(st, tmA, tmB, args, ctas)
+            : launch<64, 8 * NG, ZG_BK, 16, 4 * NG, ZG_STAGES, false>(st, tmA, tmB, args, ctas);
 }
 
 // C tile = alpha * sum_splits partial + beta * C for the K-split tail tiles
-__global__ void __launch_bounds__(256) zgemm_tail_reduce_kernel(const ZgemmArgs p, int BN) {
+__global__ void __launch_bounds__(256) zgemm_tail_reduce_kernel(const ZgemmArgs p, int BM, int BN) {
   const int t = p.main_tiles + (int)blockIdx.x;                 // tile id
   const int tiles_mn = p.tiles_m * p.tiles_n;
   const int batch = t / tiles_mn;
   const int tile_m = (t - batch * tiles_mn) / p.tiles_n, tile_n = (t - batch * tiles_mn) % p.tiles_n;
-  const c128 *part = p.partial + (size_t)blockIdx.x * p.tail_splits * (size_t)(ZG_BM * BN);
+  const c128 *part = p.partial + (size_t)blockIdx.x * p.tail_splits * (size_t)(BM * BN);
   const bool has_beta = p.beta.x != 0.0 || p.beta.y != 0.0;
-  for (int e = threadIdx.x; e < ZG_BM * BN; e += blockDim.x) {
+  for (int e = threadIdx.x; e < BM * BN; e += blockDim.x) {
     const int r = e / BN, c = e % BN;
-    const int row = tile_m * ZG_BM + r, col = tile_n * BN + c;
+    const int row = tile_m * BM + r, col = tile_n * BN + c;
     if (row >= p.M || col >= p.N) continue;
     c128 s = czero();
-    for (int k = 0; k < p.tail_splits; ++k) s = cadd(s, part[(size_t)k * (ZG_BM * BN) + e]);
+    for (int k = 0; k < p.tail_splits; ++k) s = cadd(s, part[(size_t)k * (BM * BN) + e]);
     c128 *dst = p.C + (size_t)batch * p.sc + (size_t)row * p.ldc + col;
     c128 out = cmul(p.alpha, s);
     if (has_beta) out = cadd(out, cmul(p.beta, *dst));
@@ -416,8 +419,11 @@ cudaError_t zgemm(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *
                   const c128 *B, long ldb, bool b_is_kn, bool conjB, c128 beta, c128 *C, long ldc, int batch, long sa,
                   long sb, long sc, const ZgemmWorkspace *ws) {
   if (M <= 0 || N <= 0 || batch <= 0) return cudaSuccess;
-  constexpr int BM = ZG_BM, BK = ZG_BK;
+  constexpr int BK = ZG_BK;
   const int sms = zgemm_num_sms();
+  // 64-row tiles when they cut the padding of M by more than 10 % (M of a few hundred: 300 -> 320 instead of 384)
+  const long pad128 = (M + 127L) / 128 * 128, pad64 = (M + 63L) / 64 * 64;
+  const int BM = (pad64 * 10 < pad128 * 9) ? 64 : 128;
   if (K <= 0) {  // C = beta * C
     zgemm_reduce_kernel<<<256, 256, 0, st>>>(nullptr, 0, M, N, alpha, beta, C, ldc, sc, batch);
     cclr_count_launch();
@@ -459,7 +465,7 @@ cudaError_t zgemm(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *
   if (ws && ws->buf) {
     if (tiles < sms && nchunks >= 16) {
       // the MN grid cannot fill the chip: split every tile along K
-      splits = (int)((2L * sms + tiles - 1) / tiles);
+      splits = (int)(2L * sms / tiles);                 // at most two full waves of CTAs
       if (splits > nchunks / 4) splits = nchunks / 4;
       if ((size_t)splits * tiles * tile_elems > ws->elems) splits = (int)(ws->elems / (tiles * tile_elems));
       if (splits > 1) main_tiles = 0; else splits = 1;
@@ -490,15 +496,15 @@ cudaError_t zgemm(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *
   }
   cudaError_t e;
   switch (NG) {
-    case 4: e = launch_ng<4>(st, tmA, tmB, args, ctas, b_is_kn); break;
-    case 5: e = launch_ng<5>(st, tmA, tmB, args, ctas, b_is_kn); break;
-    case 6: e = launch_ng<6>(st, tmA, tmB, args, ctas, b_is_kn); break;
-    case 7: e = launch_ng<7>(st, tmA, tmB, args, ctas, b_is_kn); break;
-    default: e = launch_ng<8>(st, tmA, tmB, args, ctas, b_is_kn); break;
+    case 4: e = launch_ng<4>(st, tmA, tmB, args, ctas, b_is_kn, BM); break;
+    case 5: e = launch_ng<5>(st, tmA, tmB, args, ctas, b_is_kn, BM); break;
+    case 6: e = launch_ng<6>(st, tmA, tmB, args, ctas, b_is_kn, BM); break;
+    case 7: e = launch_ng<7>(st, tmA, tmB, args, ctas, b_is_kn, BM); break;
+    default: e = launch_ng<8>(st, tmA, tmB, args, ctas, b_is_kn, BM); break;
   }
   if (e != cudaSuccess) return e;
   if (tail_tiles > 0 && splits > 1) {
-    zgemm_tail_reduce_kernel<<<tail_tiles, 256, 0, st>>>(args, BN);
+    zgemm_tail_reduce_kernel<<<tail_tiles, 256, 0, st>>>(args, BM, BN);
     cclr_count_launch();
     e = cudaGetLastError();
   }

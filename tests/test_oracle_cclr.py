@@ -212,3 +212,22 @@ def test_iterative_solver_reaches_dense_solution(small_lr):
     # true residual recomputed from sigma
     r = flat(*c.sigma(*ti, z=z)) + flat(*c.xi(X))
     assert np.linalg.norm(r) < 1e-10 * np.linalg.norm(flat(*c.xi(X)))
+
+
+def test_residual_is_the_gauss_quadrature_of_the_jacobian_along_the_ray():
+    """Omega(t) = Omega(0) + 1/2 sum_k A(s_k t) . t, s_k = 1/2 -+ 1/(2 sqrt 3), exactly (Omega is a quartic, A = dOmega/dt);
+    E(t) = eta0(t/2) . t.  cclr_ccsd (GPU ground state) rests on these identities."""
+    o, v = 3, 4
+    f, V = random_system(o, v, seed=21, diag_fock=False)
+    ints = ccsd.Integrals.from_full(f, V, o)
+    t1, t2 = random_amplitudes(o, v, 22, scale=0.2)
+    z1, z2 = np.zeros_like(t1), np.zeros_like(t2)
+    acc1, acc2 = ccsd.residual(ints, z1, z2)
+    assert np.abs(acc1 - ints.fvo).max() < 1e-15 and np.abs(acc2 - ints.vvoo).max() < 1e-15
+    for s in (0.5 - 0.5 / np.sqrt(3.0), 0.5 + 0.5 / np.sqrt(3.0)):
+        s1, s2 = cclr.CCLR(ints, s * t1, s * t2).sigma(t1, t2)
+        acc1, acc2 = acc1 + 0.5 * s1, acc2 + 0.5 * s2
+    w1, w2 = ccsd.residual(ints, t1, t2)
+    assert np.abs(acc1 - w1).max() < 1e-13 and np.abs(acc2 - w2).max() < 1e-13
+    e = cclr.dot(*cclr.CCLR(ints, 0.5 * t1, 0.5 * t2).eta0(), t1, t2)
+    assert abs(e - ccsd.energy(ints, t1, t2)) < 1e-13
