@@ -158,12 +158,17 @@ def workload_name(cfg, o, v):
 # ---------------------------------------------------------------------------------------------------------------
 # the CUDA path
 # ---------------------------------------------------------------------------------------------------------------
-def build_workload(cc, torch, synth, o, v, nvec, seed):
+def build_workload(cc, torch, synth, o, v, nvec, seed, ccsd):
     """Synthetic inputs generated on the device, context built in place over vvvv."""
     dev = "cuda"
     eri = {k: synth.eri_class(k, o, v, seed=0, device=dev) for k in ("oooo", "ooov", "oovv", "ovvo", "ovvv", "vvvv")}
     f = synth.fock(o, v, seed=0).to(dev)
     t1, t2 = synth.first_order_amplitudes(o, v, f, eri["oovv"])
+    ground = {"kind": "first-order doubles conj<ij||ab>/(e_i+e_j-e_a-e_b), t1=0"}
+    if ccsd:   # paper step 1 on the device: converge Omega(t) = 0 to 1e-10 from the first-order guess (cclr_ccsd)
+        t1, t2, ginfo = cc.cclr_ccsd(o, v, f, eri, t1, t2, tol=1e-10, maxiter=100)
+        ground = {"kind": "cclr_ccsd converged" if ginfo.converged else "cclr_ccsd NOT converged", "iterations": ginfo.iterations,
+                  "residual": ginfo.residual, "energy": [ginfo.energy_re, ginfo.energy_im], "seconds": ginfo.seconds}
     torch.cuda.synchronize()
     l0 = cc.cclr_kernel_launches()
     t0 = time.perf_counter()
@@ -174,7 +179,7 @@ def build_workload(cc, torch, synth, o, v, nvec, seed):
     keep = eri["vvvv"]
     del eri
     x1, x2 = synth.amplitudes(o, v, seed=100 + seed, cls1="x1", cls2="x2", device=dev, nvec=nvec)
-    return ctx, keep, x1, x2, create_s, create_launches
+    return ctx, keep, x1, x2, create_s, create_launches, ground
 
 
 def run_ours(args):
@@ -202,7 +207,7 @@ def run_ours(args):
     o, v, nvec = cfg["o"], cfg["v"], cfg["nvec"]
     n1, n2 = o * v, npair(o) * npair(v)
     omega, gamma = 0.0773, (0.0045 if args.config in (2, 5) else 0.0)
-    ctx, keep, x1, x2, create_s, create_launches = build_workload(cc, torch, synth, o, v, nvec, seed=rank)
+    ctx, keep, x1, x2, create_s, create_launches, ground = build_workload(cc, torch, synth, o, v, nvec, rank, args.ccsd)
     out1, out2 = torch.empty_like(x1), torch.empty_like(x2)
     flops_step = sigma_flops(o, v) * nvec
     cm = sigma_cmacs(o, v)
@@ -250,8 +255,7 @@ def run_ours(args):
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": workload_name(args.config, o, v), "o": o, "v": v, "nvec": nvec, "omega": omega,
-                   "gamma": gamma, "sigma_V": synth.sigma_v(v), "amplitudes": "first-order doubles conj<ij||ab>/(e_i+e_j-e_a-e_b), t1=0 "
-                   "(sigma does not depend on the convergence of T; DESIGN.md)", "parallelism": "replicas x%d" % world,
+                   "gamma": gamma, "sigma_V": synth.sigma_v(v), "ground_state": ground, "parallelism": "replicas x%d" % world,
                    "l2": "inputs larger than L2 (W_vvvv %.2f GB streamed every step)" % (npair(v) ** 2 * 16 / 1e9),
                    "flops_per_step": flops_step, "context_bytes": ctx.bytes()},
         "e2e": {"value": flops_step * world * args.steps / (e2e_ms * 1e-3) / 1e12, "unit": UNIT,
@@ -315,6 +319,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--tol", type=float, default=1e-10)
     ap.add_argument("--no-solve", action="store_true")
+    ap.add_argument("--ccsd", action="store_true", help="converge the ground-state amplitudes with cclr_ccsd first "
+                    "(default: first-order amplitudes; sigma does not depend on the convergence of T, DESIGN.md)")
     ap.add_argument("--ops", action="store_true", help="add the per-operation times of the last sigma step to the line")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
     args = ap.parse_args()
