@@ -283,6 +283,7 @@ def run_ours(args):
         line["phase_share"] = {k: val / tot for k, val in phases.items() if k != "total"}
         ring_ms = phases["ring"] / (args.steps * nvec)
         line["ring_tflops"] = 8.0 * cm["T8"] / (ring_ms * 1e-3) / 1e12
+        line["fp64_pipe_probe_tflops"] = {"dmma": peak, "dfma": cc.cclr_fp64_pipe_probe(1), "dmma+dfma by warp": cc.cclr_fp64_pipe_probe(2)}
         line["hbm_copy_gbs_measured"] = cc.cclr_hbm_copy_peak(4 << 30)
         line["clocks"] = clocks
     # ---- time per solve (rows C, D): 3 right-hand sides x the config's frequencies in one call -----------------

@@ -109,6 +109,23 @@ typedef struct {
 int cclr_ccsd(int o, int v, const cclr_c128 *fock, const cclr_eri_packed *eri, cclr_c128 *t1, cclr_c128 *t2, double tol,
               int maxiter, void *cuda_stream, cclr_ccsd_info *info);
 
+typedef struct {
+  int iterations;       /* subspace expansions performed                          */
+  int sigma_calls;      /* single-vector A.b products evaluated                   */
+  int subspace;         /* final trial-space dimension                            */
+  int converged;        /* 1 if every root met tol                                */
+  double max_residual;  /* max over roots of ||A x - theta x||_2, ||x||_2 = 1 (unique elements) */
+  double seconds;
+} cclr_eom_info;
+
+/* The nroots EOM-EE excitation energies of lowest real part = eigenvalues of the Jacobian A = poles of the response function
+ * and their right eigenvectors, by a block Davidson method on the same sigma routine
+ * and orbital-energy preconditioner as cclr_solve.  eig: HOST array [nroots] (A is not Hermitian: eigenvalues are complex
+ * in general, reading 17); r1_out [nroots][v*o], r2_out [nroots][vv*oo]: device, unit 2-norm over unique elements.
+ * Returns CCLR_OK or CCLR_ENOTCONV (best Ritz pairs written, info filled). */
+int cclr_eom(cclr_ctx *ctx, int nroots, double tol, int maxiter, cclr_c128 *eig, cclr_c128 *r1_out, cclr_c128 *r2_out,
+             cclr_eom_info *info);
+
 /* Cap the trial-space dimension of cclr_solve (memory = 2 * dim * (v*o + vv*oo) * 16 bytes); 0 = sized from the free
  * device memory.  When the space is full it is collapsed onto the current solutions and the iteration continues. */
 int cclr_set_max_subspace(cclr_ctx *ctx, int dim);
@@ -168,9 +185,18 @@ int cclr_last_sigma_op_ms(const cclr_ctx *ctx, double *ms, int capacity);
  * L x L row-major matrix G, through one Hessenberg reduction.  All pointers are host pointers; beta is [nz][L]. */
 int cclr_host_shifted_solve(int L, const cclr_c128 *G, const cclr_c128 *rhs, int nz, const cclr_c128 *z, cclr_c128 *beta);
 
+/* HOST-only: eigenvalues w [L] and right eigenvectors (columns of the row-major L x L matrix V, unit 2-norm) of a general
+ * complex row-major L x L matrix G — the reduced eigenproblem of cclr_eom (Hessenberg reduction + complex QR). */
+int cclr_host_eigen(int L, const cclr_c128 *G, cclr_c128 *w, cclr_c128 *V);
+
 /* FP64 tensor-core (DMMA m8n8k4) issue-rate probe: runs `iters` dependent-chain-free DMMA per warp on every SM
  * and returns the measured TFLOP/s in *tflops (host).  This is the roofline denominator used by bench.py. */
 int cclr_fp64_tensor_peak(void *cuda_stream, int iters, double *tflops);
+
+/* FP64 datapath probe: mode 0 = DMMA only (same as cclr_fp64_tensor_peak), 1 = vector DFMA only, 2 = half the warps DMMA and
+ * half DFMA.  On B200 all three give the same ~37 TFLOP/s: the tensor and vector FP64 paths share one datapath, so mixing
+ * them cannot raise a contraction above the DMMA peak. */
+int cclr_fp64_pipe_probe(void *cuda_stream, int mode, int iters, double *tflops);
 
 /* Streaming-copy probe over `bytes` of device memory (read + write) -> GB/s in *gbs (host). */
 int cclr_hbm_copy_peak(void *cuda_stream, size_t bytes, double *gbs);

@@ -11,7 +11,7 @@ import torch
 from . import _lib
 from ._lib import CclrError, SolveInfo  # noqa: F401
 
-__all__ = ["Context", "cclr_create", "cclr_ccsd", "cclr_sigma", "cclr_solve", "cclr_property", "cclr_zgemm", "cclr_ladder",
+__all__ = ["Context", "cclr_create", "cclr_ccsd", "cclr_eom", "cclr_sigma", "cclr_solve", "cclr_property", "cclr_zgemm", "cclr_ladder",
            "cclr_ring", "cclr_fp64_tensor_peak", "cclr_hbm_copy_peak", "CclrError"]
 
 
@@ -174,6 +174,19 @@ def cclr_solve(ctx, xi1, xi2, omegas, gamma=0.0, tol=1e-10, maxiter=200):
     return t1, t2, info
 
 
+def cclr_eom(ctx, nroots, tol=1e-8, maxiter=200):
+    """Lowest nroots eigenpairs of the Jacobian: (list of complex eigenvalues, r1 [nroots, v*o], r2 [nroots, vv*oo], info)."""
+    eig = (_lib.Complex * nroots)()
+    r1 = torch.empty((nroots, ctx.n1), dtype=torch.complex128, device="cuda")
+    r2 = torch.empty((nroots, ctx.n2), dtype=torch.complex128, device="cuda")
+    info = _lib.EomInfo()
+    rc = _lib.load().cclr_eom(ctx.handle, int(nroots), float(tol), int(maxiter), eig, _dev(r1, "r1"), _dev(r2, "r2"),
+                              C.byref(info))
+    if rc not in (0, -4):
+        _lib.check(rc, "cclr_eom")
+    return [complex(e.re, e.im) for e in eig], r1, r2, info
+
+
 def cclr_property(ctx, eta1, eta2, x1, x2):
     """Bilinear eta . x_k for every vector k; returns a Python list of complex."""
     nvec = x1.numel() // ctx.n1
@@ -224,6 +237,12 @@ def cclr_kernel_launches():
 def cclr_fp64_tensor_peak(iters=20000):
     out = C.c_double()
     _lib.check(_lib.load().cclr_fp64_tensor_peak(_stream(), iters, C.byref(out)), "cclr_fp64_tensor_peak")
+    return out.value
+
+
+def cclr_fp64_pipe_probe(mode, iters=20000):
+    out = C.c_double()
+    _lib.check(_lib.load().cclr_fp64_pipe_probe(_stream(), int(mode), iters, C.byref(out)), "cclr_fp64_pipe_probe")
     return out.value
 
 

@@ -25,6 +25,11 @@ class CcsdInfo(C.Structure):
                 ("energy_re", C.c_double), ("energy_im", C.c_double), ("seconds", C.c_double)]
 
 
+class EomInfo(C.Structure):
+    _fields_ = [("iterations", C.c_int), ("sigma_calls", C.c_int), ("subspace", C.c_int), ("converged", C.c_int),
+                ("max_residual", C.c_double), ("seconds", C.c_double)]
+
+
 class Complex(C.Structure):
     _fields_ = [("re", C.c_double), ("im", C.c_double)]
 
@@ -39,6 +44,8 @@ SIGNATURES = {
     "cclr_property": (C.c_int, [C.c_void_p, c128_p, c128_p, c128_p, c128_p, C.c_int, C.POINTER(Complex)]),
     "cclr_ccsd": (C.c_int, [C.c_int, C.c_int, c128_p, C.POINTER(EriPacked), c128_p, c128_p, C.c_double, C.c_int, C.c_void_p,
                             C.POINTER(CcsdInfo)]),
+    "cclr_eom": (C.c_int, [C.c_void_p, C.c_int, C.c_double, C.c_int, C.c_void_p, c128_p, c128_p, C.POINTER(EomInfo)]),
+    "cclr_host_eigen": (C.c_int, [C.c_int, c128_p, c128_p, c128_p]),
     "cclr_set_max_subspace": (C.c_int, [C.c_void_p, C.c_int]),
     "cclr_destroy": (None, [C.c_void_p]),
     "cclr_strerror": (C.c_char_p, [C.c_int]),
@@ -60,6 +67,7 @@ SIGNATURES = {
     "cclr_sigma_op_text": (C.c_char_p, [C.c_void_p, C.c_int]),
     "cclr_last_sigma_op_ms": (C.c_int, [C.c_void_p, C.POINTER(C.c_double), C.c_int]),
     "cclr_fp64_tensor_peak": (C.c_int, [C.c_void_p, C.c_int, C.POINTER(C.c_double)]),
+    "cclr_fp64_pipe_probe": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.POINTER(C.c_double)]),
     "cclr_hbm_copy_peak": (C.c_int, [C.c_void_p, C.c_size_t, C.POINTER(C.c_double)]),
 }
 

@@ -31,6 +31,38 @@ __global__ void __launch_bounds__(256) dmma_peak_kernel(double *out, int iters, 
   out[blockIdx.x * blockDim.x + threadIdx.x] = s;
 }
 
+// mode 1: vector DFMA only; mode 2: even warps DMMA, odd warps DFMA (do the two FP64 paths overlap? on B200 they do not)
+template <int MODE>
+__global__ void __launch_bounds__(256) fp64_mix_kernel(double *out, int iters, double seed) {
+  double c[8][2], d[16];
+  const double a = seed * (threadIdx.x + 1), b = seed * 3.0;
+#pragma unroll
+  for (int j = 0; j < 8; ++j) c[j][0] = c[j][1] = 0.0;
+#pragma unroll
+  for (int j = 0; j < 16; ++j) d[j] = seed * j;
+  const bool odd = (threadIdx.x >> 5) & 1;
+  for (int it = 0; it < iters; ++it) {
+    if (MODE == 2 && !odd) {
+#pragma unroll
+      for (int j = 0; j < 8; ++j)
+        asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                     : "+d"(c[j][0]), "+d"(c[j][1]) : "d"(a), "d"(b));
+    }
+    if (MODE == 1 || (MODE == 2 && odd)) {
+#pragma unroll
+      for (int r = 0; r < 4; ++r)
+#pragma unroll
+        for (int j = 0; j < 16; ++j) asm volatile("fma.rn.f64 %0, %1, %2, %0;" : "+d"(d[j]) : "d"(a), "d"(b));
+    }
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int j = 0; j < 8; ++j) s += c[j][0] + c[j][1];
+#pragma unroll
+  for (int j = 0; j < 16; ++j) s += d[j];
+  out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
 __global__ void copy_kernel(const double2 *__restrict__ src, double2 *__restrict__ dst, size_t n) {
   for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
     dst[i] = src[i];
@@ -81,6 +113,39 @@ extern "C" int cclr_fp64_tensor_peak(void *cuda_stream, int iters, double *tflop
   if (e != cudaSuccess) { g_last_cuda_error = e; return CCLR_ECUDA; }
   const double flops = (double)grid * (threads / 32) * (double)iters * 16.0 * (8.0 * 8.0 * 4.0 * 2.0);
   *tflops = flops / (best * 1e-3) / 1e12;
+  return CCLR_OK;
+}
+
+extern "C" int cclr_fp64_pipe_probe(void *cuda_stream, int mode, int iters, double *tflops) {
+  if (!tflops || iters < 1 || mode < 0 || mode > 2) return CCLR_EINVAL;
+  if (mode == 0) return cclr_fp64_tensor_peak(cuda_stream, iters, tflops);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const int grid = zgemm_num_sms() * 2, threads = 256;
+  double *out = nullptr;
+  cudaError_t e = cudaMalloc(&out, sizeof(double) * grid * threads);
+  if (e != cudaSuccess) { g_last_cuda_error = e; return CCLR_ENOMEM; }
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0);
+  cudaEventCreate(&e1);
+  float best = 1e30f;
+  for (int rep = 0; rep < 4; ++rep) {   // first repetition is the warm-up
+    cudaEventRecord(e0, st);
+    if (mode == 1) fp64_mix_kernel<1><<<grid, threads, 0, st>>>(out, iters, 1e-9);
+    else fp64_mix_kernel<2><<<grid, threads, 0, st>>>(out, iters, 1e-9);
+    cudaEventRecord(e1, st);
+    e = cudaEventSynchronize(e1);
+    if (e != cudaSuccess) break;
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    if (rep > 0 && ms < best) best = ms;
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(out);
+  if (e != cudaSuccess) { g_last_cuda_error = e; return CCLR_ECUDA; }
+  const double warps = (double)grid * (threads / 32);
+  // per warp and iteration: DMMA warps 8 x 512 flop, DFMA warps 64 fma x 32 lanes x 2 flop (both 4096)
+  *tflops = warps * (double)iters * 4096.0 / (best * 1e-3) / 1e12;
   return CCLR_OK;
 }
 

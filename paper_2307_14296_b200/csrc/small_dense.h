@@ -4,6 +4,7 @@
 // subspace) makes every shifted system an O(L^2) Hessenberg solve:  beta(z) = Q (H - z)^{-1} Q^H c.
 // Host-only, plain C++ (no CUDA); L is the subspace dimension (<= a few hundred).
 #pragma once
+#include <algorithm>
 #include <cmath>
 #include <complex>
 #include <vector>
@@ -104,5 +105,89 @@ struct Hessenberg {
     return true;
   }
 };
+
+// Eigenvalues w[k] and right eigenvectors (columns of V, row-major n x n, unit 2-norm) of a general complex matrix G
+// (row-major n x n): Householder reduction to Hessenberg form, single-shift complex QR with Givens rotations to the
+// Schur form G = U T U^H, back-substitution for the eigenvectors of T.  The reduced eigenproblem of the EOM-EE Davidson
+// solver (the sigma routine is shared with the eigen-solver).  Returns false if QR does not converge.
+inline bool eigen(const cplx *G, int n, std::vector<cplx> &w, std::vector<cplx> &V) {
+  Hessenberg hs;
+  hs.factor(G, n);
+  std::vector<cplx> &H = hs.H, &U = hs.Q;
+  auto h = [&](int i, int j) -> cplx & { return H[(size_t)i * n + j]; };
+  const double eps = 2.2e-16;
+  int hi = n - 1, iter = 0;
+  std::vector<cplx> cs(n), sn(n);
+  while (hi > 0) {
+    int l = hi;
+    for (; l > 0; --l) {
+      double sc = std::abs(h(l - 1, l - 1)) + std::abs(h(l, l));
+      if (sc == 0.0) sc = 1.0;
+      if (std::abs(h(l, l - 1)) <= eps * sc) { h(l, l - 1) = 0.0; break; }
+    }
+    if (l == hi) { --hi; iter = 0; continue; }
+    if (++iter > 300) return false;
+    // Wilkinson shift: the eigenvalue of the trailing 2 x 2 block closer to its last diagonal element
+    const cplx a = h(hi - 1, hi - 1), b = h(hi - 1, hi), c = h(hi, hi - 1), d = h(hi, hi);
+    const cplx tr2 = 0.5 * (a + d), disc = std::sqrt(tr2 * tr2 - (a * d - b * c));
+    cplx mu = std::abs(tr2 + disc - d) < std::abs(tr2 - disc - d) ? tr2 + disc : tr2 - disc;
+    if (iter % 11 == 10) mu = d + cplx(std::abs(h(hi, hi - 1)), std::abs(h(hi - 1, hi > 1 ? hi - 2 : 0)));   // exceptional
+    for (int k = l; k <= hi; ++k) h(k, k) -= mu;
+    for (int k = l; k < hi; ++k) {            // R = G_k^H ... G_l^H (H - mu)
+      const cplx x = h(k, k), y = h(k + 1, k);
+      const double r = std::sqrt(std::norm(x) + std::norm(y));
+      cs[k] = r > 0.0 ? x / r : cplx(1.0);
+      sn[k] = r > 0.0 ? y / r : cplx(0.0);
+      for (int j = k; j < n; ++j) {
+        const cplx t1 = h(k, j), t2 = h(k + 1, j);
+        h(k, j) = std::conj(cs[k]) * t1 + std::conj(sn[k]) * t2;
+        h(k + 1, j) = -sn[k] * t1 + cs[k] * t2;
+      }
+    }
+    for (int k = l; k < hi; ++k) {            // H = R G_l ... G_k + mu, U = U G_l ... G_k
+      for (int i = 0; i <= std::min(hi, k + 1); ++i) {
+        const cplx t1 = h(i, k), t2 = h(i, k + 1);
+        h(i, k) = t1 * cs[k] + t2 * sn[k];
+        h(i, k + 1) = -t1 * std::conj(sn[k]) + t2 * std::conj(cs[k]);
+      }
+      for (int i = 0; i < n; ++i) {
+        const cplx t1 = U[(size_t)i * n + k], t2 = U[(size_t)i * n + k + 1];
+        U[(size_t)i * n + k] = t1 * cs[k] + t2 * sn[k];
+        U[(size_t)i * n + k + 1] = -t1 * std::conj(sn[k]) + t2 * std::conj(cs[k]);
+      }
+    }
+    for (int k = l; k <= hi; ++k) h(k, k) += mu;
+  }
+  w.resize(n);
+  V.assign((size_t)n * n, cplx(0.0));
+  double tnorm = 0.0;
+  for (int i = 0; i < n; ++i)
+    for (int j = i; j < n; ++j) tnorm = std::max(tnorm, std::abs(h(i, j)));
+  const double tiny = std::max(tnorm, 1e-300) * eps;
+  std::vector<cplx> x(n);
+  for (int k = 0; k < n; ++k) {
+    w[k] = h(k, k);
+    for (int i = 0; i < n; ++i) x[i] = 0.0;
+    x[k] = 1.0;
+    for (int i = k - 1; i >= 0; --i) {
+      cplx sacc = 0.0;
+      for (int j = i + 1; j <= k; ++j) sacc += h(i, j) * x[j];
+      cplx den = h(i, i) - w[k];
+      if (std::abs(den) < tiny) den = tiny;
+      x[i] = -sacc / den;
+    }
+    double nv = 0.0;
+    for (int i = 0; i < n; ++i) {
+      cplx sacc = 0.0;
+      for (int j = 0; j <= k; ++j) sacc += U[(size_t)i * n + j] * x[j];
+      V[(size_t)i * n + k] = sacc;
+      nv += std::norm(sacc);
+    }
+    nv = std::sqrt(nv);
+    if (nv > 0.0)
+      for (int i = 0; i < n; ++i) V[(size_t)i * n + k] /= nv;
+  }
+  return true;
+}
 
 }  // namespace small_dense

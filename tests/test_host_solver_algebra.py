@@ -36,3 +36,27 @@ def test_structured_matrices():
         assert lib.cclr_host_shifted_solve(L, G.ctypes.data_as(C.c_void_p), rhs.ctypes.data_as(C.c_void_p), 1,
                                            z.ctypes.data_as(C.c_void_p), beta.ctypes.data_as(C.c_void_p)) == 0
         assert np.abs(beta[0] - np.linalg.solve(G - z[0] * np.eye(L), rhs)).max() < 1e-12
+
+
+@pytest.mark.parametrize("L", [1, 2, 3, 7, 40, 90])
+def test_host_eigen_matches_numpy(L):
+    """The reduced eigenproblem of cclr_eom (small_dense::eigen: Hessenberg + complex QR + back-substitution)."""
+    import ctypes as C
+    from paper_2307_14296_b200 import _lib
+    lib = _lib.load()
+    rng = np.random.default_rng(L)
+    G = rng.normal(size=(L, L)) + 1j * rng.normal(size=(L, L))
+    if L == 7:
+        G = np.diag(np.arange(7.0)).astype(complex) + np.triu(G, 1) * 1e-3      # nearly triangular, tiny couplings
+    if L == 40:
+        G = G + G.conj().T                                                      # Hermitian
+    G = np.ascontiguousarray(G)
+    w = np.zeros(L, complex)
+    V = np.zeros((L, L), complex)
+    rc = lib.cclr_host_eigen(L, G.ctypes.data_as(C.c_void_p), w.ctypes.data_as(C.c_void_p), V.ctypes.data_as(C.c_void_p))
+    assert rc == 0
+    ref = np.linalg.eigvals(G)
+    assert np.abs(np.sort_complex(w) - np.sort_complex(ref)).max() < 1e-10 * max(1.0, np.abs(ref).max())
+    for k in range(L):
+        assert abs(np.linalg.norm(V[:, k]) - 1.0) < 1e-12
+        assert np.linalg.norm(G @ V[:, k] - w[k] * V[:, k]) < 1e-9 * max(1.0, np.abs(ref).max())
