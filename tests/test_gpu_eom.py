@@ -60,7 +60,9 @@ def test_small_trial_space_collapses_and_still_converges(cfg1):
 
 
 def test_response_pole_sits_at_the_first_eom_energy(cfg1):
-    """t(w) = -(A - w)^-1 xi ~ -x_1 (l_1 . xi) / (theta_1 - w) next to the first pole."""
+    """t(z) = -(A - z)^-1 xi ~ -x_1 (l_1 . xi) / (theta_1 - z) next to the first pole.  A is not Hermitian
+    and the synthetic integrals have no time-reversal symmetry, so theta_1 is complex (Im ~ 1e-3 here, reading 17):
+    the pole is approached along z = theta_1 - delta with the damping gamma = Im theta_1 (Eq. 20-21)."""
     s = cfg1
     cc = s["cc"]
     eig, r1, r2, info = cc.cclr_eom(s["ctx"], 1, tol=1e-9, maxiter=200)
@@ -69,11 +71,11 @@ def test_response_pole_sits_at_the_first_eom_energy(cfg1):
     xi = s["c"].xi(synth.hermitian_operator(s["o"] + s["v"], 0, 0))
     a, b = packing.pack_amplitudes(*xi)
     xi1, xi2 = torch.from_numpy(a.reshape(1, -1)).cuda(), torch.from_numpy(b.reshape(1, -1)).cuda()
-    t1, t2, sinfo = cc.cclr_solve(s["ctx"], xi1, xi2, [th - 0.002, th - 0.004], 0.0, tol=1e-9, maxiter=300)
+    t1, t2, sinfo = cc.cclr_solve(s["ctx"], xi1, xi2, [th - 0.002, th - 0.004], eig[0].imag, tol=1e-9, maxiter=400)
     assert sinfo.converged == 1
     T = torch.cat([t1[0], t2[0]], dim=1)                                   # [2, n]
     norms = T.abs().pow(2).sum(dim=1).sqrt()
-    assert abs(float(norms[0] / norms[1]) - 2.0) < 0.1                      # 1/(theta - w) growth
+    assert abs(float(norms[0] / norms[1]) - 2.0) < 0.06                     # 1/(theta - w) growth
     x = torch.cat([r1[0], r2[0]])
     overlap = abs(complex(torch.dot(x.conj(), T[0]))) / float(norms[0])
     assert overlap > 0.99                                                   # and it grows along the eigenvector
