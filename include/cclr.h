@@ -87,6 +87,11 @@ int cclr_solve(cclr_ctx *ctx, const cclr_c128 *xi1, const cclr_c128 *xi2, int nr
                int nomega, double gamma, double tol, int maxiter, cclr_c128 *t1_out, cclr_c128 *t2_out,
                cclr_solve_info *info);
 
+/* xi^X = <mu| exp(-T) X exp(T) |R>, the right-hand side of the response equations for the one-body perturbation X
+ * (Eq. 19; S-Eq. 1-3): X is a DEVICE [n][n] row-major matrix <p|X|q>, n = o + v (all four
+ * blocks are used); xi1 [v*o], xi2 [vv*oo] device outputs. */
+int cclr_xi(cclr_ctx *ctx, const cclr_c128 *X, cclr_c128 *xi1, cclr_c128 *xi2);
+
 /* result[k] = sum_ai eta1 x1_k + sum_{a<b,i<j} eta2 x2_k  (bilinear, no conjugation; PAPER.md:137 Eq. 15, :203) for
  * nvec vectors x_k; result is a HOST array of nvec complex numbers. */
 int cclr_property(cclr_ctx *ctx, const cclr_c128 *eta1, const cclr_c128 *eta2, const cclr_c128 *x1,

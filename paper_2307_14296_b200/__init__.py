@@ -11,7 +11,7 @@ import torch
 from . import _lib
 from ._lib import CclrError, SolveInfo  # noqa: F401
 
-__all__ = ["Context", "cclr_create", "cclr_ccsd", "cclr_eom", "cclr_sigma", "cclr_solve", "cclr_property", "cclr_zgemm", "cclr_ladder",
+__all__ = ["Context", "cclr_create", "cclr_ccsd", "cclr_eom", "cclr_xi", "cclr_sigma", "cclr_solve", "cclr_property", "cclr_zgemm", "cclr_ladder",
            "cclr_ring", "cclr_fp64_tensor_peak", "cclr_hbm_copy_peak", "CclrError"]
 
 
@@ -185,6 +185,15 @@ def cclr_eom(ctx, nroots, tol=1e-8, maxiter=200):
     if rc not in (0, -4):
         _lib.check(rc, "cclr_eom")
     return [complex(e.re, e.im) for e in eig], r1, r2, info
+
+
+def cclr_xi(ctx, X):
+    """xi^X for a one-body operator X ([n, n] complex128 CUDA tensor): returns (xi1 [v*o], xi2 [vv*oo])."""
+    n = ctx.o + ctx.v
+    xi1 = torch.empty(ctx.n1, dtype=torch.complex128, device="cuda")
+    xi2 = torch.empty(ctx.n2, dtype=torch.complex128, device="cuda")
+    _lib.check(_lib.load().cclr_xi(ctx.handle, _dev(X, "X", n * n), _dev(xi1, "xi1"), _dev(xi2, "xi2")), "cclr_xi")
+    return xi1, xi2
 
 
 def cclr_property(ctx, eta1, eta2, x1, x2):

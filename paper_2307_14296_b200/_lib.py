@@ -41,6 +41,7 @@ SIGNATURES = {
     "cclr_sigma": (C.c_int, [C.c_void_p, c128_p, c128_p, C.c_int, C.c_double, C.c_double, c128_p, c128_p]),
     "cclr_solve": (C.c_int, [C.c_void_p, c128_p, c128_p, C.c_int, C.POINTER(C.c_double), C.c_int, C.c_double,
                              C.c_double, C.c_int, c128_p, c128_p, C.POINTER(SolveInfo)]),
+    "cclr_xi": (C.c_int, [C.c_void_p, c128_p, c128_p, c128_p]),
     "cclr_property": (C.c_int, [C.c_void_p, c128_p, c128_p, c128_p, c128_p, C.c_int, C.POINTER(Complex)]),
     "cclr_ccsd": (C.c_int, [C.c_int, C.c_int, c128_p, C.POINTER(EriPacked), c128_p, c128_p, C.c_double, C.c_int, C.c_void_p,
                             C.POINTER(CcsdInfo)]),

@@ -88,6 +88,7 @@ void destroy(cclr_ctx *ctx) {
   if (ctx->dot_partial) cudaFree(ctx->dot_partial);
   if (ctx->dot_out) cudaFree(ctx->dot_out);
   if (ctx->host_stage) cudaFree(ctx->host_stage);
+  if (ctx->xblocks) cudaFree(ctx->xblocks);
   for (cudaEvent_t ev : ctx->events) cudaEventDestroy(ev);
   delete ctx;
 }
@@ -205,6 +206,15 @@ extern "C" int cclr_create(int o, int v, const cclr_c128 *fock, const cclr_eri_p
     P.compile(CCLR_PLAN_SIGMA, ctx->sigma_ops);
     P.compile(PLAN_LADDER, ctx->ladder_ops);
     P.compile(PLAN_RING, ctx->ring_ops);
+    // the xi plan works on blocks of the operator matrix kept in a small context buffer
+    const size_t no = (size_t)o, nv = (size_t)v;
+    check(cudaMalloc(&ctx->xblocks, (no * no + 2 * no * nv + nv * nv) * sizeof(c128)), "cudaMalloc(X blocks)");
+    ctx->extra_bytes += (no * no + 2 * no * nv + nv * nv) * sizeof(c128);
+    P.bind("xoo", "mi", ctx->xblocks);
+    P.bind("xov", "me", ctx->xblocks + no * no);
+    P.bind("xvo", "ai", ctx->xblocks + no * no + no * nv);
+    P.bind("xvv", "ae", ctx->xblocks + no * no + 2 * no * nv);
+    P.compile(CCLR_PLAN_XI, ctx->xi_ops);
     cclr_ensure_dot_scratch(ctx, 256);
   } catch (const PlanError &e) {
     destroy(ctx);
@@ -295,6 +305,28 @@ extern "C" int cclr_ring(cclr_ctx *ctx, const cclr_c128 *x2, cclr_c128 *out2) {
   try {
     bind_vectors(ctx, nullptr, (const c128 *)x2, nullptr, (c128 *)out2);
     run_ops(ctx, ctx->ring_ops, false);
+  } catch (const PlanError &e) {
+    return cclr_fail(e);
+  }
+  return CCLR_OK;
+}
+
+extern "C" int cclr_xi(cclr_ctx *ctx, const cclr_c128 *X, cclr_c128 *xi1, cclr_c128 *xi2) {
+  if (!ctx || !X || !xi1 || !xi2) {
+    cclr_set_error("cclr_xi: null pointer", cudaSuccess);
+    return CCLR_EINVAL;
+  }
+  try {
+    const size_t o = (size_t)ctx->o, v = (size_t)ctx->v, nf = o + v;
+    const c128 *F = (const c128 *)X;
+    struct { size_t off, r0, c0, rows, cols; } blocks[4] = {
+        {0, 0, 0, o, o}, {o * o, 0, o, o, v}, {o * o + o * v, o, 0, v, o}, {o * o + 2 * o * v, o, o, v, v}};
+    for (auto &b : blocks)
+      check(cudaMemcpy2DAsync(ctx->xblocks + b.off, b.cols * sizeof(c128), F + b.r0 * nf + b.c0, nf * sizeof(c128),
+                              b.cols * sizeof(c128), b.rows, cudaMemcpyDeviceToDevice, ctx->st),
+            "copy X block");
+    bind_vectors(ctx, nullptr, nullptr, (c128 *)xi1, (c128 *)xi2);
+    run_ops(ctx, ctx->xi_ops, false);
   } catch (const PlanError &e) {
     return cclr_fail(e);
   }

@@ -11,7 +11,8 @@ struct cclr_ctx {
   cudaStream_t st = nullptr;
   Plan *plan = nullptr;
   ZgemmWorkspace ws;
-  std::vector<ResolvedOp> sigma_ops, ladder_ops, ring_ops;
+  std::vector<ResolvedOp> sigma_ops, ladder_ops, ring_ops, xi_ops;
+  c128 *xblocks = nullptr;        // X_oo, X_ov, X_vo, X_vv of cclr_xi, contiguous
   int x1_id = -1, x2_id = -1, out1_id = -1, out2_id = -1;
   double *D = nullptr;            // orbital-energy denominators over unique elements, [n1 + n2]
   // small device scratch for dot products (vecops.cu)

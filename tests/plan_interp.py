@@ -324,3 +324,16 @@ def run_sigma(it, x1, x2p, z):
     it.bind("out2", "(ab)(ij)", np.zeros(npair(v) * npair(o), complex))
     it.run(load_plan("CCLR_PLAN_SIGMA"))
     return it.get("out1").copy(), it.get("out2").copy()
+
+
+def run_xi(it, X):
+    """Execute CCLR_PLAN_XI (after run_sigma has declared the work buffers it reuses) for the one-body matrix X [n][n]."""
+    o, v = it.o, it.v
+    it.bind("xoo", "mi", np.ascontiguousarray(X[:o, :o]).reshape(-1))
+    it.bind("xov", "me", np.ascontiguousarray(X[:o, o:]).reshape(-1))
+    it.bind("xvo", "ai", np.ascontiguousarray(X[o:, :o]).reshape(-1))
+    it.bind("xvv", "ae", np.ascontiguousarray(X[o:, o:]).reshape(-1))
+    it.bind("out1", "ai", np.zeros(v * o, complex))
+    it.bind("out2", "(ab)(ij)", np.zeros(npair(v) * npair(o), complex))
+    it.run(load_plan("CCLR_PLAN_XI"))
+    return it.get("out1").copy(), it.get("out2").copy()

@@ -148,3 +148,14 @@ def test_zero_right_hand_side_gives_zero(cfg1):
     z1, z2 = torch.zeros_like(s["xi1"][:1]), torch.zeros_like(s["xi2"][:1])
     t1, t2, info = s["cc"].cclr_solve(s["ctx"], z1, z2, [0.0773], 0.0045)
     assert info.converged == 1 and t1.abs().max().item() == 0.0 and t2.abs().max().item() == 0.0
+
+
+def test_xi_built_on_the_device_matches_oracle(cfg1):
+    """cclr_xi (S-Eq. 2-3) for the dipole-type and the imaginary-antisymmetric operators."""
+    s = cfg1
+    for k, X in enumerate(s["ops"]):
+        g1, g2 = s["cc"].cclr_xi(s["ctx"], torch.from_numpy(np.ascontiguousarray(X)).cuda())
+        torch.cuda.synchronize()
+        w1, w2 = packing.pack_amplitudes(*s["xis"][k])
+        assert np.linalg.norm(g1.cpu().numpy() - w1.reshape(-1)) <= 1e-12 * np.linalg.norm(w1)
+        assert np.linalg.norm(g2.cpu().numpy() - w2.reshape(-1)) <= 1e-12 * np.linalg.norm(w2)

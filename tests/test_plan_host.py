@@ -57,3 +57,16 @@ def test_sigma_plan_reproduces_oracle_sigma(o, v, chunk):
         r1, r2 = packing.pack_amplitudes(*c.sigma(x1, x2, z))
         assert np.linalg.norm(s1 - r1) <= 1e-12 * np.linalg.norm(r1)
         assert np.linalg.norm(s2 - r2) <= 1e-12 * np.linalg.norm(r2)
+
+
+@pytest.mark.parametrize("o,v", [(3, 5), (4, 6)])
+def test_xi_plan_reproduces_oracle_xi(o, v):
+    from conftest import random_hermitian
+    it, c = _setup(o, v, seed=70 + v)
+    x1, x2 = random_amplitudes(o, v, seed=71, scale=1.0)
+    plan_interp.run_sigma(it, *packing.pack_amplitudes(x1, x2), 0.0)          # declares the shared work buffers
+    X = random_hermitian(o + v, 72) + 0.3j * np.random.default_rng(73).normal(size=(o + v, o + v))   # not even Hermitian
+    s1, s2 = plan_interp.run_xi(it, X)
+    r1, r2 = packing.pack_amplitudes(*c.xi(X))
+    assert np.linalg.norm(s1.reshape(-1) - r1.reshape(-1)) <= 1e-12 * np.linalg.norm(r1)
+    assert np.linalg.norm(s2.reshape(-1) - r2.reshape(-1)) <= 1e-12 * np.linalg.norm(r2)
