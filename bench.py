@@ -147,6 +147,9 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+# DRAM traffic of one ladder launch from the ncu captures under profiles/ (bytes; None where no capture exists)
+NCU_LADDER_TRAFFIC = {3: 7.12e9, 4: 43.55e9}
+
 CONFIGS = {1: dict(o=4, v=20, nvec=1), 2: dict(o=10, v=80, nvec=1), 3: dict(o=24, v=200, nvec=1),
            4: dict(o=34, v=300, nvec=1), 5: dict(o=18, v=150, nvec=3)}
 
@@ -274,7 +277,9 @@ def run_ours(args):
             "frac": lad_flops / (lad_ms * 1e-3) / 1e12 / peak,
             "peak_source": "FP64 tensor (DMMA m8n8k4) issue-rate probe cclr_fp64_tensor_peak measured in this run; "
                            "MEASURED_PEAKS.json has no FP64 entry (nominal HGX B200: 37 TFLOP/s)",
-            "traffic": None, "algorithmic_bytes": 16.0 * (npair(v) ** 2 + 2 * n2), "ms_per_launch": lad_ms,
+            "traffic": NCU_LADDER_TRAFFIC.get(args.config), "traffic_source": "profiles/r01_config4_sigma_step_ncu.md / "
+            "r01_zgemm_ncu_full_config3.md (dram__bytes_read.sum + dram__bytes_write.sum of the ladder launch)",
+            "algorithmic_bytes": 16.0 * (npair(v) ** 2 + 2 * n2), "ms_per_launch": lad_ms,
         }
         tot = max(phases["total"], 1e-9)
         if args.ops:

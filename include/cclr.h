@@ -69,6 +69,13 @@ int cclr_create(int o, int v, const cclr_c128 *fock, const cclr_eri_packed *eri,
 int cclr_sigma(cclr_ctx *ctx, const cclr_c128 *x1, const cclr_c128 *x2, int nvec, double omega, double gamma,
                cclr_c128 *out1, cclr_c128 *out2);
 
+/* out = l (A - (omega + i*gamma)) for nvec left vectors l1[a][i] = l^i_a, l2[(ab)][(ij)] = l^ij_ab (same layouts as amplitudes):
+ * the left Jacobian transform of the Lambda equations and of left response equations (Eq. 13; S-Eq. 13,
+ * PAPER.md:895-901 in the reading of DESIGN.md: the term-by-term adjoint of S-Eq. 11-12).  Same cost as cclr_sigma; the
+ * pp ladder runs with W_vvvv as the [K][N] operand, so nothing is stored twice.  out must not alias l. */
+int cclr_sigma_left(cclr_ctx *ctx, const cclr_c128 *l1, const cclr_c128 *l2, int nvec, double omega, double gamma,
+                    cclr_c128 *out1, cclr_c128 *out2);
+
 typedef struct {
   int iterations;       /* subspace expansions performed                                   */
   int sigma_calls;      /* number of single-vector A.b products evaluated                  */

@@ -112,6 +112,56 @@ class CCLR:
         s2 += 0.5 * np.einsum("abef,efij->abij", self.Wabef, r2)                                # T11
         return s1 - z * r1, s2 - z * r2
 
+    # ---- left transform l A (adjoint of S-Eq. 11-12 term by term) ------------------------------------------
+    def sigma_left(self, l1, l2, z=0.0):
+        """l (A - z) for l1[a,i] = l^i_a, l2[a,b,i,j] = l^ij_ab: the left Jacobian transform of the Lambda / left response
+        equations (Eq. 13; S-Eq. 13, whose printed form has three misprints, DESIGN.md
+        reading 5).  Written here as the adjoint of sigma(): every term of S-Eq. 11-12 is bilinear in an intermediate and r,
+        so with <l, s> = sum l1 s1 + 1/4 sum l2 s2 each term  s[out] += W . r[in]  gives  L[in] += W . l[out]; the three-index
+        terms T3, T4, T9, T10 produce the one-index intermediates G of S-Eq. 26-27."""
+        I, t2 = self.I, self.t2
+        GL = np.einsum("abij,afij->bf", l2, t2)            # = -2 G^f_b of S-Eq. 26
+        GO = np.einsum("abij,abin->jn", l2, t2)            # =  2 G^j_n of S-Eq. 27
+        L1 = (np.einsum("ai,ae->ei", l1, self.Fae) - np.einsum("ai,mi->am", l1, self.Fmi)            # S1, S2
+              + np.einsum("ai,maei->em", l1, self.Wmbej)                                            # S4
+              - 0.5 * np.einsum("abij,mbij->am", l2, self.Wmbij)                                    # T1
+              + 0.5 * np.einsum("abij,abej->ei", l2, self.Wabej)                                    # T2
+              + 0.5 * np.einsum("bf,bmfe->em", GL, self.Wamef)                                      # T3
+              - 0.5 * np.einsum("jn,nmje->em", GO, self.Wmnie))                                     # T4
+        L2 = _Pab(_Pij(np.einsum("ai,me->aeim", l1, self.Fme)))                                     # S3
+        L2 += _Pij(np.einsum("ai,amef->efim", l1, self.Wamef))                                      # S5
+        L2 -= _Pab(np.einsum("ai,mnie->aemn", l1, self.Wmnie))                                      # S6
+        L2 += _Pab(np.einsum("abij,be->aeij", l2, self.Fae))                                        # T5
+        L2 -= _Pij(np.einsum("abij,mj->abim", l2, self.Fmi))                                        # T6
+        L2 += 0.5 * np.einsum("abij,mnij->abmn", l2, self.Wmnij)                                    # T7
+        L2 += _Pab(_Pij(np.einsum("abij,mbej->aeim", l2, self.Wmbej)))                              # T8
+        L2 -= 0.5 * _Pab(np.einsum("af,nmfe->eamn", GL, I.oovv))                                    # T9
+        L2 -= 0.5 * _Pij(np.einsum("in,nmfe->feim", GO, I.oovv))                                    # T10
+        L2 += 0.5 * np.einsum("abij,abef->efij", l2, self.Wabef)                                    # T11
+        return L1 - z * l1, L2 - z * l2
+
+    def solve_lambda_iterative(self, tol=1e-11, maxiter=200):
+        """lambda A = -eta0 by a plain preconditioned Krylov iteration on sigma_left (same scheme as solve_iterative)."""
+        o, v = self.o, self.v
+        d = flat(self.D1 + 0j, self.D2 + 0j)
+        rhs = flat(*self.eta0())
+        B, S = [], []
+        new = -rhs / d
+        for it in range(maxiter):
+            for _ in range(2):
+                for bj in B:
+                    new = new - bj * np.vdot(bj, new)
+            new = new / np.linalg.norm(new)
+            B.append(new)
+            S.append(flat(*self.sigma_left(*unflat(new, o, v))))
+            Bm, Sm = np.array(B).T, np.array(S).T
+            beta = np.linalg.solve(Bm.conj().T @ Sm, -Bm.conj().T @ rhs)
+            r = Sm @ beta + rhs
+            if np.linalg.norm(r) <= tol * np.linalg.norm(rhs):
+                break
+            new = -r / d
+        return unflat(Bm @ beta, o, v)
+
     # ---- dense algebra over unique elements (small sizes) ---------------------------------------------------
     def dim(self):
         o, v = self.o, self.v

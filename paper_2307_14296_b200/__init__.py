@@ -149,6 +149,20 @@ def cclr_sigma(ctx, x1, x2, omega=0.0, gamma=0.0, out1=None, out2=None):
     return out1, out2
 
 
+def cclr_sigma_left(ctx, l1, l2, omega=0.0, gamma=0.0, out1=None, out2=None):
+    """out = l (A - (omega + i gamma)): the left Jacobian transform.  l1: [nvec, v*o] (or [v*o]), l2: [nvec, vv*oo]."""
+    nvec = l1.numel() // ctx.n1
+    if out1 is None:
+        out1 = torch.empty_like(l1)
+    if out2 is None:
+        out2 = torch.empty_like(l2)
+    rc = _lib.load().cclr_sigma_left(ctx.handle, _dev(l1, "l1", nvec * ctx.n1), _dev(l2, "l2", nvec * ctx.n2), nvec,
+                                     float(omega), float(gamma), _dev(out1, "out1", nvec * ctx.n1),
+                                     _dev(out2, "out2", nvec * ctx.n2))
+    _lib.check(rc, "cclr_sigma_left")
+    return out1, out2
+
+
 def cclr_sigma_host(ctx, x1, x2, omega, gamma, out1, out2):
     """Same through HOST tensors (copies inside the call)."""
     nvec = x1.numel() // ctx.n1

@@ -39,6 +39,7 @@ SIGNATURES = {
     "cclr_create": (C.c_int, [C.c_int, C.c_int, c128_p, C.POINTER(EriPacked), c128_p, c128_p, C.c_uint, C.c_void_p,
                               C.POINTER(C.c_void_p)]),
     "cclr_sigma": (C.c_int, [C.c_void_p, c128_p, c128_p, C.c_int, C.c_double, C.c_double, c128_p, c128_p]),
+    "cclr_sigma_left": (C.c_int, [C.c_void_p, c128_p, c128_p, C.c_int, C.c_double, C.c_double, c128_p, c128_p]),
     "cclr_solve": (C.c_int, [C.c_void_p, c128_p, c128_p, C.c_int, C.POINTER(C.c_double), C.c_int, C.c_double,
                              C.c_double, C.c_int, c128_p, c128_p, C.POINTER(SolveInfo)]),
     "cclr_xi": (C.c_int, [C.c_void_p, c128_p, c128_p, c128_p]),

@@ -95,10 +95,10 @@ void destroy(cclr_ctx *ctx) {
 
 }  // namespace
 
-void cclr_sigma_one(cclr_ctx *ctx, const c128 *x1, const c128 *x2, c128 z, c128 *out1, c128 *out2, bool profile) {
+void cclr_sigma_one(cclr_ctx *ctx, const c128 *x1, const c128 *x2, c128 z, c128 *out1, c128 *out2, bool profile, bool left) {
   bind_vectors(ctx, x1, x2, out1, out2);
   ctx->plan->set_scalar(0, make_double2(-z.x, -z.y));
-  run_ops(ctx, ctx->sigma_ops, profile);
+  run_ops(ctx, left ? ctx->left_ops : ctx->sigma_ops, profile);
 }
 
 void cclr_ensure_dot_scratch(cclr_ctx *ctx, int npairs) {
@@ -215,6 +215,7 @@ extern "C" int cclr_create(int o, int v, const cclr_c128 *fock, const cclr_eri_p
     P.bind("xvo", "ai", ctx->xblocks + no * no + no * nv);
     P.bind("xvv", "ae", ctx->xblocks + no * no + 2 * no * nv);
     P.compile(CCLR_PLAN_XI, ctx->xi_ops);
+    P.compile(CCLR_PLAN_SIGMA_LEFT, ctx->left_ops);
     cclr_ensure_dot_scratch(ctx, 256);
   } catch (const PlanError &e) {
     destroy(ctx);
@@ -249,6 +250,23 @@ extern "C" int cclr_sigma(cclr_ctx *ctx, const cclr_c128 *x1, const cclr_c128 *x
       cclr_sigma_one(ctx, (const c128 *)x1 + (size_t)k * ctx->n1, (const c128 *)x2 + (size_t)k * ctx->n2,
                      make_double2(omega, gamma), (c128 *)out1 + (size_t)k * ctx->n1, (c128 *)out2 + (size_t)k * ctx->n2,
                      ctx->profiling);
+  } catch (const PlanError &e) {
+    return cclr_fail(e);
+  }
+  return CCLR_OK;
+}
+
+extern "C" int cclr_sigma_left(cclr_ctx *ctx, const cclr_c128 *l1, const cclr_c128 *l2, int nvec, double omega,
+                               double gamma, cclr_c128 *out1, cclr_c128 *out2) {
+  if (!ctx || !l1 || !l2 || !out1 || !out2 || nvec < 1 || l1 == out1 || l2 == out2) {
+    cclr_set_error("cclr_sigma_left: null pointer, nvec < 1 or aliased output", cudaSuccess);
+    return CCLR_EINVAL;
+  }
+  try {
+    for (int k = 0; k < nvec; ++k)
+      cclr_sigma_one(ctx, (const c128 *)l1 + (size_t)k * ctx->n1, (const c128 *)l2 + (size_t)k * ctx->n2,
+                     make_double2(omega, gamma), (c128 *)out1 + (size_t)k * ctx->n1, (c128 *)out2 + (size_t)k * ctx->n2,
+                     false, true);
   } catch (const PlanError &e) {
     return cclr_fail(e);
   }

@@ -11,7 +11,7 @@ struct cclr_ctx {
   cudaStream_t st = nullptr;
   Plan *plan = nullptr;
   ZgemmWorkspace ws;
-  std::vector<ResolvedOp> sigma_ops, ladder_ops, ring_ops, xi_ops;
+  std::vector<ResolvedOp> sigma_ops, ladder_ops, ring_ops, xi_ops, left_ops, eta_ops;
   c128 *xblocks = nullptr;        // X_oo, X_ov, X_vo, X_vv of cclr_xi, contiguous
   int x1_id = -1, x2_id = -1, out1_id = -1, out2_id = -1;
   double *D = nullptr;            // orbital-energy denominators over unique elements, [n1 + n2]
@@ -35,5 +35,7 @@ void cclr_set_error(const std::string &msg, cudaError_t e);
 int cclr_fail(const PlanError &e);
 
 // out = A x for one vector on the context's stream (no shift when z == 0); throws PlanError
-void cclr_sigma_one(cclr_ctx *ctx, const c128 *x1, const c128 *x2, c128 z, c128 *out1, c128 *out2, bool profile);
+// left = true: out = l (A - z), the left transform (CCLR_PLAN_SIGMA_LEFT)
+void cclr_sigma_one(cclr_ctx *ctx, const c128 *x1, const c128 *x2, c128 z, c128 *out1, c128 *out2, bool profile,
+                    bool left = false);
 void cclr_ensure_dot_scratch(cclr_ctx *ctx, int npairs);

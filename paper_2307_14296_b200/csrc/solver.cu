@@ -44,9 +44,9 @@ struct Solver : subspace::Space {
 
 }  // namespace
 
-extern "C" int cclr_solve(cclr_ctx *ctx, const cclr_c128 *xi1, const cclr_c128 *xi2, int nrhs, const double *omegas,
-                          int nomega, double gamma, double tol, int maxiter, cclr_c128 *t1_out, cclr_c128 *t2_out,
-                          cclr_solve_info *info) {
+static int solve_impl(cclr_ctx *ctx, const cclr_c128 *xi1, const cclr_c128 *xi2, int nrhs, const double *omegas,
+                      int nomega, double gamma, double tol, int maxiter, cclr_c128 *t1_out, cclr_c128 *t2_out,
+                      cclr_solve_info *info, bool left) {
   if (!ctx || !xi1 || !xi2 || !omegas || !t1_out || !t2_out || nrhs < 1 || nomega < 1 || !(tol > 0.0) || maxiter < 1) {
     cclr_set_error("cclr_solve: null pointer, nrhs < 1, nomega < 1, tol <= 0 or maxiter < 1", cudaSuccess);
     return CCLR_EINVAL;
@@ -91,7 +91,7 @@ extern "C" int cclr_solve(cclr_ctx *ctx, const cclr_c128 *xi1, const cclr_c128 *
       const int nsys = nr * nomega;
       Solver S;
       S.ctx = ctx; S.st = st; S.n = n; S.n1 = n1; S.n2 = n2;
-      S.maxdim = maxdim; S.rcap = rcap; S.nrhs = nr;
+      S.maxdim = maxdim; S.rcap = rcap; S.nrhs = nr; S.left = left;
       S.Bm.alloc((size_t)maxdim * n, "cudaMalloc(trial space)");
       S.Sm.alloc((size_t)maxdim * n, "cudaMalloc(sigma space)");
       S.XI.alloc((size_t)nr * n, "cudaMalloc(xi)");
@@ -363,6 +363,29 @@ extern "C" int cclr_solve(cclr_ctx *ctx, const cclr_c128 *xi1, const cclr_c128 *
   if (info) *info = res;
   if (rc == CCLR_ENOTCONV) cclr_set_error("cclr_solve: maxiter reached before every system met tol", cudaSuccess);
   return rc;
+}
+
+extern "C" int cclr_solve(cclr_ctx *ctx, const cclr_c128 *xi1, const cclr_c128 *xi2, int nrhs, const double *omegas,
+                          int nomega, double gamma, double tol, int maxiter, cclr_c128 *t1_out, cclr_c128 *t2_out,
+                          cclr_solve_info *info) {
+  return solve_impl(ctx, xi1, xi2, nrhs, omegas, nomega, gamma, tol, maxiter, t1_out, t2_out, info, false);
+}
+
+// l (A - z) = -eta: the same subspace method on the left transform (the reduced matrix is b^H A^T b)
+extern "C" int cclr_solve_left(cclr_ctx *ctx, const cclr_c128 *eta1, const cclr_c128 *eta2, int nrhs, const double *omegas,
+                               int nomega, double gamma, double tol, int maxiter, cclr_c128 *l1_out, cclr_c128 *l2_out,
+                               cclr_solve_info *info) {
+  return solve_impl(ctx, eta1, eta2, nrhs, omegas, nomega, gamma, tol, maxiter, l1_out, l2_out, info, true);
+}
+
+// lambda A = -eta0, eta0 = (F_me[i,a], <ij||ab>)  (Eq. 13)
+extern "C" int cclr_lambda(cclr_ctx *ctx, double tol, int maxiter, cclr_c128 *lam1, cclr_c128 *lam2, cclr_solve_info *info) {
+  if (!ctx || !lam1 || !lam2) return CCLR_EINVAL;
+  const int i1 = ctx->plan->find("FmeT"), i2 = ctx->plan->find("eta02");
+  if (i1 < 0 || i2 < 0 || !ctx->plan->buf(i1).ptr || !ctx->plan->buf(i2).ptr) return CCLR_EINVAL;
+  const double zero = 0.0;
+  return solve_impl(ctx, (const cclr_c128 *)ctx->plan->buf(i1).ptr, (const cclr_c128 *)ctx->plan->buf(i2).ptr, 1, &zero, 1, 0.0,
+                    tol, maxiter, lam1, lam2, info, true);
 }
 
 // Host-only entry point used by the CPU tests of the reduced-space algebra: beta_k = (G - z_k)^{-1} rhs for nz shifts.

@@ -30,6 +30,7 @@ struct Space {
   DeviceBuf Bm, Sm, coef;
   std::vector<cplx> G;        // maxdim x maxdim, row-major: G[i][j] = b_i^H sigma_j
   int sigma_calls = 0;
+  bool left = false;          // sigma_j = A^T b_j (left transform) instead of A b_j
 
   c128 *b(int j) { return Bm.p + (size_t)j * n; }
   c128 *s(int j) { return Sm.p + (size_t)j * n; }
@@ -78,7 +79,7 @@ struct Space {
   // sigma_j = A b_j for j in [L0, L) and the new rows / columns of G
   void extend_sigma(int L0) {
     for (int j = L0; j < L; ++j) {
-      cclr_sigma_one(ctx, b(j), b(j) + n1, make_double2(0.0, 0.0), s(j), s(j) + n1, false);
+      cclr_sigma_one(ctx, b(j), b(j) + n1, make_double2(0.0, 0.0), s(j), s(j) + n1, false, left);
       ++sigma_calls;
     }
     const int nn = L - L0;

@@ -84,6 +84,7 @@ struct ZgemmArgs {
   // wave-quantisation loss of the last partial wave (and is the split-K path of tall-K / tiny-MN contractions when
   // main_tiles == 0).
   int tiles_m, tiles_n;
+  int m_fastest;       // raster order: consecutive CTAs walk tile_m (they share one B column panel) instead of tile_n
   int main_tiles, tail_splits, chunks_per_split;
   c128 *partial;
 };
@@ -116,7 +117,9 @@ zgemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CU
   }
   const int tiles_mn = p.tiles_m * p.tiles_n;
   const int batch = tile / tiles_mn;
-  const int tile_m = (tile - batch * tiles_mn) / p.tiles_n, tile_n = (tile - batch * tiles_mn) % p.tiles_n;
+  const int trem = tile - batch * tiles_mn;
+  const int tile_m = p.m_fastest ? trem % p.tiles_m : trem / p.tiles_n;
+  const int tile_n = p.m_fastest ? trem / p.tiles_m : trem % p.tiles_n;
   const int nchunks_total = (p.K + BK - 1) / BK;
   int chunk0 = 0, nchunks = nchunks_total;
   if (is_tail) {
@@ -348,7 +351,9 @@ __global__ void __launch_bounds__(256) zgemm_tail_reduce_kernel(const ZgemmArgs 
   const int t = p.main_tiles + (int)blockIdx.x;                 // tile id
   const int tiles_mn = p.tiles_m * p.tiles_n;
   const int batch = t / tiles_mn;
-  const int tile_m = (t - batch * tiles_mn) / p.tiles_n, tile_n = (t - batch * tiles_mn) % p.tiles_n;
+  const int trem = t - batch * tiles_mn;
+  const int tile_m = p.m_fastest ? trem % p.tiles_m : trem / p.tiles_n;
+  const int tile_n = p.m_fastest ? trem / p.tiles_m : trem % p.tiles_n;
   const c128 *part = p.partial + (size_t)blockIdx.x * p.tail_splits * (size_t)(BM * BN);
   const bool has_beta = p.beta.x != 0.0 || p.beta.y != 0.0;
   for (int e = threadIdx.x; e < BM * BN; e += blockDim.x) {
@@ -362,6 +367,45 @@ __global__ void __launch_bounds__(256) zgemm_tail_reduce_kernel(const ZgemmArgs 
     if (has_beta) out = cadd(out, cmul(p.beta, *dst));
     *dst = out;
   }
+}
+
+// y[n] = sum_{k in slab} opA(a[k]) * opB(B[k][n])  (row vector times a [K][N] matrix: the M = 1 adjoint contractions of the left
+// transform): one thread per column, coalesced 16-byte loads along n, K split over gridDim.y slabs whose partial rows go to
+// part[slab][N] (fixed order -> deterministic) and are combined by zgemv_t_reduce_kernel.
+__global__ void __launch_bounds__(128) zgemv_t_kernel(int N, int K, const c128 *__restrict__ a, int conjA,
+                                                      const c128 *__restrict__ B, long ldb, int conjB, int kslab,
+                                                      c128 *__restrict__ part) {
+  const int n = blockIdx.x * blockDim.x + threadIdx.x;
+  if (n >= N) return;
+  const int k0 = blockIdx.y * kslab;
+  int k1 = k0 + kslab;
+  if (k1 > K) k1 = K;
+  const double sa = conjA ? -1.0 : 1.0, sb = conjB ? -1.0 : 1.0;
+  double x0 = 0.0, y0 = 0.0, x1 = 0.0, y1 = 0.0;
+  int k = k0;
+  for (; k + 1 < k1; k += 2) {
+    c128 u = a[k], w = B[(size_t)k * ldb + n], u2 = a[k + 1], w2 = B[(size_t)(k + 1) * ldb + n];
+    u.y *= sa; w.y *= sb; u2.y *= sa; w2.y *= sb;
+    x0 = fma(u.x, w.x, x0); x0 = fma(-u.y, w.y, x0); y0 = fma(u.x, w.y, y0); y0 = fma(u.y, w.x, y0);
+    x1 = fma(u2.x, w2.x, x1); x1 = fma(-u2.y, w2.y, x1); y1 = fma(u2.x, w2.y, y1); y1 = fma(u2.y, w2.x, y1);
+  }
+  if (k < k1) {
+    c128 u = a[k], w = B[(size_t)k * ldb + n];
+    u.y *= sa; w.y *= sb;
+    x0 = fma(u.x, w.x, x0); x0 = fma(-u.y, w.y, x0); y0 = fma(u.x, w.y, y0); y0 = fma(u.y, w.x, y0);
+  }
+  part[(size_t)blockIdx.y * N + n] = make_double2(x0 + x1, y0 + y1);
+}
+
+__global__ void __launch_bounds__(256) zgemv_t_reduce_kernel(int N, int slabs, const c128 *__restrict__ part, c128 alpha,
+                                                             c128 beta, c128 *y) {
+  const int n = blockIdx.x * blockDim.x + threadIdx.x;
+  if (n >= N) return;
+  c128 s = czero();
+  for (int k = 0; k < slabs; ++k) s = cadd(s, part[(size_t)k * N + n]);
+  c128 out = cmul(alpha, s);
+  if (beta.x != 0.0 || beta.y != 0.0) out = cadd(out, cmul(beta, y[n]));
+  y[n] = out;
 }
 
 // y[m] = alpha * sum_k opA(A[m][k]) * opB(b[k]) + beta * y[m]: the N = 1 contractions (S3, S4, G3, G4, F_me) are
@@ -423,7 +467,7 @@ cudaError_t zgemm(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *
   const int sms = zgemm_num_sms();
   // 64-row tiles when they cut the padding of M by more than 10 % (M of a few hundred: 300 -> 320 instead of 384)
   const long pad128 = (M + 127L) / 128 * 128, pad64 = (M + 63L) / 64 * 64;
-  const int BM = (pad64 * 10 < pad128 * 9) ? 64 : 128;
+  const int BM = (pad64 * 10 <= pad128 * 9) ? 64 : 128;
   if (K <= 0) {  // C = beta * C
     zgemm_reduce_kernel<<<256, 256, 0, st>>>(nullptr, 0, M, N, alpha, beta, C, ldc, sc, batch);
     cclr_count_launch();
@@ -441,12 +485,30 @@ cudaError_t zgemm(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *
     cclr_count_launch();
     return cudaGetLastError();
   }
+  if (batch == 1 && M == 1 && b_is_kn && K >= 32 && ws && ws->buf && (size_t)N <= ws->elems) {
+    const int nblk = (N + 127) / 128;
+    int slabs = (4 * sms + nblk - 1) / nblk;
+    if (slabs > K / 16) slabs = K / 16;
+    if ((size_t)slabs * N > ws->elems) slabs = (int)(ws->elems / N);
+    if (slabs < 1) slabs = 1;
+    const int kslab = (K + slabs - 1) / slabs;
+    slabs = (K + kslab - 1) / kslab;
+    zgemv_t_kernel<<<dim3(nblk, slabs), 128, 0, st>>>(N, K, A, conjA, B, ldb, conjB, kslab, ws->buf);
+    zgemv_t_reduce_kernel<<<(N + 255) / 256, 256, 0, st>>>(N, slabs, ws->buf, alpha, beta, C);
+    cclr_count_launch(2);
+    return cudaGetLastError();
+  }
   // ---- N-tile width: the least padded N, widest tile on ties ----
+  // (the widest tile within 1 % of the least padding: narrower tiles re-read the A panels more often)
   int NG = 8;
   long best = -1;
   for (int ng = 8; ng >= 4; --ng) {
     const long bn = 8 * ng, padded = (N + bn - 1) / bn * bn;
-    if (best < 0 || padded < best) { best = padded; NG = ng; }
+    if (best < 0 || padded < best) best = padded;
+  }
+  for (int ng = 8; ng >= 4; --ng) {
+    const long bn = 8 * ng, padded = (N + bn - 1) / bn * bn;
+    if (padded * 100 <= best * 101) { NG = ng; break; }
   }
   const int BN = 8 * NG;
   ZgemmArgs args{};
@@ -456,6 +518,7 @@ cudaError_t zgemm(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *
   args.conjA = conjA; args.conjB = conjB;
   args.tiles_m = (M + BM - 1) / BM;
   args.tiles_n = (N + BN - 1) / BN;
+  args.m_fastest = N > M;   // the larger operand's panels are the ones shared through L2 by concurrently running CTAs
   const long tiles = (long)args.tiles_m * args.tiles_n * batch;
   if (tiles > 0x7fffffffL / 2) return cudaErrorInvalidValue;
   const int nchunks = (K + BK - 1) / BK;

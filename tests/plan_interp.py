@@ -337,3 +337,39 @@ def run_xi(it, X):
     it.bind("out2", "(ab)(ij)", np.zeros(npair(v) * npair(o), complex))
     it.run(load_plan("CCLR_PLAN_XI"))
     return it.get("out1").copy(), it.get("out2").copy()
+
+
+def run_sigma_left(it, l1, l2p, z):
+    """Execute CCLR_PLAN_SIGMA_LEFT (after run_sigma has declared the shared work buffers)."""
+    o, v = it.o, it.v
+    it.scalars["$nz"] = -complex(z)
+    it.bind("x1", "ai", l1)
+    it.bind("x2", "(ab)(ij)", l2p)
+    it.bind("out1", "ai", np.zeros(v * o, complex))
+    it.bind("out2", "(ab)(ij)", np.zeros(npair(v) * npair(o), complex))
+    it.run(load_plan("CCLR_PLAN_SIGMA_LEFT"))
+    return it.get("out1").copy(), it.get("out2").copy()
+
+
+def run_eta(it, X, l1, l2p, eom):
+    """Execute CCLR_PLAN_XI (into xiw1 / xiw2), CCLR_PLAN_ETA and optionally CCLR_PLAN_ETA_EOM for operator X and multipliers."""
+    o, v = it.o, it.v
+    it.bind("xoo", "mi", np.ascontiguousarray(X[:o, :o]).reshape(-1))
+    it.bind("xov", "me", np.ascontiguousarray(X[:o, o:]).reshape(-1))
+    it.bind("xvo", "ai", np.ascontiguousarray(X[o:, :o]).reshape(-1))
+    it.bind("xvv", "ae", np.ascontiguousarray(X[o:, o:]).reshape(-1))
+    it.bind("x1", "ai", l1)
+    it.bind("x2", "(ab)(ij)", l2p)
+    xi1, xi2 = np.zeros(v * o, complex), np.zeros(npair(v) * npair(o), complex)
+    if eom:
+        it.bind("out1", "ai", xi1)
+        it.bind("out2", "(ab)(ij)", xi2)
+        it.run(load_plan("CCLR_PLAN_XI"))
+        xi1 = it.get("out1").copy()
+    it.bind("out1", "ai", np.zeros(v * o, complex))
+    it.bind("out2", "(ab)(ij)", np.zeros(npair(v) * npair(o), complex))
+    it.run(load_plan("CCLR_PLAN_ETA"))
+    if eom:
+        it.get("xiw1")[...] = xi1.reshape(it.get("xiw1").shape)
+        it.run(load_plan("CCLR_PLAN_ETA_EOM"))
+    return it.get("out1").copy(), it.get("out2").copy()

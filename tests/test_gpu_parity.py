@@ -283,3 +283,29 @@ def test_config2_ground_state_sigma_and_damped_solve_against_full_oracle():
     res = packing.flat(q1, q2) + packing.flat(*xi)
     assert np.linalg.norm(res) <= 2e-10 * np.linalg.norm(packing.flat(*xi))
     ctx.close()
+
+
+@pytest.mark.parametrize("o,v,flags,nvec", [(3, 5, 0, 1), (4, 7, 2, 2), (4, 20, 0, 2), (6, 40, 0, 1)])
+def test_sigma_left_matches_oracle(o, v, flags, nvec):
+    """The left transform l (A - z) (cclr_sigma_left) against the oracle's adjoint of S-Eq. 11-12 (pinned by A^T of the dense
+    Jacobian), norm-wise 1e-10; and the duality <l, A x> = <l A, x> between the two GPU transforms."""
+    cc = _lib()
+    s = make_system(o, v, seed=o * 100 + v + 2)
+    ctx = gpu_context(s, flags)
+    c = cclr.CCLR(s["ints"], s["t1f"], s["t2f"])
+    l1, l2 = synth.amplitudes(o, v, seed=13, cls1="x1", cls2="x2", nvec=nvec)
+    for (w, g) in [(0.0, 0.0), (0.0773, 0.0045)]:
+        o1, o2 = cc.cclr_sigma_left(ctx, l1.cuda(), l2.cuda(), w, g)
+        torch.cuda.synchronize()
+        for k in range(nvec):
+            r1, r2 = c.sigma_left(*packing.unpack_amplitudes(l1[k].numpy(), l2[k].numpy(), o, v), z=w + 1j * g)
+            r1p, r2p = packing.pack_amplitudes(r1, r2)
+            assert rel(o1[k].cpu().numpy(), r1p.reshape(-1)) < 1e-10, ("left sigma1", k, w, g)
+            assert rel(o2[k].cpu().numpy(), r2p.reshape(-1)) < 1e-10, ("left sigma2", k, w, g)
+    x1, x2 = synth.amplitudes(o, v, seed=14, cls1="x1", cls2="x2")
+    s1, s2 = cc.cclr_sigma(ctx, x1.cuda(), x2.cuda())
+    q1, q2 = cc.cclr_sigma_left(ctx, l1[:1].contiguous().cuda(), l2[:1].contiguous().cuda())
+    lhs = (l1[0].cuda() * s1[0]).sum() + (l2[0].cuda() * s2[0]).sum()           # bilinear, unique elements
+    rhs = (q1[0] * x1[0].cuda()).sum() + (q2[0] * x2[0].cuda()).sum()
+    assert abs(complex(lhs - rhs)) <= 1e-11 * abs(complex(lhs))
+    ctx.close()

@@ -231,3 +231,26 @@ def test_residual_is_the_gauss_quadrature_of_the_jacobian_along_the_ray():
     assert np.abs(acc1 - w1).max() < 1e-13 and np.abs(acc2 - w2).max() < 1e-13
     e = cclr.dot(*cclr.CCLR(ints, 0.5 * t1, 0.5 * t2).eta0(), t1, t2)
     assert abs(e - ccsd.energy(ints, t1, t2)) < 1e-13
+
+
+@pytest.mark.parametrize("o,v", [(3, 4), (2, 5), (4, 4)])
+def test_sigma_left_is_the_transpose_of_the_pinned_jacobian(o, v):
+    """l A through sigma_left equals A^T l with A the dense Jacobian built from sigma() (pinned by the determinant space),
+    at random unconverged t, complex shift included."""
+    f, V = random_system(o, v, seed=31 + o, diag_fock=False)
+    ints = ccsd.Integrals.from_full(f, V, o)
+    t1, t2 = random_amplitudes(o, v, 32, scale=0.2)
+    c = cclr.CCLR(ints, t1, t2)
+    A = c.dense_jacobian()
+    l1, l2 = random_amplitudes(o, v, 33, scale=1.0)
+    z = 0.0773 + 0.0045j
+    got = flat(*c.sigma_left(l1, l2, z))
+    want = A.T @ flat(l1, l2) - z * flat(l1, l2)
+    assert np.abs(got - want).max() < 1e-12 * max(1.0, np.abs(want).max())
+
+
+def test_iterative_lambda_matches_dense_lambda(small_lr):
+    s = small_lr[(3, 4)]
+    c = s["c"]
+    w1, w2 = c.solve_lambda_iterative()
+    assert np.abs(flat(w1, w2) - flat(s["l1"], s["l2"])).max() < 1e-9

@@ -70,3 +70,32 @@ def test_xi_plan_reproduces_oracle_xi(o, v):
     r1, r2 = packing.pack_amplitudes(*c.xi(X))
     assert np.linalg.norm(s1.reshape(-1) - r1.reshape(-1)) <= 1e-12 * np.linalg.norm(r1)
     assert np.linalg.norm(s2.reshape(-1) - r2.reshape(-1)) <= 1e-12 * np.linalg.norm(r2)
+
+
+@pytest.mark.parametrize("o,v,chunk", [(3, 5, None), (4, 6, 2)])
+def test_left_sigma_plan_reproduces_oracle_left_sigma(o, v, chunk):
+    it, c = _setup(o, v, seed=80 + v, chunk_override=chunk)
+    x1, x2 = random_amplitudes(o, v, seed=81, scale=1.0)
+    plan_interp.run_sigma(it, *packing.pack_amplitudes(x1, x2), 0.0)          # declares the shared work buffers
+    for k, z in enumerate([0.0, 0.0773 + 0.0045j]):
+        l1, l2 = random_amplitudes(o, v, seed=82 + k, scale=1.0)
+        s1, s2 = plan_interp.run_sigma_left(it, *packing.pack_amplitudes(l1, l2), z)
+        r1, r2 = packing.pack_amplitudes(*c.sigma_left(l1, l2, z))
+        assert np.linalg.norm(s1.reshape(-1) - r1.reshape(-1)) <= 1e-12 * np.linalg.norm(r1)
+        assert np.linalg.norm(s2.reshape(-1) - r2.reshape(-1)) <= 1e-12 * np.linalg.norm(r2)
+
+
+@pytest.mark.parametrize("o,v,eom", [(3, 5, False), (4, 6, True)])
+def test_eta_plan_reproduces_oracle_eta(o, v, eom):
+    from conftest import random_hermitian
+    it, c = _setup(o, v, seed=90 + v)
+    x1, x2 = random_amplitudes(o, v, seed=91, scale=1.0)
+    plan_interp.run_sigma(it, *packing.pack_amplitudes(x1, x2), 0.0)          # declares the shared work buffers
+    l1, l2 = random_amplitudes(o, v, seed=92, scale=1.0)
+    plan_interp.run_xi(it, random_hermitian(o + v, 1))                         # (xi / left plans declare FX, HX, GLh, GOh ...)
+    plan_interp.run_sigma_left(it, *packing.pack_amplitudes(l1, l2), 0.0)
+    X = random_hermitian(o + v, 93) + 0.2j * np.random.default_rng(94).normal(size=(o + v, o + v))
+    s1, s2 = plan_interp.run_eta(it, X, *packing.pack_amplitudes(l1, l2), eom)
+    r1, r2 = packing.pack_amplitudes(*(c.eta_eom(X, l1, l2) if eom else c.eta(X, l1, l2)))
+    assert np.linalg.norm(s1.reshape(-1) - r1.reshape(-1)) <= 1e-12 * np.linalg.norm(r1)
+    assert np.linalg.norm(s2.reshape(-1) - r2.reshape(-1)) <= 1e-12 * np.linalg.norm(r2)
