@@ -99,6 +99,27 @@ int cclr_solve(cclr_ctx *ctx, const cclr_c128 *xi1, const cclr_c128 *xi2, int nr
  * blocks are used); xi1 [v*o], xi2 [vv*oo] device outputs. */
 int cclr_xi(cclr_ctx *ctx, const cclr_c128 *X, cclr_c128 *xi1, cclr_c128 *xi2);
 
+/* eta^X = <Lambda| [Xbar, tau_nu] |R> (S-Eq. 4-6) for the one-body operator X (device [n][n]) and the
+ * ground-state multipliers lam1 [v*o] (lambda^i_a at [a][i]), lam2 [vv*oo]; eom != 0 adds the EOM term of S-Eq. 7
+ * (PAPER.md:853), giving the EOM-eta vector of the CC-CI response function Eq. 16.  eta1, eta2: device outputs. */
+int cclr_eta(cclr_ctx *ctx, const cclr_c128 *X, const cclr_c128 *lam1, const cclr_c128 *lam2, int eom, cclr_c128 *eta1,
+             cclr_c128 *eta2);
+
+/* Left equations  l (A - z_k) = -eta_r  for every right-hand side and shift: the same shared-subspace method as cclr_solve on
+ * the left transform (arguments as cclr_solve).  cclr_lambda solves the ground-state multiplier equations
+ * lambda A = -eta0, eta0 = (F_me[i,a], <ij||ab>) (Eq. 13): lam1 [v*o], lam2 [vv*oo] device outputs. */
+int cclr_solve_left(cclr_ctx *ctx, const cclr_c128 *eta1, const cclr_c128 *eta2, int nrhs, const double *omegas, int nomega,
+                    double gamma, double tol, int maxiter, cclr_c128 *l1_out, cclr_c128 *l2_out, cclr_solve_info *info);
+int cclr_lambda(cclr_ctx *ctx, double tol, int maxiter, cclr_c128 *lam1, cclr_c128 *lam2, cclr_solve_info *info);
+
+/* <<X;Y>>_z, z = omega + i*gamma, in the CC-CI (EOM-CC) form of PAPER.md:142 Eq. 16 with the symmetriser of Eq. 17
+ * (readings 7-8 of DESIGN.md), computed end to end on the device: lambda (solved once per context and cached),
+ * xi^X, xi^Y, EOM-eta^X, EOM-eta^Y, the response amplitudes t^Y(z), t^Y(-conj z), t^X(-z), t^X(conj z), and the dot products.
+ * X, Y: device [n][n] one-body matrices; result: HOST, one complex number (alpha_XY = -<<X;Y>>, reading 9); info (host, may be
+ * NULL) accumulates the solver statistics.  Returns CCLR_OK, or CCLR_ENOTCONV if a solve missed tol (result still written). */
+int cclr_response_ci(cclr_ctx *ctx, const cclr_c128 *X, const cclr_c128 *Y, double omega, double gamma, double tol,
+                     int maxiter, cclr_c128 *result, cclr_solve_info *info);
+
 /* result[k] = sum_ai eta1 x1_k + sum_{a<b,i<j} eta2 x2_k  (bilinear, no conjugation; PAPER.md:137 Eq. 15, :203) for
  * nvec vectors x_k; result is a HOST array of nvec complex numbers. */
 int cclr_property(cclr_ctx *ctx, const cclr_c128 *eta1, const cclr_c128 *eta2, const cclr_c128 *x1,

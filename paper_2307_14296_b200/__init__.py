@@ -11,7 +11,7 @@ import torch
 from . import _lib
 from ._lib import CclrError, SolveInfo  # noqa: F401
 
-__all__ = ["Context", "cclr_create", "cclr_ccsd", "cclr_eom", "cclr_xi", "cclr_sigma", "cclr_solve", "cclr_property", "cclr_zgemm", "cclr_ladder",
+__all__ = ["Context", "cclr_create", "cclr_ccsd", "cclr_response_ci", "cclr_eom", "cclr_xi", "cclr_eta", "cclr_lambda", "cclr_solve_left", "cclr_sigma_left", "cclr_sigma", "cclr_solve", "cclr_property", "cclr_zgemm", "cclr_ladder",
            "cclr_ring", "cclr_fp64_tensor_peak", "cclr_hbm_copy_peak", "CclrError"]
 
 
@@ -208,6 +208,54 @@ def cclr_xi(ctx, X):
     xi2 = torch.empty(ctx.n2, dtype=torch.complex128, device="cuda")
     _lib.check(_lib.load().cclr_xi(ctx.handle, _dev(X, "X", n * n), _dev(xi1, "xi1"), _dev(xi2, "xi2")), "cclr_xi")
     return xi1, xi2
+
+
+def cclr_solve_left(ctx, eta1, eta2, omegas, gamma=0.0, tol=1e-10, maxiter=200):
+    """Solve l (A - (omega_k + i gamma)) = -eta_r.  Returns l1 [nrhs, nomega, v*o], l2 [nrhs, nomega, vv*oo], info."""
+    nrhs = eta1.numel() // ctx.n1
+    om = (C.c_double * len(omegas))(*[float(w) for w in omegas])
+    l1 = torch.empty((nrhs, len(omegas), ctx.n1), dtype=torch.complex128, device="cuda")
+    l2 = torch.empty((nrhs, len(omegas), ctx.n2), dtype=torch.complex128, device="cuda")
+    info = SolveInfo()
+    rc = _lib.load().cclr_solve_left(ctx.handle, _dev(eta1, "eta1", nrhs * ctx.n1), _dev(eta2, "eta2", nrhs * ctx.n2), nrhs,
+                                     om, len(omegas), float(gamma), float(tol), int(maxiter), _dev(l1, "l1"), _dev(l2, "l2"),
+                                     C.byref(info))
+    if rc not in (0, -4):
+        _lib.check(rc, "cclr_solve_left")
+    return l1, l2, info
+
+
+def cclr_lambda(ctx, tol=1e-10, maxiter=200):
+    """Ground-state multipliers: lambda A = -eta0.  Returns (lam1 [v*o], lam2 [vv*oo], info)."""
+    lam1 = torch.empty(ctx.n1, dtype=torch.complex128, device="cuda")
+    lam2 = torch.empty(ctx.n2, dtype=torch.complex128, device="cuda")
+    info = SolveInfo()
+    rc = _lib.load().cclr_lambda(ctx.handle, float(tol), int(maxiter), _dev(lam1, "lam1"), _dev(lam2, "lam2"), C.byref(info))
+    if rc not in (0, -4):
+        _lib.check(rc, "cclr_lambda")
+    return lam1, lam2, info
+
+
+def cclr_eta(ctx, X, lam1, lam2, eom=False):
+    """eta^X (eom=False, S-Eq. 5-6) or EOM-eta^X (eom=True, S-Eq. 7) for operator X [n, n] and multipliers lam1, lam2."""
+    n = ctx.o + ctx.v
+    e1 = torch.empty(ctx.n1, dtype=torch.complex128, device="cuda")
+    e2 = torch.empty(ctx.n2, dtype=torch.complex128, device="cuda")
+    _lib.check(_lib.load().cclr_eta(ctx.handle, _dev(X, "X", n * n), _dev(lam1, "lam1", ctx.n1), _dev(lam2, "lam2", ctx.n2),
+                                    int(bool(eom)), _dev(e1, "eta1"), _dev(e2, "eta2")), "cclr_eta")
+    return e1, e2
+
+
+def cclr_response_ci(ctx, X, Y, omega, gamma=0.0, tol=1e-10, maxiter=200):
+    """<<X;Y>>_{omega + i gamma} (CC-CI form, Eq. 16-17) computed end to end on the device; returns (complex, info)."""
+    n = ctx.o + ctx.v
+    res = _lib.Complex()
+    info = SolveInfo()
+    rc = _lib.load().cclr_response_ci(ctx.handle, _dev(X, "X", n * n), _dev(Y, "Y", n * n), float(omega), float(gamma),
+                                      float(tol), int(maxiter), C.byref(res), C.byref(info))
+    if rc not in (0, -4):
+        _lib.check(rc, "cclr_response_ci")
+    return complex(res.re, res.im), info
 
 
 def cclr_property(ctx, eta1, eta2, x1, x2):

@@ -42,6 +42,12 @@ SIGNATURES = {
     "cclr_sigma_left": (C.c_int, [C.c_void_p, c128_p, c128_p, C.c_int, C.c_double, C.c_double, c128_p, c128_p]),
     "cclr_solve": (C.c_int, [C.c_void_p, c128_p, c128_p, C.c_int, C.POINTER(C.c_double), C.c_int, C.c_double,
                              C.c_double, C.c_int, c128_p, c128_p, C.POINTER(SolveInfo)]),
+    "cclr_solve_left": (C.c_int, [C.c_void_p, c128_p, c128_p, C.c_int, C.POINTER(C.c_double), C.c_int, C.c_double,
+                                  C.c_double, C.c_int, c128_p, c128_p, C.POINTER(SolveInfo)]),
+    "cclr_lambda": (C.c_int, [C.c_void_p, C.c_double, C.c_int, c128_p, c128_p, C.POINTER(SolveInfo)]),
+    "cclr_eta": (C.c_int, [C.c_void_p, c128_p, c128_p, c128_p, C.c_int, c128_p, c128_p]),
+    "cclr_response_ci": (C.c_int, [C.c_void_p, c128_p, c128_p, C.c_double, C.c_double, C.c_double, C.c_int,
+                                   C.POINTER(Complex), C.POINTER(SolveInfo)]),
     "cclr_xi": (C.c_int, [C.c_void_p, c128_p, c128_p, c128_p]),
     "cclr_property": (C.c_int, [C.c_void_p, c128_p, c128_p, c128_p, c128_p, C.c_int, C.POINTER(Complex)]),
     "cclr_ccsd": (C.c_int, [C.c_int, C.c_int, c128_p, C.POINTER(EriPacked), c128_p, c128_p, C.c_double, C.c_int, C.c_void_p,

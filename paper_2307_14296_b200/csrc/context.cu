@@ -89,6 +89,7 @@ void destroy(cclr_ctx *ctx) {
   if (ctx->dot_out) cudaFree(ctx->dot_out);
   if (ctx->host_stage) cudaFree(ctx->host_stage);
   if (ctx->xblocks) cudaFree(ctx->xblocks);
+  if (ctx->lambda) cudaFree(ctx->lambda);
   for (cudaEvent_t ev : ctx->events) cudaEventDestroy(ev);
   delete ctx;
 }
@@ -216,6 +217,8 @@ extern "C" int cclr_create(int o, int v, const cclr_c128 *fock, const cclr_eri_p
     P.bind("xvv", "ae", ctx->xblocks + no * no + 2 * no * nv);
     P.compile(CCLR_PLAN_XI, ctx->xi_ops);
     P.compile(CCLR_PLAN_SIGMA_LEFT, ctx->left_ops);
+    P.compile(CCLR_PLAN_ETA, ctx->eta_ops);
+    P.compile(CCLR_PLAN_ETA_EOM, ctx->eta_eom_ops);
     cclr_ensure_dot_scratch(ctx, 256);
   } catch (const PlanError &e) {
     destroy(ctx);
@@ -329,22 +332,50 @@ extern "C" int cclr_ring(cclr_ctx *ctx, const cclr_c128 *x2, cclr_c128 *out2) {
   return CCLR_OK;
 }
 
+static void load_x_blocks(cclr_ctx *ctx, const cclr_c128 *X);
+
 extern "C" int cclr_xi(cclr_ctx *ctx, const cclr_c128 *X, cclr_c128 *xi1, cclr_c128 *xi2) {
   if (!ctx || !X || !xi1 || !xi2) {
     cclr_set_error("cclr_xi: null pointer", cudaSuccess);
     return CCLR_EINVAL;
   }
   try {
-    const size_t o = (size_t)ctx->o, v = (size_t)ctx->v, nf = o + v;
-    const c128 *F = (const c128 *)X;
-    struct { size_t off, r0, c0, rows, cols; } blocks[4] = {
-        {0, 0, 0, o, o}, {o * o, 0, o, o, v}, {o * o + o * v, o, 0, v, o}, {o * o + 2 * o * v, o, o, v, v}};
-    for (auto &b : blocks)
-      check(cudaMemcpy2DAsync(ctx->xblocks + b.off, b.cols * sizeof(c128), F + b.r0 * nf + b.c0, nf * sizeof(c128),
-                              b.cols * sizeof(c128), b.rows, cudaMemcpyDeviceToDevice, ctx->st),
-            "copy X block");
+    load_x_blocks(ctx, X);
     bind_vectors(ctx, nullptr, nullptr, (c128 *)xi1, (c128 *)xi2);
     run_ops(ctx, ctx->xi_ops, false);
+  } catch (const PlanError &e) {
+    return cclr_fail(e);
+  }
+  return CCLR_OK;
+}
+
+static void load_x_blocks(cclr_ctx *ctx, const cclr_c128 *X) {
+  const size_t o = (size_t)ctx->o, v = (size_t)ctx->v, nf = o + v;
+  const c128 *F = (const c128 *)X;
+  struct { size_t off, r0, c0, rows, cols; } blocks[4] = {
+      {0, 0, 0, o, o}, {o * o, 0, o, o, v}, {o * o + o * v, o, 0, v, o}, {o * o + 2 * o * v, o, o, v, v}};
+  for (auto &b : blocks)
+    check(cudaMemcpy2DAsync(ctx->xblocks + b.off, b.cols * sizeof(c128), F + b.r0 * nf + b.c0, nf * sizeof(c128),
+                            b.cols * sizeof(c128), b.rows, cudaMemcpyDeviceToDevice, ctx->st),
+          "copy X block");
+}
+
+extern "C" int cclr_eta(cclr_ctx *ctx, const cclr_c128 *X, const cclr_c128 *lam1, const cclr_c128 *lam2, int eom,
+                        cclr_c128 *eta1, cclr_c128 *eta2) {
+  if (!ctx || !X || !lam1 || !lam2 || !eta1 || !eta2 || lam1 == eta1 || lam2 == eta2) {
+    cclr_set_error("cclr_eta: null pointer or aliased output", cudaSuccess);
+    return CCLR_EINVAL;
+  }
+  try {
+    load_x_blocks(ctx, X);
+    if (eom) {   // xi^X into the work buffers xiw1 / xiw2 first (the EOM term contracts lambda2 with xi1)
+      c128 *w1 = ctx->plan->buf(ctx->plan->find("xiw1")).ptr, *w2 = ctx->plan->buf(ctx->plan->find("xiw2")).ptr;
+      bind_vectors(ctx, nullptr, nullptr, w1, w2);
+      run_ops(ctx, ctx->xi_ops, false);
+    }
+    bind_vectors(ctx, (const c128 *)lam1, (const c128 *)lam2, (c128 *)eta1, (c128 *)eta2);
+    run_ops(ctx, ctx->eta_ops, false);
+    if (eom) run_ops(ctx, ctx->eta_eom_ops, false);
   } catch (const PlanError &e) {
     return cclr_fail(e);
   }

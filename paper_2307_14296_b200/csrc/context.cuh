@@ -11,7 +11,7 @@ struct cclr_ctx {
   cudaStream_t st = nullptr;
   Plan *plan = nullptr;
   ZgemmWorkspace ws;
-  std::vector<ResolvedOp> sigma_ops, ladder_ops, ring_ops, xi_ops, left_ops, eta_ops;
+  std::vector<ResolvedOp> sigma_ops, ladder_ops, ring_ops, xi_ops, left_ops, eta_ops, eta_eom_ops;
   c128 *xblocks = nullptr;        // X_oo, X_ov, X_vo, X_vv of cclr_xi, contiguous
   int x1_id = -1, x2_id = -1, out1_id = -1, out2_id = -1;
   double *D = nullptr;            // orbital-energy denominators over unique elements, [n1 + n2]
@@ -26,6 +26,8 @@ struct cclr_ctx {
   // staging buffers of cclr_sigma_host
   c128 *host_stage = nullptr;
   size_t host_stage_elems = 0;
+  c128 *lambda = nullptr;         // ground-state multipliers [n1 + n2], solved on first use by cclr_response_ci
+  bool have_lambda = false;
   int max_subspace = 0;           // cclr_set_max_subspace (0 = automatic)
   size_t extra_bytes = 0;         // device bytes owned outside the plan
 };
