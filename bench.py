@@ -241,6 +241,18 @@ def run_ours(args):
     clocks = sampler.stop() if rank == 0 else None
     ctx.set_profiling(False)
 
+    # ---- the left transform l (A - z) (Lambda / left response equations; same flop count), 3 steps --------------------------
+    for _ in range(2):
+        cc.cclr_sigma_left(ctx, x1, x2, omega, gamma, out1, out2)
+    barrier()
+    l0, l1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0.record()
+    for _ in range(3):
+        cc.cclr_sigma_left(ctx, x1, x2, omega, gamma, out1, out2)
+    l1.record()
+    barrier()
+    left_ms = l0.elapsed_time(l1) / 3
+
     # ---- end to end: host buffers, copies inside the call ---------------------------------------------------
     hx1, hx2 = x1.cpu().pin_memory(), x2.cpu().pin_memory()
     ho1, ho2 = torch.empty_like(hx1).pin_memory(), torch.empty_like(hx2).pin_memory()
@@ -264,6 +276,7 @@ def run_ours(args):
         "e2e": {"value": flops_step * world * args.steps / (e2e_ms * 1e-3) / 1e12, "unit": UNIT,
                 "h2d_bytes_per_step": (n1 + n2) * nvec * 16, "d2h_bytes_per_step": (n1 + n2) * nvec * 16,
                 "ms_per_step": e2e_ms / args.steps},
+        "left_sigma": {"ms_per_step": left_ms, "tflops": flops_step / (left_ms * 1e-3) / 1e12},
         "gpu_launches": int(launches), "create_s": create_s, "create_launches": int(create_launches),
     }
     if rank == 0:
