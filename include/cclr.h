@@ -120,6 +120,23 @@ int cclr_lambda(cclr_ctx *ctx, double tol, int maxiter, cclr_c128 *lam1, cclr_c1
 int cclr_response_ci(cclr_ctx *ctx, const cclr_c128 *X, const cclr_c128 *Y, double omega, double gamma, double tol,
                      int maxiter, cclr_c128 *result, cclr_solve_info *info);
 
+/* x . F . y with the CC Hessian F of Table 1 (S-Eq. 8) for amplitude-shaped device vectors x, y and
+ * the ground-state multipliers: F is never formed; the contraction is the exact derivative
+ * d/da [(eta0 + lambda A)(t + a x) . y] at a = 0 (a cubic in a, 4-point stencil), i.e. four cclr_create + cclr_sigma_left
+ * evaluations at shifted amplitudes (reading 6: the printed t.F formulas are unrecoverable).  Needs the bare
+ * integrals and t (only read).  result: HOST. */
+int cclr_xfy(int o, int v, const cclr_c128 *fock, const cclr_eri_packed *eri, const cclr_c128 *t1, const cclr_c128 *t2,
+             const cclr_c128 *lam1, const cclr_c128 *lam2, const cclr_c128 *x1, const cclr_c128 *x2, const cclr_c128 *y1,
+             const cclr_c128 *y2, void *cuda_stream, cclr_c128 *result);
+
+/* <<X;Y>>_z in the symmetric CC-CC (LR-CC) form of PAPER.md:137 Eq. 15 with Eq. 17:
+ * g(w) = eta^X . t^Y(w) + eta^Y . t^X(-w) + t^X(-w) . F . t^Y(w),  <<X;Y>>_z = 1/2 [g(z) + conj g(-conj z)].  Same arguments as
+ * cclr_response_ci plus the inputs the context was created from (fock, eri, t1, t2: the F contraction rebuilds intermediates
+ * at shifted amplitudes, so the context must NOT have been created with CCLR_ERI_INPLACE over this eri->vvvv). */
+int cclr_response_cc(cclr_ctx *ctx, const cclr_c128 *fock, const cclr_eri_packed *eri, const cclr_c128 *t1, const cclr_c128 *t2,
+                     const cclr_c128 *X, const cclr_c128 *Y, double omega, double gamma, double tol, int maxiter,
+                     cclr_c128 *result, cclr_solve_info *info);
+
 /* result[k] = sum_ai eta1 x1_k + sum_{a<b,i<j} eta2 x2_k  (bilinear, no conjugation; PAPER.md:137 Eq. 15, :203) for
  * nvec vectors x_k; result is a HOST array of nvec complex numbers. */
 int cclr_property(cclr_ctx *ctx, const cclr_c128 *eta1, const cclr_c128 *eta2, const cclr_c128 *x1,

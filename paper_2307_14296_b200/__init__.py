@@ -11,7 +11,7 @@ import torch
 from . import _lib
 from ._lib import CclrError, SolveInfo  # noqa: F401
 
-__all__ = ["Context", "cclr_create", "cclr_ccsd", "cclr_response_ci", "cclr_eom", "cclr_xi", "cclr_eta", "cclr_lambda", "cclr_solve_left", "cclr_sigma_left", "cclr_sigma", "cclr_solve", "cclr_property", "cclr_zgemm", "cclr_ladder",
+__all__ = ["Context", "cclr_create", "cclr_ccsd", "cclr_response_ci", "cclr_response_cc", "cclr_xfy", "cclr_eom", "cclr_xi", "cclr_eta", "cclr_lambda", "cclr_solve_left", "cclr_sigma_left", "cclr_sigma", "cclr_solve", "cclr_property", "cclr_zgemm", "cclr_ladder",
            "cclr_ring", "cclr_fp64_tensor_peak", "cclr_hbm_copy_peak", "CclrError"]
 
 
@@ -255,6 +255,32 @@ def cclr_response_ci(ctx, X, Y, omega, gamma=0.0, tol=1e-10, maxiter=200):
                                       float(tol), int(maxiter), C.byref(res), C.byref(info))
     if rc not in (0, -4):
         _lib.check(rc, "cclr_response_ci")
+    return complex(res.re, res.im), info
+
+
+def cclr_xfy(o, v, fock, eri, t1, t2, lam1, lam2, x1, x2, y1, y2):
+    """x . F . y (CC Hessian contraction) as an exact derivative of the left transform; returns a complex."""
+    e = _eri_struct(o, v, eri)
+    res = _lib.Complex()
+    n1, n2 = o * v, (o * (o - 1) // 2) * (v * (v - 1) // 2)
+    rc = _lib.load().cclr_xfy(o, v, _dev(fock, "fock", (o + v) ** 2), C.byref(e), _dev(t1, "t1", n1), _dev(t2, "t2", n2),
+                              _dev(lam1, "lam1", n1), _dev(lam2, "lam2", n2), _dev(x1, "x1", n1), _dev(x2, "x2", n2),
+                              _dev(y1, "y1", n1), _dev(y2, "y2", n2), _stream(), C.byref(res))
+    _lib.check(rc, "cclr_xfy")
+    return complex(res.re, res.im)
+
+
+def cclr_response_cc(ctx, fock, eri, t1, t2, X, Y, omega, gamma=0.0, tol=1e-10, maxiter=200):
+    """<<X;Y>>_{omega + i gamma} in the symmetric CC-CC form (Eq. 15, 17) on the device; returns (complex, info)."""
+    n = ctx.o + ctx.v
+    e = _eri_struct(ctx.o, ctx.v, eri)
+    res = _lib.Complex()
+    info = SolveInfo()
+    rc = _lib.load().cclr_response_cc(ctx.handle, _dev(fock, "fock", n * n), C.byref(e), _dev(t1, "t1", ctx.n1),
+                                      _dev(t2, "t2", ctx.n2), _dev(X, "X", n * n), _dev(Y, "Y", n * n), float(omega),
+                                      float(gamma), float(tol), int(maxiter), C.byref(res), C.byref(info))
+    if rc not in (0, -4):
+        _lib.check(rc, "cclr_response_cc")
     return complex(res.re, res.im), info
 
 

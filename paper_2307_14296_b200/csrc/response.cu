@@ -12,12 +12,81 @@
 using subspace::check;
 using subspace::DeviceBuf;
 
-extern "C" int cclr_response_ci(cclr_ctx *ctx, const cclr_c128 *X, const cclr_c128 *Y, double omega, double gamma, double tol,
-                                int maxiter, cclr_c128 *result, cclr_solve_info *info) {
-  if (!ctx || !X || !Y || !result || !(tol > 0.0) || maxiter < 1) {
-    cclr_set_error("cclr_response_ci: null pointer, tol <= 0 or maxiter < 1", cudaSuccess);
+namespace {
+struct GroundState {   // what the F contraction of the CC-CC form needs besides the context
+  const cclr_c128 *fock;
+  const cclr_eri_packed *eri;
+  const cclr_c128 *t1, *t2;
+};
+}  // namespace
+
+// x . F . y = d/da [ (eta0 + lambda A)(t + a x) . y ] at a = 0  (F = CC Hessian of Table 1; S-Eq. 8, PAPER.md:855-857;
+// the printed contraction formulas PAPER.md:861-879 are unrecoverable, reading 6).  The bracket is a cubic polynomial
+// in a (A is cubic in t, eta0 linear), so the 4-point stencil [w(-2h) - 8 w(-h) + 8 w(h) - w(2h)] / 12h is exact; every w is one
+// cclr_create at shifted amplitudes plus one left transform of lambda: "F is never formed, only t.F".
+extern "C" int cclr_xfy(int o, int v, const cclr_c128 *fock, const cclr_eri_packed *eri, const cclr_c128 *t1, const cclr_c128 *t2,
+                        const cclr_c128 *lam1, const cclr_c128 *lam2, const cclr_c128 *x1, const cclr_c128 *x2,
+                        const cclr_c128 *y1, const cclr_c128 *y2, void *cuda_stream, cclr_c128 *result) {
+  if (o < 2 || v < 2 || !fock || !eri || !t1 || !t2 || !lam1 || !lam2 || !x1 || !x2 || !y1 || !y2 || !result) {
+    cclr_set_error("cclr_xfy: null pointer or o < 2 or v < 2", cudaSuccess);
     return CCLR_EINVAL;
   }
+  typedef std::complex<double> cplx;
+  try {
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const long n1 = (long)o * v, n2 = npair(o) * npair(v), n = n1 + n2;
+    DeviceBuf T, Xc, TS, W, coef, dpart, dout;
+    T.alloc(n, "cudaMalloc(t)"); Xc.alloc(n, "cudaMalloc(x)"); TS.alloc(n, "cudaMalloc(t + a x)"); W.alloc(n, "cudaMalloc(w)");
+    coef.alloc(1, "cudaMalloc(coef)"); dpart.alloc(dots_scratch_elems(2), "cudaMalloc(dot scratch)"); dout.alloc(2, "cudaMalloc(dot out)");
+    check(cudaMemcpyAsync(T.p, t1, (size_t)n1 * sizeof(c128), cudaMemcpyDeviceToDevice, st), "copy t1");
+    check(cudaMemcpyAsync(T.p + n1, t2, (size_t)n2 * sizeof(c128), cudaMemcpyDeviceToDevice, st), "copy t2");
+    check(cudaMemcpyAsync(Xc.p, x1, (size_t)n1 * sizeof(c128), cudaMemcpyDeviceToDevice, st), "copy x1");
+    check(cudaMemcpyAsync(Xc.p + n1, x2, (size_t)n2 * sizeof(c128), cudaMemcpyDeviceToDevice, st), "copy x2");
+    cplx nrm[2];
+    check(multi_dot(st, T.p, n, 1, T.p, n, 1, n, true, false, dpart.p, dout.p), "multi_dot");
+    check(multi_dot(st, Xc.p, n, 1, Xc.p, n, 1, n, true, false, dpart.p + dots_scratch_elems(1), dout.p + 1), "multi_dot");
+    check(cudaMemcpyAsync(nrm, dout.p, 2 * sizeof(c128), cudaMemcpyDeviceToHost, st), "D2H norms");
+    check(cudaStreamSynchronize(st), "sync");
+    const double nt = std::sqrt(std::max(0.0, nrm[0].real())), nx = std::sqrt(std::max(0.0, nrm[1].real()));
+    if (!(nx > 0.0)) { result->re = result->im = 0.0; return CCLR_OK; }
+    const double h = std::max(nt, 0.1) / nx;      // steps of the size of t itself balance round-off
+    const double cs[4] = {1.0, -8.0, 8.0, -1.0}, ss[4] = {-2.0, -1.0, 1.0, 2.0};
+    cplx acc = 0.0;
+    for (int k = 0; k < 4; ++k) {
+      const cplx step(ss[k] * h, 0.0);
+      check(cudaMemcpyAsync(coef.p, &step, sizeof(c128), cudaMemcpyHostToDevice, st), "H2D step");
+      check(cudaMemcpyAsync(TS.p, T.p, (size_t)n * sizeof(c128), cudaMemcpyDeviceToDevice, st), "copy t");
+      check(lincomb(st, TS.p, make_double2(1.0, 0.0), coef.p, Xc.p, n, 1, n), "t + a x");
+      check(cudaStreamSynchronize(st), "sync");
+      cclr_ctx *ck = nullptr;
+      int rc = cclr_create(o, v, fock, eri, (const cclr_c128 *)TS.p, (const cclr_c128 *)(TS.p + n1), 0, cuda_stream, &ck);
+      if (rc != CCLR_OK) return rc;
+      cclr_c128 a, b;
+      rc = cclr_sigma_left(ck, lam1, lam2, 1, 0.0, 0.0, (cclr_c128 *)W.p, (cclr_c128 *)(W.p + n1));
+      if (rc == CCLR_OK) rc = cclr_property(ck, (const cclr_c128 *)W.p, (const cclr_c128 *)(W.p + n1), y1, y2, 1, &a);
+      if (rc == CCLR_OK)
+        rc = cclr_property(ck, (const cclr_c128 *)ck->plan->buf(ck->plan->find("FmeT")).ptr,
+                           (const cclr_c128 *)ck->plan->buf(ck->plan->find("eta02")).ptr, y1, y2, 1, &b);
+      cclr_destroy(ck);
+      if (rc != CCLR_OK) return rc;
+      acc += cs[k] * (cplx(a.re, a.im) + cplx(b.re, b.im));
+    }
+    acc /= 12.0 * h;
+    result->re = acc.real();
+    result->im = acc.imag();
+  } catch (const PlanError &e) {
+    return cclr_fail(e);
+  }
+  return CCLR_OK;
+}
+
+static int response_impl(cclr_ctx *ctx, const cclr_c128 *X, const cclr_c128 *Y, double omega, double gamma, double tol,
+                         int maxiter, cclr_c128 *result, cclr_solve_info *info, const GroundState *gs) {
+  if (!ctx || !X || !Y || !result || !(tol > 0.0) || maxiter < 1) {
+    cclr_set_error("cclr_response: null pointer, tol <= 0 or maxiter < 1", cudaSuccess);
+    return CCLR_EINVAL;
+  }
+  const int eom = gs ? 0 : 1;
   typedef std::complex<double> cplx;
   cclr_solve_info total{};
   total.converged = 1;
@@ -49,8 +118,8 @@ extern "C" int cclr_response_ci(cclr_ctx *ctx, const cclr_c128 *X, const cclr_c1
     auto p2 = [&](DeviceBuf &b) { return (cclr_c128 *)(b.p + n1); };
     if ((rc = cclr_xi(ctx, X, p1(xiX), p2(xiX))) != CCLR_OK) return rc;
     if ((rc = cclr_xi(ctx, Y, p1(xiY), p2(xiY))) != CCLR_OK) return rc;
-    if ((rc = cclr_eta(ctx, X, lam1, lam2, 1, p1(eX), p2(eX))) != CCLR_OK) return rc;
-    if ((rc = cclr_eta(ctx, Y, lam1, lam2, 1, p1(eY), p2(eY))) != CCLR_OK) return rc;
+    if ((rc = cclr_eta(ctx, X, lam1, lam2, eom, p1(eX), p2(eX))) != CCLR_OK) return rc;
+    if ((rc = cclr_eta(ctx, Y, lam1, lam2, eom, p1(eY), p2(eY))) != CCLR_OK) return rc;
     // response amplitudes: t^Y at {z, -conj z} = ({omega, -omega}, +gamma); t^X at {-z, conj z} = ({-omega, omega}, -gamma);
     // outputs are [shift][n1] and [shift][n2]
     cclr_c128 *tY1 = (cclr_c128 *)tY.p, *tY2 = (cclr_c128 *)(tY.p + 2 * n1);
@@ -66,13 +135,24 @@ extern "C" int cclr_response_ci(cclr_ctx *ctx, const cclr_c128 *X, const cclr_c1
     cclr_c128 a[2], b[2], c[2], d[2], e, f;
     if ((rc = cclr_property(ctx, p1(eX), p2(eX), tY1, tY2, 2, a)) != CCLR_OK) return rc;
     if ((rc = cclr_property(ctx, p1(eY), p2(eY), tX1, tX2, 2, b)) != CCLR_OK) return rc;
-    if ((rc = cclr_property(ctx, lam1, lam2, tX1, tX2, 2, c)) != CCLR_OK) return rc;
-    if ((rc = cclr_property(ctx, lam1, lam2, tY1, tY2, 2, d)) != CCLR_OK) return rc;
-    if ((rc = cclr_property(ctx, lam1, lam2, p1(xiY), p2(xiY), 1, &e)) != CCLR_OK) return rc;
-    if ((rc = cclr_property(ctx, lam1, lam2, p1(xiX), p2(xiX), 1, &f)) != CCLR_OK) return rc;
     auto C = [](const cclr_c128 &q) { return cplx(q.re, q.im); };
-    const cplx g0 = C(a[0]) - C(c[0]) * C(e) + C(b[0]) - C(d[0]) * C(f);
-    const cplx g1 = C(a[1]) - C(c[1]) * C(e) + C(b[1]) - C(d[1]) * C(f);
+    cplx g0, g1;
+    if (!gs) {   // CC-CI, Eq. 16
+      if ((rc = cclr_property(ctx, lam1, lam2, tX1, tX2, 2, c)) != CCLR_OK) return rc;
+      if ((rc = cclr_property(ctx, lam1, lam2, tY1, tY2, 2, d)) != CCLR_OK) return rc;
+      if ((rc = cclr_property(ctx, lam1, lam2, p1(xiY), p2(xiY), 1, &e)) != CCLR_OK) return rc;
+      if ((rc = cclr_property(ctx, lam1, lam2, p1(xiX), p2(xiX), 1, &f)) != CCLR_OK) return rc;
+      g0 = C(a[0]) - C(c[0]) * C(e) + C(b[0]) - C(d[0]) * C(f);
+      g1 = C(a[1]) - C(c[1]) * C(e) + C(b[1]) - C(d[1]) * C(f);
+    } else {     // CC-CC, Eq. 15: g(w) = eta^X . t^Y(w) + eta^Y . t^X(-w) + t^X(-w) . F . t^Y(w)
+      for (int k = 0; k < 2; ++k) {
+        rc = cclr_xfy(ctx->o, ctx->v, gs->fock, gs->eri, gs->t1, gs->t2, lam1, lam2, tX1 + (size_t)k * n1, tX2 + (size_t)k * n2,
+                      tY1 + (size_t)k * n1, tY2 + (size_t)k * n2, (void *)ctx->st, &c[k]);
+        if (rc != CCLR_OK) return rc;
+      }
+      g0 = C(a[0]) + C(b[0]) + C(c[0]);
+      g1 = C(a[1]) + C(b[1]) + C(c[1]);
+    }
     const cplx r = 0.5 * (g0 + std::conj(g1));
     result->re = r.real();
     result->im = r.imag();
@@ -81,4 +161,20 @@ extern "C" int cclr_response_ci(cclr_ctx *ctx, const cclr_c128 *X, const cclr_c1
   }
   if (info) *info = total;
   return total.converged ? CCLR_OK : CCLR_ENOTCONV;
+}
+
+extern "C" int cclr_response_ci(cclr_ctx *ctx, const cclr_c128 *X, const cclr_c128 *Y, double omega, double gamma, double tol,
+                                int maxiter, cclr_c128 *result, cclr_solve_info *info) {
+  return response_impl(ctx, X, Y, omega, gamma, tol, maxiter, result, info, nullptr);
+}
+
+extern "C" int cclr_response_cc(cclr_ctx *ctx, const cclr_c128 *fock, const cclr_eri_packed *eri, const cclr_c128 *t1,
+                                const cclr_c128 *t2, const cclr_c128 *X, const cclr_c128 *Y, double omega, double gamma,
+                                double tol, int maxiter, cclr_c128 *result, cclr_solve_info *info) {
+  if (!fock || !eri || !t1 || !t2) {
+    cclr_set_error("cclr_response_cc: null pointer", cudaSuccess);
+    return CCLR_EINVAL;
+  }
+  const GroundState gs{fock, eri, t1, t2};
+  return response_impl(ctx, X, Y, omega, gamma, tol, maxiter, result, info, &gs);
 }

@@ -31,7 +31,9 @@ def cfg1():
                          torch.from_numpy(t2p).cuda())
     ops = [synth.hermitian_operator(o + v, 0, comp) for comp in range(3)]
     ops.append(synth.hermitian_operator(o + v, 0, 3, imaginary_antisymmetric=True))
-    yield dict(cc=cc, o=o, v=v, c=c, A=A, lam=(l1, l2), ctx=ctx, ops=ops)
+    dev = dict(f=f.cuda(), eri={k: x.cuda() for k, x in eri.items()}, t1=torch.from_numpy(t1p.reshape(-1).copy()).cuda(),
+               t2=torch.from_numpy(t2p.reshape(-1).copy()).cuda())
+    yield dict(cc=cc, o=o, v=v, c=c, A=A, lam=(l1, l2), ctx=ctx, ops=ops, dev=dev)
     ctx.close()
 
 
@@ -102,3 +104,31 @@ def test_two_level_closed_form_from_integrals_only():
         assert rinfo.converged == 1
         assert abs(got - want) <= 1e-8 * abs(want), (z, got, want)
     ctx.close()
+
+
+def test_hessian_contraction_matches_oracle(cfg1):
+    """x . F . y (cclr_xfy: exact derivative of the left transform along x) against the oracle's Richardson second derivative
+    of the Lagrangian (pinned by the explicit determinant-space F)."""
+    s = cfg1
+    d = s["dev"]
+    l1p, l2p = packing.pack_amplitudes(*s["lam"])
+    x1, x2 = synth.amplitudes(s["o"], s["v"], seed=21, cls1="x1", cls2="x2", nvec=2)
+    got = s["cc"].cclr_xfy(s["o"], s["v"], d["f"], d["eri"], d["t1"], d["t2"], _dev(l1p), _dev(l2p), x1[0].cuda(), x2[0].cuda(),
+                           x1[1].cuda(), x2[1].cuda())
+    ux = packing.unpack_amplitudes(x1[0].numpy(), x2[0].numpy(), s["o"], s["v"])
+    uy = packing.unpack_amplitudes(x1[1].numpy(), x2[1].numpy(), s["o"], s["v"])
+    want = s["c"].xFy(*s["lam"], *ux, *uy)
+    assert abs(got - want) <= 1e-9 * abs(want), (got, want)
+
+
+@pytest.mark.parametrize("z", [0.0, 0.0773 + 0.0045j])
+def test_cc_cc_response_function_end_to_end(cfg1, z):
+    s = cfg1
+    c, A, (l1, l2), ops, d = s["c"], s["A"], s["lam"], s["ops"], s["dev"]
+    dense = lambda a, b, zz: c.solve_dense(A, a, b, zz)
+    for (P, Q) in [(ops[0], ops[1]), (ops[2], ops[3])]:
+        want = c.response_cc_cc(dense, P, Q, z, l1, l2)
+        got, info = s["cc"].cclr_response_cc(s["ctx"], d["f"], d["eri"], d["t1"], d["t2"], _dev(P), _dev(Q), complex(z).real,
+                                             complex(z).imag, tol=1e-11)
+        assert info.converged == 1
+        assert abs(got - want) <= 1e-8 * abs(want), (z, got, want)
