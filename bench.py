@@ -304,6 +304,30 @@ def run_ours(args):
         line["fp64_pipe_probe_tflops"] = {"dmma": peak, "dfma": cc.cclr_fp64_pipe_probe(1), "dmma+dfma by warp": cc.cclr_fp64_pipe_probe(2)}
         line["hbm_copy_gbs_measured"] = cc.cclr_hbm_copy_peak(4 << 30)
         line["clocks"] = clocks
+    # ---- bandwidth kernels against the HBM roofline: the property dot (row D) and the layout kernels of the last sigma step --
+    reps = 20
+    cc.cclr_property(ctx, x1[0].contiguous(), x2[0].contiguous(), out1[:1].contiguous(), out2[:1].contiguous())
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(reps):
+        cc.cclr_property(ctx, x1[0], x2[0], out1[:1], out2[:1])       # synchronises: returns host data
+    dot_s = (time.perf_counter() - t0) / reps
+    if rank == 0:
+        hbm = line["hbm_copy_gbs_measured"]
+        oo, vv = npair(o), npair(v)
+        layout_bytes = {   # algorithmic bytes: every source element read once, every destination element written once
+            "perm Ur[ea(ij)]": 16 * (n2 + v * v * oo), "perm Xt[im(ef)]": 16 * (n2 + o * o * vv),
+            "perm R[aiem]": 16 * (n2 + (o * v) ** 2), "perm Xo[(ab)in]": 16 * (n2 + vv * o * o),
+            "perm out2[(ab)(ij)]": 16 * (3 * n2 + v * v * oo + vv * o * o + (o * v) ** 2),
+        }
+        bw = {"property_dot": {"bytes": 32 * (n1 + n2), "ms": dot_s * 1e3, "gbs": 32 * (n1 + n2) / dot_s / 1e9,
+                               "frac_of_copy_peak": 32 * (n1 + n2) / dot_s / 1e9 / hbm}}
+        for text, msv in ops_last:
+            for key, nbytes in layout_bytes.items():
+                if text.startswith(key) and msv > 0:
+                    per = msv / nvec
+                    bw[key] = {"bytes": nbytes, "ms": per, "gbs": nbytes / per / 1e6, "frac_of_copy_peak": nbytes / per / 1e6 / hbm}
+        line["bandwidth_kernels"] = bw
     # ---- time per solve (rows C, D): 3 right-hand sides x the config's frequencies in one call -----------------
     if not args.no_solve:
         xi1, xi2 = synth.amplitudes(o, v, seed=200 + rank, cls1="x1", cls2="x2", device="cuda", nvec=3)

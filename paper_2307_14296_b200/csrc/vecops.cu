@@ -31,13 +31,29 @@ __global__ void __launch_bounds__(DOT_THREADS) dot_partial_kernel(const c128 *__
   if (i1 > n) i1 = n;
   double sx = 0.0, sy = 0.0;
   const double sgn = conjA ? -1.0 : 1.0;
-  for (long i = i0 + threadIdx.x; i < i1; i += DOT_THREADS) {
+  // four independent 16-byte loads per operand in flight per thread (memory-level parallelism), fixed summation order
+  double tx[4] = {0.0, 0.0, 0.0, 0.0}, ty[4] = {0.0, 0.0, 0.0, 0.0};
+  long i = i0 + threadIdx.x;
+  for (; i + 3 * DOT_THREADS < i1; i += 4 * DOT_THREADS) {
+    c128 x[4], y[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) { x[u] = a[i + u * DOT_THREADS]; y[u] = b[i + u * DOT_THREADS]; }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      x[u].y *= sgn;
+      tx[u] = fma(x[u].x, y[u].x, tx[u]); tx[u] = fma(-x[u].y, y[u].y, tx[u]);
+      ty[u] = fma(x[u].x, y[u].y, ty[u]); ty[u] = fma(x[u].y, y[u].x, ty[u]);
+    }
+  }
+  for (; i < i1; i += DOT_THREADS) {
     c128 x = a[i];
     const c128 y = b[i];
     x.y *= sgn;
-    sx = fma(x.x, y.x, sx); sx = fma(-x.y, y.y, sx);
-    sy = fma(x.x, y.y, sy); sy = fma(x.y, y.x, sy);
+    tx[0] = fma(x.x, y.x, tx[0]); tx[0] = fma(-x.y, y.y, tx[0]);
+    ty[0] = fma(x.x, y.y, ty[0]); ty[0] = fma(x.y, y.x, ty[0]);
   }
+  sx = (tx[0] + tx[1]) + (tx[2] + tx[3]);
+  sy = (ty[0] + ty[1]) + (ty[2] + ty[3]);
   __shared__ c128 red[DOT_THREADS / 32];
   c128 w = warp_sum(make_double2(sx, sy));
   if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = w;
