@@ -245,7 +245,7 @@ def test_gpu_linearity_and_shift_identity():
     ctx.close()
 
 
-def test_config2_ground_state_sigma_and_damped_solve_against_full_oracle():
+def test_config2_ground_state_sigma_solve_and_response_function_against_full_oracle():
     """BASELINE.json configs[1] (o=10, v=80, damped gamma=0.0045) at full size, everything against the full-tensor oracle:
     the GPU ground state (cclr_ccsd, 1e-10) is certified by ONE oracle residual evaluation, sigma matches norm-wise to 1e-10,
     and the damped response amplitudes of a dipole perturbation satisfy the oracle's (A - z) t + xi = 0 to 2e-10."""
@@ -282,6 +282,30 @@ def test_config2_ground_state_sigma_and_damped_solve_against_full_oracle():
     q1, q2 = c.sigma(g1, g2, z=z)
     res = packing.flat(q1, q2) + packing.flat(*xi)
     assert np.linalg.norm(res) <= 2e-10 * np.linalg.norm(packing.flat(*xi))
+    # the complete CC-CI response function <<X;X>>_z at this size: the device value (cclr_response_ci: lambda, xi, EOM-eta,
+    # four response solves, dots) against the oracle's own assembly of Eq. 16-17 from amplitudes it has CERTIFIED -- lambda and
+    # every t(z) come from the GPU, and the oracle checks each against its own residual before using it.
+    X = synth.hermitian_operator(o + v, 0, 0)
+    got, rinfo = cc.cclr_response_ci(ctx, torch.from_numpy(X).cuda(), torch.from_numpy(X).cuda(), z.real, z.imag, tol=1e-10)
+    assert rinfo.converged == 1
+    lg1, lg2, linfo = cc.cclr_lambda(ctx, tol=1e-10)
+    assert linfo.converged == 1
+    lam = packing.unpack_amplitudes(lg1.cpu().numpy(), lg2.cpu().numpy(), o, v)
+    e0 = packing.flat(*c.eta0())
+    assert np.linalg.norm(packing.flat(*c.sigma_left(*lam)) + e0) <= 2e-10 * np.linalg.norm(e0)      # lambda A + eta0 = 0
+
+    def certified_gpu_solve(x1f, x2f, zz):
+        pa, pb = packing.pack_amplitudes(x1f, x2f)
+        u1, u2, uinfo = cc.cclr_solve(ctx, torch.from_numpy(pa.reshape(1, -1)).cuda(), torch.from_numpy(pb.reshape(1, -1)).cuda(),
+                                      [complex(zz).real], complex(zz).imag, tol=1e-10, maxiter=100)
+        assert uinfo.converged == 1
+        h1, h2 = packing.unpack_amplitudes(u1[0, 0].cpu().numpy(), u2[0, 0].cpu().numpy(), o, v)
+        rr = packing.flat(*c.sigma(h1, h2, z=zz)) + packing.flat(x1f, x2f)
+        assert np.linalg.norm(rr) <= 2e-10 * np.linalg.norm(packing.flat(x1f, x2f))
+        return h1, h2
+
+    want = c.response_cc_ci(certified_gpu_solve, X, X, z, *lam)
+    assert abs(got - want) <= 1e-8 * abs(want), (got, want)
     ctx.close()
 
 
