@@ -145,15 +145,15 @@ int cclr_property(cclr_ctx *ctx, const cclr_c128 *eta1, const cclr_c128 *eta2, c
 typedef struct {
   int iterations;        /* residual evaluations that were followed by an amplitude update          */
   int converged;         /* 1 if ||Omega|| <= tol                                                    */
-  int sigma_calls;       /* cclr_create + cclr_sigma pairs spent (two per residual)                  */
+  int sigma_calls;       /* residual evaluations performed                                           */
   double residual;       /* final ||Omega||_2 over the FULL tensors (= sqrt(|O1|^2 + 4 |O2 unique|^2)) */
   double energy_re, energy_im; /* CCSD correlation energy  sum f[i,a] t1[a,i] + 1/4 sum <ij||ab> tau[ab,ij]  */
   double seconds;
 } cclr_ccsd_info;
 
 /* Ground-state CCSD amplitudes (paper step 1): solves Omega(t) = 0 by quasi-Newton steps
- * t -= Omega / D with DIIS, where the residual is assembled from this library's own Jacobian transform through the exact
- * identity  Omega(t) = Omega(0) + 1/2 sum_k A(s_k t) . t,  s_k = 1/2 -+ 1/(2 sqrt 3).
+ * t -= Omega / D with DIIS on the direct residual plan (csrc/plans.inc CCLR_PLAN_OMEGA; the
+ * quadrature of the Jacobian, cclr_ccsd_residual mode 1, is the independent cross-check).
  * t1 [v][o], t2 [vv][oo] are IN/OUT device arrays: the start amplitudes on entry (zeros are fine), the solution on exit.
  * The integrals are only read.  Returns CCLR_OK, or CCLR_ENOTCONV (best iterate written, info filled). */
 int cclr_ccsd(int o, int v, const cclr_c128 *fock, const cclr_eri_packed *eri, cclr_c128 *t1, cclr_c128 *t2, double tol,
@@ -175,6 +175,12 @@ typedef struct {
  * Returns CCLR_OK or CCLR_ENOTCONV (best Ritz pairs written, info filled). */
 int cclr_eom(cclr_ctx *ctx, int nroots, double tol, int maxiter, cclr_c128 *eig, cclr_c128 *r1_out, cclr_c128 *r2_out,
              cclr_eom_info *info);
+
+/* The CCSD residual Omega(t) = <mu| exp(-T) H exp(T) |R> at arbitrary amplitudes, by either of the library's two independent
+ * routes: mode 0 = the direct residual plan cclr_ccsd iterates on, mode 1 = Omega(0) + 1/2 sum_k A(s_k t) . t through
+ * cclr_create + cclr_sigma at the two Gauss points (the cross-check; ~6 times more work).  om1 [v*o], om2 [vv*oo]: device. */
+int cclr_ccsd_residual(int o, int v, const cclr_c128 *fock, const cclr_eri_packed *eri, const cclr_c128 *t1, const cclr_c128 *t2,
+                       int mode, void *cuda_stream, cclr_c128 *om1, cclr_c128 *om2);
 
 /* Cap the trial-space dimension of cclr_solve (memory = 2 * dim * (v*o + vv*oo) * 16 bytes); 0 = sized from the free
  * device memory.  When the space is full it is collapsed onto the current solutions and the iteration continues. */

@@ -135,6 +135,18 @@ def cclr_ccsd(o, v, fock, eri, t1=None, t2=None, tol=1e-10, maxiter=100):
     return t1, t2, info
 
 
+def cclr_ccsd_residual(o, v, fock, eri, t1, t2, mode=0):
+    """Omega(t) on the device: mode 0 = direct residual plan, mode 1 = quadrature of the Jacobian.  Returns (om1, om2)."""
+    oo, vv, n = o * (o - 1) // 2, v * (v - 1) // 2, o + v
+    e = _eri_struct(o, v, eri)
+    om1 = torch.empty(o * v, dtype=torch.complex128, device="cuda")
+    om2 = torch.empty(vv * oo, dtype=torch.complex128, device="cuda")
+    rc = _lib.load().cclr_ccsd_residual(o, v, _dev(fock, "fock", n * n), C.byref(e), _dev(t1, "t1", o * v),
+                                        _dev(t2, "t2", vv * oo), int(mode), _stream(), _dev(om1, "om1"), _dev(om2, "om2"))
+    _lib.check(rc, "cclr_ccsd_residual")
+    return om1, om2
+
+
 def cclr_sigma(ctx, x1, x2, omega=0.0, gamma=0.0, out1=None, out2=None):
     """out = A x - (omega + i gamma) x.  x1: [nvec, v*o] (or [v*o]), x2: [nvec, vv*oo]."""
     nvec = x1.numel() // ctx.n1

@@ -58,6 +58,8 @@ SIGNATURES = {
                             C.POINTER(CcsdInfo)]),
     "cclr_eom": (C.c_int, [C.c_void_p, C.c_int, C.c_double, C.c_int, C.c_void_p, c128_p, c128_p, C.POINTER(EomInfo)]),
     "cclr_host_eigen": (C.c_int, [C.c_int, c128_p, c128_p, c128_p]),
+    "cclr_ccsd_residual": (C.c_int, [C.c_int, C.c_int, c128_p, C.POINTER(EriPacked), c128_p, c128_p, C.c_int, C.c_void_p,
+                                     c128_p, c128_p]),
     "cclr_set_max_subspace": (C.c_int, [C.c_void_p, C.c_int]),
     "cclr_destroy": (None, [C.c_void_p]),
     "cclr_strerror": (C.c_char_p, [C.c_int]),

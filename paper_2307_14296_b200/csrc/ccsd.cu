@@ -1,18 +1,18 @@
-// ccsd.cu — cclr_ccsd: the ground-state CCSD amplitudes (paper step 1) on the GPU, built ONLY from the
-// response machinery of this library.
+// ccsd.cu — cclr_ccsd: the ground-state CCSD amplitudes (paper step 1) on the GPU.
 //
-// The CCSD residual Omega(t) is a polynomial of degree <= 4 in t and the Jacobian of PAPER.md:131 Eq. 14 is its derivative,
-// A(t) = dOmega/dt, so along the ray s -> s*t
-//
-//     Omega(t) = Omega(0) + int_0^1 A(s t) . t ds = Omega(0) + 1/2 [ A(s_1 t) . t + A(s_2 t) . t ],   s_k = 1/2 -+ 1/(2 sqrt 3)
-//
-// exactly (2-point Gauss-Legendre integrates the cubic s -> A(s t) . t exactly), with Omega(0) = (f[a,i], <ab||ij>).  One residual
-// is therefore two cclr_create + cclr_sigma pairs at scaled amplitudes; no separate residual code exists.  The amplitude update is
-// the quasi-Newton step t -= Omega / D with DIIS extrapolation (the paper uses CROP; the fixed point is the same).
-// The energy uses the same idea: dE/dt . x = eta0(t) . x with eta0 linear in t, so E(t) = eta0(t/2) . t; here it is evaluated
-// directly as  sum_ia f[i,a] t1[a,i] + sum_{a<b,i<j} <ij||ab> tau[ab,ij]  (tau of S-Eq. 28).
+// Residual, two independent routes (cclr_ccsd_residual exposes both; cclr_ccsd iterates on the first):
+//   mode 0  the direct residual plan CCLR_PLAN_OMEGA (plans.inc): the textbook spin-orbital CCSD equations as ~60 GEMM / layout
+//           statements on the library's kernels, <ab||ef> only read (the vvvv term is applied factorised); about 4.3
+//           ladder-equivalents per evaluation;
+//   mode 1  the quadrature of the Jacobian: Omega is a quartic polynomial in t and A(t) = dOmega/dt, so
+//               Omega(t) = Omega(0) + int_0^1 A(s t) . t ds = Omega(0) + 1/2 [ A(s_1 t) . t + A(s_2 t) . t ],  s = 1/2 -+ 1/(2 sqrt 3)
+//           exactly (2-point Gauss-Legendre integrates the cubic s -> A(s t) . t), with Omega(0) = (f[a,i], <ab||ij>): two
+//           cclr_create + cclr_sigma pairs, no residual code of its own (about 25 ladder-equivalents) -- the cross-check.
+// Amplitude update: quasi-Newton step t -= Omega / D with DIIS (the paper uses CROP; the fixed point is the same).
+// Energy: sum_ia f[i,a] t1[a,i] + sum_{a<b,i<j} <ij||ab> tau[ab,ij]  (tau of S-Eq. 28).
 #include "context.cuh"
 #include "small_dense.h"
+#include "plans.inc"
 #include <chrono>
 #include <cmath>
 #include <complex>
@@ -47,12 +47,134 @@ perm tau[(ab)(ij)] = 1 t2[(ab)(ij)] 1 tt[aibj] -1 tt[biaj]
 free tt
 )PLAN";
 
+// Everything a residual evaluation needs: the plan object with the integral classes and Fock blocks bound, Omega(0), scratch.
+struct Engine {
+  int o, v;
+  long n1, n2, n;
+  cudaStream_t st;
+  void *stream_arg;
+  const cclr_c128 *fock;
+  const cclr_eri_packed *eri;
+  Plan P;
+  Buf fblocks, S, TS, coef;
+  const c128 *W0 = nullptr, *fovT = nullptr, *fvo = nullptr;
+  int t1_id = -1, t2_id = -1;
+  int sigma_calls = 0;
+
+  Engine(int o_, int v_, const cclr_c128 *fock_, const cclr_eri_packed *eri_, void *stream)
+      : o(o_), v(v_), n1((long)o_ * v_), n2(npair(o_) * npair(v_)), n(n1 + n2), st((cudaStream_t)stream), stream_arg(stream),
+        fock(fock_), eri(eri_), P(o_, v_, (cudaStream_t)stream) {
+    const size_t no = (size_t)o, nv = (size_t)v, nf = no + nv;
+    const c128 *F = (const c128 *)fock;
+    fblocks.alloc(no * no + 2 * no * nv + nv * nv, "cudaMalloc(fock blocks)");
+    coef.alloc(1, "cudaMalloc(coef)");
+    struct { const char *name, *spec; size_t off, r0, c0, rows, cols; } blocks[4] = {
+        {"foo", "mi", 0, 0, 0, no, no}, {"fov", "me", no * no, 0, no, no, nv},
+        {"fvo", "ai", no * no + no * nv, no, 0, nv, no}, {"fvv", "ae", no * no + 2 * no * nv, no, no, nv, nv}};
+    for (auto &b : blocks) {
+      check(cudaMemcpy2DAsync(fblocks.p + b.off, b.cols * sizeof(c128), F + b.r0 * nf + b.c0, nf * sizeof(c128),
+                              b.cols * sizeof(c128), b.rows, cudaMemcpyDeviceToDevice, st), "copy fock block");
+      P.bind(b.name, b.spec, fblocks.p + b.off);
+    }
+    fvo = fblocks.p + no * no + no * nv;
+    P.bind("oooo", "(mn)(ij)", (c128 *)eri->oooo);
+    P.bind("ooov", "(mn)ie", (c128 *)eri->ooov);
+    P.bind("oovv", "(mn)(ef)", (c128 *)eri->oovv);
+    P.bind("ovvo", "mbej", (c128 *)eri->ovvo);
+    P.bind("ovvv", "mb(ef)", (c128 *)eri->ovvv);
+    P.bind("vvvv", "(ab)(ef)", (c128 *)eri->vvvv);
+    P.bind("t1", "ai", nullptr);
+    P.bind("t2", "(ab)(ij)", nullptr);
+    t1_id = P.find("t1");
+    t2_id = P.find("t2");
+    P.execute(PLAN_OMEGA0);
+    W0 = P.buf(P.find("W0")).ptr;
+    fovT = P.buf(P.find("fovT")).ptr;
+  }
+
+  // mode 0: OM = Omega(T) by the direct residual plan
+  void direct(const c128 *T, c128 *OM) {
+    P.rebind(t1_id, const_cast<c128 *>(T));
+    P.rebind(t2_id, const_cast<c128 *>(T) + n1);
+    P.execute(CCLR_PLAN_OMEGA);
+    check(cudaMemcpyAsync(OM, P.buf(P.find("om1")).ptr, (size_t)n1 * sizeof(c128), cudaMemcpyDeviceToDevice, st), "copy Omega1");
+    check(cudaMemcpyAsync(OM + n1, P.buf(P.find("om2")).ptr, (size_t)n2 * sizeof(c128), cudaMemcpyDeviceToDevice, st), "copy Omega2");
+    check(cudaStreamSynchronize(st), "sync");
+    P.free_class(BUF_TEMP);
+  }
+
+  // mode 1: OM = Omega(0) + 1/2 sum_k A(s_k T) . T; returns a CCLR_* code
+  int quadrature(const c128 *T, c128 *OM) {
+    if (!S.p) { S.alloc(n, "cudaMalloc(sigma)"); TS.alloc(n, "cudaMalloc(scaled t)"); }
+    const double sq[2] = {0.5 - 0.5 / std::sqrt(3.0), 0.5 + 0.5 / std::sqrt(3.0)};
+    check(cudaMemcpyAsync(OM, fvo, (size_t)n1 * sizeof(c128), cudaMemcpyDeviceToDevice, st), "copy Omega1(0)");
+    check(cudaMemcpyAsync(OM + n1, W0, (size_t)n2 * sizeof(c128), cudaMemcpyDeviceToDevice, st), "copy Omega2(0)");
+    auto set_coef = [&](cplx c) {
+      check(cudaMemcpyAsync(coef.p, &c, sizeof(c128), cudaMemcpyHostToDevice, st), "H2D coef");
+      check(cudaStreamSynchronize(st), "sync coef");
+    };
+    for (int k = 0; k < 2; ++k) {
+      set_coef(cplx(sq[k], 0.0));
+      check(lincomb(st, TS.p, make_double2(0.0, 0.0), coef.p, T, n, 1, n), "scale t");
+      cclr_ctx *ctx = nullptr;
+      const int e = cclr_create(o, v, fock, eri, (const cclr_c128 *)TS.p, (const cclr_c128 *)(TS.p + n1), 0, stream_arg, &ctx);
+      if (e != CCLR_OK) return e;
+      try {
+        cclr_sigma_one(ctx, T, T + n1, make_double2(0.0, 0.0), S.p, S.p + n1, false);
+        ++sigma_calls;
+        set_coef(cplx(0.5, 0.0));
+        check(lincomb(st, OM, make_double2(1.0, 0.0), coef.p, S.p, n, 1, n), "accumulate Omega");
+        check(cudaStreamSynchronize(st), "sync");
+      } catch (...) {
+        cclr_destroy(ctx);
+        throw;
+      }
+      cclr_destroy(ctx);
+    }
+    return CCLR_OK;
+  }
+};
+
+bool valid_inputs(int o, int v, const cclr_c128 *fock, const cclr_eri_packed *eri, const void *t1, const void *t2) {
+  return o >= 2 && v >= 2 && fock && eri && t1 && t2 && eri->oooo && eri->ooov && eri->oovv && eri->ovvo && eri->ovvv && eri->vvvv;
+}
+
 }  // namespace
+
+extern "C" int cclr_ccsd_residual(int o, int v, const cclr_c128 *fock, const cclr_eri_packed *eri, const cclr_c128 *t1,
+                                  const cclr_c128 *t2, int mode, void *cuda_stream, cclr_c128 *om1, cclr_c128 *om2) {
+  if (!valid_inputs(o, v, fock, eri, t1, t2) || !om1 || !om2 || mode < 0 || mode > 1) {
+    cclr_set_error("cclr_ccsd_residual: null pointer, o < 2, v < 2 or unknown mode", cudaSuccess);
+    return CCLR_EINVAL;
+  }
+  try {
+    Engine E(o, v, fock, eri, cuda_stream);
+    Buf T, OM;
+    T.alloc(E.n, "cudaMalloc(t)");
+    OM.alloc(E.n, "cudaMalloc(omega)");
+    check(cudaMemcpyAsync(T.p, t1, (size_t)E.n1 * sizeof(c128), cudaMemcpyDeviceToDevice, E.st), "copy t1");
+    check(cudaMemcpyAsync(T.p + E.n1, t2, (size_t)E.n2 * sizeof(c128), cudaMemcpyDeviceToDevice, E.st), "copy t2");
+    if (mode == 0) {
+      E.direct(T.p, OM.p);
+    } else {
+      const int rc = E.quadrature(T.p, OM.p);
+      if (rc != CCLR_OK) return rc;
+    }
+    check(cudaMemcpyAsync(om1, OM.p, (size_t)E.n1 * sizeof(c128), cudaMemcpyDeviceToDevice, E.st), "copy Omega1 out");
+    check(cudaMemcpyAsync(om2, OM.p + E.n1, (size_t)E.n2 * sizeof(c128), cudaMemcpyDeviceToDevice, E.st), "copy Omega2 out");
+    check(cudaStreamSynchronize(E.st), "cclr_ccsd_residual sync");
+  } catch (const PlanError &e) {
+    return cclr_fail(e);
+  } catch (const std::exception &e) {
+    cclr_set_error(e.what(), cudaSuccess);
+    return CCLR_EINVAL;
+  }
+  return CCLR_OK;
+}
 
 extern "C" int cclr_ccsd(int o, int v, const cclr_c128 *fock, const cclr_eri_packed *eri, cclr_c128 *t1, cclr_c128 *t2,
                          double tol, int maxiter, void *cuda_stream, cclr_ccsd_info *info) {
-  if (o < 2 || v < 2 || !fock || !eri || !t1 || !t2 || !(tol > 0.0) || maxiter < 1 || !eri->oooo || !eri->ooov || !eri->oovv ||
-      !eri->ovvo || !eri->ovvv || !eri->vvvv) {
+  if (!valid_inputs(o, v, fock, eri, t1, t2) || !(tol > 0.0) || maxiter < 1) {
     cclr_set_error("cclr_ccsd: null pointer, o < 2, v < 2, tol <= 0 or maxiter < 1", cudaSuccess);
     return CCLR_EINVAL;
   }
@@ -60,40 +182,27 @@ extern "C" int cclr_ccsd(int o, int v, const cclr_c128 *fock, const cclr_eri_pac
   cclr_ccsd_info res{};
   int rc = CCLR_ENOTCONV;
   try {
-    cudaStream_t st = (cudaStream_t)cuda_stream;
-    const long oo = npair(o), vv = npair(v), n1 = (long)o * v, n2 = oo * vv, n = n1 + n2;
+    Engine E(o, v, fock, eri, cuda_stream);
+    cudaStream_t st = E.st;
+    const long n1 = E.n1, n2 = E.n2, n = E.n;
     const int ndiis = 8;
-    const size_t nf = (size_t)o + v;
-    const c128 *F = (const c128 *)fock;
-    Buf T, OM, S, TS, HT, HE, fov, om0_1, coef, dpart, dout;
-    T.alloc(n, "cudaMalloc(t)"); OM.alloc(n, "cudaMalloc(omega)"); S.alloc(n, "cudaMalloc(sigma)"); TS.alloc(n, "cudaMalloc(scaled t)");
+    Buf T, OM, HT, HE, coef, dpart, dout;
+    T.alloc(n, "cudaMalloc(t)"); OM.alloc(n, "cudaMalloc(omega)");
     HT.alloc((size_t)ndiis * n, "cudaMalloc(DIIS t)"); HE.alloc((size_t)ndiis * n, "cudaMalloc(DIIS e)");
-    fov.alloc(n1, "cudaMalloc(fov)"); om0_1.alloc(n1, "cudaMalloc(fvo)"); coef.alloc(ndiis + 1, "cudaMalloc(coef)");
+    coef.alloc(ndiis + 1, "cudaMalloc(coef)");
     const int npairs_max = ndiis * ndiis;
     dpart.alloc(dots_scratch_elems(npairs_max), "cudaMalloc(dot scratch)"); dout.alloc(npairs_max, "cudaMalloc(dot out)");
     double *D = nullptr;
     check(cudaMalloc(&D, (size_t)n * sizeof(double)), "cudaMalloc(D)");
     struct FreeD { double *p; ~FreeD() { cudaFree(p); } } freeD{D};
-    check(denominators(st, F, o, v, D), "denominators");
-    // Omega(0): f[a,i] and <ab||ij> = conj <ij||ab>;  f[i,a] transposed for the energy
-    check(cudaMemcpy2DAsync(om0_1.p, (size_t)o * sizeof(c128), F + (size_t)o * nf, nf * sizeof(c128), (size_t)o * sizeof(c128), v,
-                            cudaMemcpyDeviceToDevice, st), "copy f_vo");
-    check(cudaMemcpy2DAsync(fov.p, (size_t)v * sizeof(c128), F + o, nf * sizeof(c128), (size_t)v * sizeof(c128), o,
-                            cudaMemcpyDeviceToDevice, st), "copy f_ov");
-    Plan P(o, v, st);
-    P.bind("oovv", "(ij)(ab)", (c128 *)eri->oovv);
-    P.bind("fov", "ia", fov.p);
-    P.execute(PLAN_OMEGA0);
-    const c128 *W0 = P.buf(P.find("W0")).ptr, *fovT = P.buf(P.find("fovT")).ptr;
-
+    check(denominators(st, (const c128 *)fock, o, v, D), "denominators");
     check(cudaMemcpyAsync(T.p, t1, (size_t)n1 * sizeof(c128), cudaMemcpyDeviceToDevice, st), "copy t1");
     check(cudaMemcpyAsync(T.p + n1, t2, (size_t)n2 * sizeof(c128), cudaMemcpyDeviceToDevice, st), "copy t2");
 
-    auto host_dots = [&](const c128 *A, long lda, int na, const c128 *B, long ldb, int nb, long len, bool conjA, bool diag) {
-      const int np = diag ? na : na * nb;
-      std::vector<cplx> out(np);
-      check(multi_dot(st, A, lda, na, B, ldb, nb, len, conjA, diag, dpart.p, dout.p), "multi_dot");
-      check(cudaMemcpyAsync(out.data(), dout.p, (size_t)np * sizeof(c128), cudaMemcpyDeviceToHost, st), "D2H dots");
+    auto host_dots = [&](const c128 *A, long lda, int na, const c128 *B, long ldb, int nb, long len, bool conjA) {
+      std::vector<cplx> out((size_t)na * nb);
+      check(multi_dot(st, A, lda, na, B, ldb, nb, len, conjA, false, dpart.p, dout.p), "multi_dot");
+      check(cudaMemcpyAsync(out.data(), dout.p, out.size() * sizeof(c128), cudaMemcpyDeviceToHost, st), "D2H dots");
       check(cudaStreamSynchronize(st), "sync dots");
       return out;
     };
@@ -101,34 +210,14 @@ extern "C" int cclr_ccsd(int o, int v, const cclr_c128 *fock, const cclr_eri_pac
       check(cudaMemcpyAsync(coef.p, h.data(), h.size() * sizeof(c128), cudaMemcpyHostToDevice, st), "H2D coef");
       check(cudaStreamSynchronize(st), "sync coef");
     };
-    const double sq[2] = {0.5 - 0.5 / std::sqrt(3.0), 0.5 + 0.5 / std::sqrt(3.0)};
     int nhist = 0;
     for (int it = 0; it < maxiter; ++it) {
       res.iterations = it;
-      // ---- Omega(t) = Omega(0) + 1/2 sum_k A(s_k t) . t ----
-      check(cudaMemcpyAsync(OM.p, om0_1.p, (size_t)n1 * sizeof(c128), cudaMemcpyDeviceToDevice, st), "copy Omega1(0)");
-      check(cudaMemcpyAsync(OM.p + n1, W0, (size_t)n2 * sizeof(c128), cudaMemcpyDeviceToDevice, st), "copy Omega2(0)");
-      for (int k = 0; k < 2; ++k) {
-        set_coef({cplx(sq[k], 0.0)});
-        check(lincomb(st, TS.p, make_double2(0.0, 0.0), coef.p, T.p, n, 1, n), "scale t");
-        cclr_ctx *ctx = nullptr;
-        const int e = cclr_create(o, v, fock, eri, (const cclr_c128 *)TS.p, (const cclr_c128 *)(TS.p + n1), 0, cuda_stream, &ctx);
-        if (e != CCLR_OK) return e;
-        try {
-          cclr_sigma_one(ctx, T.p, T.p + n1, make_double2(0.0, 0.0), S.p, S.p + n1, false);
-          ++res.sigma_calls;
-          set_coef({cplx(0.5, 0.0)});
-          check(lincomb(st, OM.p, make_double2(1.0, 0.0), coef.p, S.p, n, 1, n), "accumulate Omega");
-          check(cudaStreamSynchronize(st), "sync");
-        } catch (...) {
-          cclr_destroy(ctx);
-          throw;
-        }
-        cclr_destroy(ctx);
-      }
+      E.direct(T.p, OM.p);
+      ++res.sigma_calls;     // (residual evaluations)
       // ---- convergence on the full-tensor 2-norm: ||Omega1||^2 + 4 ||Omega2 (unique)||^2 ----
-      const double d1 = host_dots(OM.p, n, 1, OM.p, n, 1, n1, true, false)[0].real();
-      const double d2 = host_dots(OM.p + n1, n, 1, OM.p + n1, n, 1, n2, true, false)[0].real();
+      const double d1 = host_dots(OM.p, n, 1, OM.p, n, 1, n1, true)[0].real();
+      const double d2 = host_dots(OM.p + n1, n, 1, OM.p + n1, n, 1, n2, true)[0].real();
       res.residual = std::sqrt(std::max(0.0, d1 + 4.0 * d2));
       if (!std::isfinite(res.residual) || res.residual > 1e6) break;
       if (res.residual <= tol) { res.converged = 1; rc = CCLR_OK; break; }
@@ -143,7 +232,7 @@ extern "C" int cclr_ccsd(int o, int v, const cclr_c128 *fock, const cclr_eri_pac
       nhist = std::min(nhist + 1, ndiis);
       if (nhist >= 2) {
         const int m = nhist;
-        std::vector<cplx> Bm = host_dots(HE.p, n, m, HE.p, n, m, n, true, false);
+        std::vector<cplx> Bm = host_dots(HE.p, n, m, HE.p, n, m, n, true);
         std::vector<cplx> M((size_t)(m + 1) * (m + 1), cplx(0.0)), rhs(m + 1, cplx(0.0)), c(m + 1, cplx(0.0));
         for (int p = 0; p < m; ++p) {
           for (int q = 0; q < m; ++q) M[(size_t)p * (m + 1) + q] = Bm[(size_t)p * m + q];
@@ -164,12 +253,12 @@ extern "C" int cclr_ccsd(int o, int v, const cclr_c128 *fock, const cclr_eri_pac
       }
     }
     // ---- energy and output ----
-    P.bind("t1", "ai", T.p);
-    P.bind("t2", "(ab)(ij)", T.p + n1);
-    P.execute(PLAN_TAU);
-    const c128 *tau = P.buf(P.find("tau")).ptr;
-    const cplx e1 = host_dots(fovT, n1, 1, T.p, n1, 1, n1, false, false)[0];
-    const cplx e2 = host_dots(W0, n2, 1, tau, n2, 1, n2, true, false)[0];     // conj(W0[(ab)(ij)]) = <ij||ab>
+    E.P.rebind(E.t1_id, T.p);
+    E.P.rebind(E.t2_id, T.p + n1);
+    E.P.execute(PLAN_TAU);
+    const c128 *tau = E.P.buf(E.P.find("tau")).ptr;
+    const cplx e1 = host_dots(E.fovT, n1, 1, T.p, n1, 1, n1, false)[0];
+    const cplx e2 = host_dots(E.W0, n2, 1, tau, n2, 1, n2, true)[0];     // conj(W0[(ab)(ij)]) = <ij||ab>
     res.energy_re = (e1 + e2).real();
     res.energy_im = (e1 + e2).imag();
     check(cudaMemcpyAsync(t1, T.p, (size_t)n1 * sizeof(c128), cudaMemcpyDeviceToDevice, st), "copy t1 out");

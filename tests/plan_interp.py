@@ -373,3 +373,19 @@ def run_eta(it, X, l1, l2p, eom):
         it.get("xiw1")[...] = xi1.reshape(it.get("xiw1").shape)
         it.run(load_plan("CCLR_PLAN_ETA_EOM"))
     return it.get("out1").copy(), it.get("out2").copy()
+
+
+def run_omega(o, v, fock, packed, t1, t2p, chunk_override=None):
+    """Execute CCLR_PLAN_OMEGA (the direct CCSD residual of cclr_ccsd) on numpy arrays; returns (om1, om2)."""
+    it = Interp(o, v, chunk_override)
+    for name, spec in (("oooo", "(mn)(ij)"), ("ooov", "(mn)ie"), ("oovv", "(mn)(ef)"), ("ovvo", "mbej"),
+                       ("ovvv", "mb(ef)"), ("vvvv", "(ab)(ef)")):
+        it.bind(name, spec, packed[name])
+    it.bind("t1", "ai", t1)
+    it.bind("t2", "(ab)(ij)", t2p)
+    it.bind("foo", "mi", fock[:o, :o])
+    it.bind("fov", "me", fock[:o, o:])
+    it.bind("fvo", "ai", fock[o:, :o])
+    it.bind("fvv", "ae", fock[o:, o:])
+    it.run(load_plan("CCLR_PLAN_OMEGA"))
+    return it.get("om1").copy(), it.get("om2").copy()

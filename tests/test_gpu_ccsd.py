@@ -56,3 +56,40 @@ def test_divergent_input_reports_not_converged():
     f = synth.fock(o, v, seed=0)
     t1, t2, info = cc.cclr_ccsd(o, v, f.cuda(), {k: x.cuda() for k, x in eri.items()}, tol=1e-10, maxiter=6)
     assert info.converged == 0 and info.residual > 1e-10
+
+
+@pytest.mark.parametrize("o,v,diag", [(3, 7, False), (6, 30, True)])
+def test_both_residual_routes_match_the_oracle(o, v, diag):
+    """cclr_ccsd_residual mode 0 (direct plan) and mode 1 (quadrature of the Jacobian) against oracle.ccsd.residual at random
+    unconverged amplitudes."""
+    import paper_2307_14296_b200 as cc
+    eri = synth.eri_packed(o, v, seed=3, scale=0.1)
+    f = synth.fock(o, v, seed=3)
+    if not diag:
+        f = f + 0.05 * torch.from_numpy(synth.hermitian_operator(o + v, 3, 7))
+    t1, t2 = synth.amplitudes(o, v, seed=4, scale=0.05)
+    ints = ccsd.Integrals(o, v, f.numpy(), **packing.unpack_eri(o, v, {k: x.numpy() for k, x in eri.items()}))
+    w1, w2 = packing.pack_amplitudes(*ccsd.residual(ints, *packing.unpack_amplitudes(t1[0].numpy(), t2[0].numpy(), o, v)))
+    dev = {k: x.cuda() for k, x in eri.items()}
+    for mode in (0, 1):
+        g1, g2 = cc.cclr_ccsd_residual(o, v, f.contiguous().cuda(), dev, t1[0].cuda(), t2[0].cuda(), mode)
+        torch.cuda.synchronize()
+        assert np.linalg.norm(g1.cpu().numpy() - w1.reshape(-1)) <= 1e-11 * np.linalg.norm(w1), mode
+        assert np.linalg.norm(g2.cpu().numpy() - w2.reshape(-1)) <= 1e-11 * np.linalg.norm(w2), mode
+
+
+def test_residual_routes_agree_at_config5_size():
+    """At a size the oracle cannot reach in seconds (o=18, v=150) the two device routes -- which share no residual code --
+    must agree with each other."""
+    import paper_2307_14296_b200 as cc
+    o, v = 18, 150
+    eri = {k: synth.eri_class(k, o, v, seed=0, device="cuda") for k in ("oooo", "ooov", "oovv", "ovvo", "ovvv", "vvvv")}
+    f = synth.fock(o, v, seed=0).cuda()
+    t1, t2 = synth.first_order_amplitudes(o, v, f, eri["oovv"])
+    t1 = t1 + synth.amplitudes(o, v, seed=5, scale=1e-3, device="cuda")[0][0]
+    a1, a2 = cc.cclr_ccsd_residual(o, v, f, eri, t1, t2, 0)
+    b1, b2 = cc.cclr_ccsd_residual(o, v, f, eri, t1, t2, 1)
+    rel = lambda x, y: float((x - y).abs().pow(2).sum().sqrt() / y.abs().pow(2).sum().sqrt())
+    assert rel(a1, b1) < 1e-11 and rel(a2, b2) < 1e-11
+    del eri
+    torch.cuda.empty_cache()

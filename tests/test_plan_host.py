@@ -99,3 +99,19 @@ def test_eta_plan_reproduces_oracle_eta(o, v, eom):
     r1, r2 = packing.pack_amplitudes(*(c.eta_eom(X, l1, l2) if eom else c.eta(X, l1, l2)))
     assert np.linalg.norm(s1.reshape(-1) - r1.reshape(-1)) <= 1e-12 * np.linalg.norm(r1)
     assert np.linalg.norm(s2.reshape(-1) - r2.reshape(-1)) <= 1e-12 * np.linalg.norm(r2)
+
+
+@pytest.mark.parametrize("o,v,chunk", [(3, 5, None), (4, 6, 2), (2, 7, 3)])
+def test_omega_plan_reproduces_oracle_residual(o, v, chunk):
+    """The direct CCSD residual plan of cclr_ccsd against oracle.ccsd.residual (pinned by the determinant space), at random
+    unconverged complex t and a non-diagonal Fock matrix."""
+    f, V = random_system(o, v, seed=100 + v, diag_fock=False)
+    t1, t2 = random_amplitudes(o, v, seed=101)
+    ints = ccsd.Integrals.from_full(f, V, o)
+    full = dict(oooo=ints.oooo, ooov=ints.ooov, oovv=ints.oovv, ovvo=ints.ovvo, ovvv=ints.ovvv, vvvv=ints.vvvv)
+    packed = packing.pack_eri(full)
+    t1p, t2p = packing.pack_amplitudes(t1, t2)
+    s1, s2 = plan_interp.run_omega(o, v, f, packed, t1p, t2p, chunk)
+    r1, r2 = packing.pack_amplitudes(*ccsd.residual(ints, t1, t2))
+    assert np.abs(s1.reshape(-1) - r1.reshape(-1)).max() <= 1e-12 * max(1.0, np.abs(r1).max())
+    assert np.abs(s2.reshape(-1) - r2.reshape(-1)).max() <= 1e-12 * max(1.0, np.abs(r2).max())
