@@ -206,6 +206,7 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
+    cc.cclr_set_gemm_mode(args.gemm == "3m")
     cfg = CONFIGS[args.config]
     o, v, nvec = cfg["o"], cfg["v"], cfg["nvec"]
     n1, n2 = o * v, npair(o) * npair(v)
@@ -272,7 +273,7 @@ def run_ours(args):
         "config": {"workload": workload_name(args.config, o, v), "o": o, "v": v, "nvec": nvec, "omega": omega,
                    "gamma": gamma, "sigma_V": synth.sigma_v(v), "ground_state": ground, "parallelism": "replicas x%d" % world,
                    "l2": "inputs larger than L2 (W_vvvv %.2f GB streamed every step)" % (npair(v) ** 2 * 16 / 1e9),
-                   "flops_per_step": flops_step, "context_bytes": ctx.bytes()},
+                   "flops_per_step": flops_step, "complex_product": args.gemm, "context_bytes": ctx.bytes()},
         "e2e": {"value": flops_step * world * args.steps / (e2e_ms * 1e-3) / 1e12, "unit": UNIT,
                 "h2d_bytes_per_step": (n1 + n2) * nvec * 16, "d2h_bytes_per_step": (n1 + n2) * nvec * 16,
                 "ms_per_step": e2e_ms / args.steps},
@@ -285,9 +286,14 @@ def run_ours(args):
         lad_ms = phases["ladder"] / (args.steps * nvec)
         lad_flops = 8.0 * cm["T11"]
         line["roofline"] = {
-            "bound": "tensor", "kernel": "zgemm_kernel<128,64,16,32,32,4,kn> (pp ladder T11)",
+            "bound": "tensor", "kernel": "zgemm_kernel<128,%s,16,...,kn,%s> (pp ladder T11)" % ("48" if args.gemm == "3m" else "64", args.gemm),
             "achieved": lad_flops / (lad_ms * 1e-3) / 1e12, "peak": peak, "unit": UNIT,
             "frac": lad_flops / (lad_ms * 1e-3) / 1e12 / peak,
+            "complex_product": args.gemm,
+            "pipe_frac": (0.75 if args.gemm == "3m" else 1.0) * lad_flops / (lad_ms * 1e-3) / 1e12 / peak,
+            "note": "achieved counts 8 real flop per complex multiply-add (SURVEY 8(d) convention, whatever the product); the 3M "
+                    "product issues 6 of them on the FP64 tensor pipe (3 real MACs instead of 4), so frac may exceed 1 while "
+                    "pipe_frac = executed DMMA flops / peak stays below it",
             "peak_source": "FP64 tensor (DMMA m8n8k4) issue-rate probe cclr_fp64_tensor_peak measured in this run; "
                            "MEASURED_PEAKS.json has no FP64 entry (nominal HGX B200: 37 TFLOP/s)",
             "traffic": NCU_LADDER_TRAFFIC.get(args.config), "traffic_source": "profiles/r01_config4_sigma_step_ncu.md / "
@@ -364,6 +370,7 @@ def main():
     ap.add_argument("--no-solve", action="store_true")
     ap.add_argument("--ccsd", action="store_true", help="converge the ground-state amplitudes with cclr_ccsd first "
                     "(default: first-order amplitudes; sigma does not depend on the convergence of T, DESIGN.md)")
+    ap.add_argument("--gemm", default="3m", choices=["3m", "4m"], help="complex product of the large contractions")
     ap.add_argument("--ops", action="store_true", help="add the per-operation times of the last sigma step to the line")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
     args = ap.parse_args()

@@ -206,6 +206,13 @@ int cclr_zgemm(void *cuda_stream, int M, int N, int K, const cclr_c128 *alpha, c
                int conj_a, const cclr_c128 *B, long ldb, int b_is_kn, int conj_b, const cclr_c128 *beta,
                cclr_c128 *C, long ldc, int batch, long sa, long sb, long sc);
 
+/* Complex-product mode of the GEMM engine (process-wide): 1 (default) = the large contractions (M >= 512, N >= 24, K >= 64:
+ * ladder, ring, W builds) use the 3M product -- T1 = Ar Br, T2 = Ai Bi, T3 = (Ar+Ai)(Br+Bi), C = (T1 - T2) + i (T3 - T1 - T2):
+ * three real FP64 tensor-core products per complex one instead of four; 0 = 4M everywhere.  Both hold the 1e-10 parity
+ * tolerance (north_star: "3M only if it holds the tolerance"). */
+int cclr_set_gemm_mode(int three_m);
+int cclr_get_gemm_mode(void);
+
 /* The particle-particle ladder alone (term T11 of S-Eq. 12):
  * out2[k][ab][ij] = sum_{e<f} W_vvvv[ab][ef] x2[k][ef][ij] for nvec vectors (no shift, no other term). */
 int cclr_ladder(cclr_ctx *ctx, const cclr_c128 *x2, int nvec, cclr_c128 *out2);

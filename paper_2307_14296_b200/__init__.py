@@ -339,6 +339,15 @@ def cclr_zgemm(A, B, C_out, alpha=1.0, beta=0.0, conj_a=False, conj_b=False, b_i
     return C_out
 
 
+def cclr_set_gemm_mode(three_m):
+    """1: large contractions use the 3M complex product (default); 0: 4M everywhere."""
+    _lib.check(_lib.load().cclr_set_gemm_mode(int(bool(three_m))), "cclr_set_gemm_mode")
+
+
+def cclr_get_gemm_mode():
+    return int(_lib.load().cclr_get_gemm_mode())
+
+
 def cclr_kernel_launches():
     return int(_lib.load().cclr_kernel_launches())
 

@@ -70,6 +70,12 @@ __global__ void copy_kernel(const double2 *__restrict__ src, double2 *__restrict
 
 }  // namespace
 
+extern "C" int cclr_set_gemm_mode(int three_m) {
+  zgemm_set_mode(three_m);
+  return CCLR_OK;
+}
+extern "C" int cclr_get_gemm_mode(void) { return zgemm_get_mode(); }
+
 extern "C" int cclr_last_cuda_error(void) { return g_last_cuda_error; }
 
 extern "C" const char *cclr_strerror(int code) {

@@ -92,7 +92,7 @@ struct ZgemmArgs {
 // ---------------------------------------------------------------------------------------------------------------
 // kernel
 // ---------------------------------------------------------------------------------------------------------------
-template <int BM, int BN, int BK, int WM, int WN, int STAGES, bool BKN>
+template <int BM, int BN, int BK, int WM, int WN, int STAGES, bool BKN, bool M3>
 __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 32 + 128, 1)
 zgemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const ZgemmArgs p) {
   constexpr int WARPS_M = BM / WM, WARPS_N = BN / WN, NCW = WARPS_M * WARPS_N;
@@ -171,8 +171,94 @@ zgemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CU
   asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(CONSUMER_REGS));
   const int gid = lane >> 2, tig = lane & 3;
   const int rmap = ((gid & 1) << 2) | (gid >> 1);   // row permutation inside an 8-row group (bank-conflict free)
-  const int par = gid & 1, nb4 = gid >> 1;
   const int wm = warp / WARPS_N, wn = warp % WARPS_N;
+  if constexpr (M3) {
+    // ===== 3M complex product (Karatsuba): T1 = Ar Br, T2 = Ai Bi, T3 = (Ar + Ai)(Br + Bi); C = (T1 - T2) + i (T3 - T1 - T2).
+    // One DMMA tile is 8 rows x 8 COMPLEX columns here (no re/im doubling of the columns), three real accumulator tiles per
+    // complex tile: 3 DMMA per 8 x 8 x 4 complex block instead of 4.  Physical column of DMMA column g is 8*g3 + rmap(g)
+    // (same permutation as the rows) so that the B fragment loads stay bank-conflict free under the 128-byte swizzle.
+    static_assert(WN % 8 == 0, "3M warp tile");
+    constexpr int NG3 = WN / 8;
+    const uint32_t sa3 = p.conjA ? 0x80000000u : 0u, sb3 = p.conjB ? 0x80000000u : 0u;
+    uint32_t a_off3[2], b_off3[2];
+#pragma unroll
+    for (int s4 = 0; s4 < 2; ++s4) {
+      const int k = 4 * s4 + tig;
+      a_off3[s4] = (uint32_t)((wm * WM + rmap) * 128 + ((k ^ rmap) << 4));
+      b_off3[s4] = !BKN ? (uint32_t)((wn * WN + rmap) * 128 + ((k ^ rmap) << 4))
+                        : (uint32_t)(((wn * WN) >> 3) * (BK * 128) + k * 128 + ((rmap ^ k) << 4));
+    }
+    double acc3[MI][NG3][3][2];
+#pragma unroll
+    for (int i = 0; i < MI; ++i)
+#pragma unroll
+      for (int g = 0; g < NG3; ++g)
+#pragma unroll
+        for (int t = 0; t < 3; ++t) acc3[i][g][t][0] = acc3[i][g][t][1] = 0.0;
+    for (int c = 0; c < nchunks; ++c) {
+      const int s = c % STAGES;
+      const uint32_t ph = (c / STAGES) & 1;
+      mbar_wait(bar_base + 8 * s, ph);
+      const uint32_t sA = smem_base + s * STAGE_BYTES, sB = sA + A_BYTES;
+#pragma unroll
+      for (int kb = 0; kb < BK / 8; ++kb) {
+#pragma unroll
+        for (int s4 = 0; s4 < 2; ++s4) {
+          double ar[MI], ai[MI], as[MI];
+#pragma unroll
+          for (int i = 0; i < MI; ++i) {
+            const double2 a = lds128(sA + kb * (BM * 128) + a_off3[s4] + i * 1024);
+            ar[i] = a.x;
+            ai[i] = flip_sign(a.y, sa3);
+            as[i] = ar[i] + ai[i];
+          }
+#pragma unroll
+          for (int g = 0; g < NG3; ++g) {
+            const uint32_t addr = !BKN ? sB + kb * (BN * 128) + g * 1024 + b_off3[s4]
+                                       : sB + g * (BK * 128) + kb * 1024 + b_off3[s4];
+            const double2 b = lds128(addr);
+            const double br = b.x, bi = flip_sign(b.y, sb3), bs = br + bi;
+#pragma unroll
+            for (int i = 0; i < MI; ++i) dmma884(acc3[i][g][0][0], acc3[i][g][0][1], ar[i], br);
+#pragma unroll
+            for (int i = 0; i < MI; ++i) dmma884(acc3[i][g][1][0], acc3[i][g][1][1], ai[i], bi);
+#pragma unroll
+            for (int i = 0; i < MI; ++i) dmma884(acc3[i][g][2][0], acc3[i][g][2][1], as[i], bs);
+          }
+        }
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar_base + 8 * (STAGES + s));
+    }
+    const bool partial3 = is_tail;
+    c128 *Cb3 = partial3 ? p.partial + ((size_t)(blockIdx.x - p.main_tiles)) * (size_t)(BM * BN) -
+                               ((size_t)tile_m * BM * BN + (size_t)tile_n * BN)
+                         : p.C + (size_t)batch * p.sc;
+    const long ldc3 = partial3 ? (long)BN : p.ldc;
+    const c128 alpha3 = partial3 ? make_double2(1.0, 0.0) : p.alpha;
+    const c128 beta3 = partial3 ? make_double2(0.0, 0.0) : p.beta;
+    const bool has_beta3 = (beta3.x != 0.0) || (beta3.y != 0.0);
+#pragma unroll
+    for (int i = 0; i < MI; ++i) {
+      const int row = tile_m * BM + wm * WM + i * 8 + rmap;
+      if (row >= p.M) continue;
+#pragma unroll
+      for (int g = 0; g < NG3; ++g) {
+#pragma unroll
+        for (int cc = 0; cc < 2; ++cc) {
+          const int col = tile_n * BN + wn * WN + g * 8 + (cc ? 4 + tig : tig);
+          if (col >= p.N) continue;
+          const double t1 = acc3[i][g][0][cc], t2 = acc3[i][g][1][cc], t3 = acc3[i][g][2][cc];
+          c128 *dst = Cb3 + (size_t)row * ldc3 + col;
+          c128 r = cmul(alpha3, make_double2(t1 - t2, t3 - t1 - t2));
+          if (has_beta3) r = cadd(r, cmul(beta3, *dst));
+          *dst = r;
+        }
+      }
+    }
+    return;
+  }
+  const int par = gid & 1, nb4 = gid >> 1;
   const int wpar = ((wn * WN) >> 2) & 1;            // WN may be an odd multiple of 4: parity of the warp's first 4-row group
   // sign masks (see header comment): f1 = m1 ^ (par ? b.im : b.re), f2 = m2 ^ (par ? b.re : b.im)
   const uint32_t sa = p.conjA ? 0x80000000u : 0u, sb = p.conjB ? 0x80000000u : 0u;
@@ -319,11 +405,11 @@ bool make_map(CUtensorMap *tm, const c128 *base, long inner_complex, long rows, 
   return r == CUDA_SUCCESS;
 }
 
-template <int BM, int BN, int BK, int WM, int WN, int STAGES, bool BKN>
+template <int BM, int BN, int BK, int WM, int WN, int STAGES, bool BKN, bool M3 = false>
 cudaError_t launch(cudaStream_t st, const CUtensorMap &tmA, const CUtensorMap &tmB, const ZgemmArgs &args, int ctas) {
   constexpr int threads = (BM / WM) * (BN / WN) * 32 + 128;
   constexpr int smem = STAGES * (BM + BN) * BK * 16 + 2 * STAGES * 8 + 1024;
-  auto kern = zgemm_kernel<BM, BN, BK, WM, WN, STAGES, BKN>;
+  auto kern = zgemm_kernel<BM, BN, BK, WM, WN, STAGES, BKN, M3>;
   static bool configured = false;
   if (!configured) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
@@ -344,6 +430,13 @@ cudaError_t launch_ng(cudaStream_t st, const CUtensorMap &tmA, const CUtensorMap
               : launch<128, 8 * NG, ZG_BK, 32, 4 * NG, ZG_STAGES, false>(st, tmA, tmB, args, ctas);
   return kn ? launch<64, 8 * NG, ZG_BK, 16, 4 * NG, ZG_STAGES, true>(st, tmA, tmB, args, ctas)
             : launch<64, 8 * NG, ZG_BK, 16, 4 * NG, ZG_STAGES, false>(st, tmA, tmB, args, ctas);
+}
+
+// 3M variant: BN = 16 * NG3 (two warps of NG3 eight-column DMMA groups), 128-row tiles
+template <int NG3>
+cudaError_t launch_3m(cudaStream_t st, const CUtensorMap &tmA, const CUtensorMap &tmB, const ZgemmArgs &args, int ctas, bool kn) {
+  return kn ? launch<128, 16 * NG3, ZG_BK, 32, 8 * NG3, ZG_STAGES, true, true>(st, tmA, tmB, args, ctas)
+            : launch<128, 16 * NG3, ZG_BK, 32, 8 * NG3, ZG_STAGES, false, true>(st, tmA, tmB, args, ctas);
 }
 
 // C tile = alpha * sum_splits partial + beta * C for the K-split tail tiles
@@ -448,6 +541,10 @@ __global__ void __launch_bounds__(256) zgemv_kernel(int M, int K, c128 alpha, co
 
 }  // namespace
 
+static int g_gemm_3m = 1;   // 1: large contractions use the 3M complex product (zgemm_set_mode)
+void zgemm_set_mode(int three_m) { g_gemm_3m = three_m ? 1 : 0; }
+int zgemm_get_mode() { return g_gemm_3m; }
+
 int zgemm_num_sms() {
   static int n = 0;
   if (!n) {
@@ -467,7 +564,10 @@ cudaError_t zgemm(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *
   const int sms = zgemm_num_sms();
   // 64-row tiles when they cut the padding of M by more than 10 % (M of a few hundred: 300 -> 320 instead of 384)
   const long pad128 = (M + 127L) / 128 * 128, pad64 = (M + 63L) / 64 * 64;
-  const int BM = (pad64 * 10 <= pad128 * 9) ? 64 : 128;
+  // 3M complex product (3 real DMMA products per complex one instead of 4) for the large contractions; the 4M kernel keeps
+  // the small and skinny ones, where tile padding, not the DMMA count, is the cost
+  const bool use3m = g_gemm_3m && M >= 512 && N >= 24 && K >= 64;
+  const int BM = use3m ? 128 : ((pad64 * 10 <= pad128 * 9) ? 64 : 128);
   if (K <= 0) {  // C = beta * C
     zgemm_reduce_kernel<<<256, 256, 0, st>>>(nullptr, 0, M, N, alpha, beta, C, ldc, sc, batch);
     cclr_count_launch();
@@ -510,7 +610,12 @@ cudaError_t zgemm(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *
     const long bn = 8 * ng, padded = (N + bn - 1) / bn * bn;
     if (padded * 100 <= best * 101) { NG = ng; break; }
   }
-  const int BN = 8 * NG;
+  int NG3 = 3;
+  if (use3m) {
+    const long p48 = (N + 47L) / 48 * 48, p32 = (N + 31L) / 32 * 32;
+    NG3 = (p32 * 100 < p48 * 99) ? 2 : 3;
+  }
+  const int BN = use3m ? 16 * NG3 : 8 * NG;
   ZgemmArgs args{};
   args.M = M; args.N = N; args.K = K;
   args.C = C; args.ldc = ldc; args.sc = sc;
@@ -558,6 +663,9 @@ cudaError_t zgemm(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *
     if (!make_map(&tmB, B, N, K, ldb, batch, sb, BK)) return cudaErrorInvalidValue;
   }
   cudaError_t e;
+  if (use3m) {
+    e = NG3 == 2 ? launch_3m<2>(st, tmA, tmB, args, ctas, b_is_kn) : launch_3m<3>(st, tmA, tmB, args, ctas, b_is_kn);
+  } else
   switch (NG) {
     case 4: e = launch_ng<4>(st, tmA, tmB, args, ctas, b_is_kn, BM); break;
     case 5: e = launch_ng<5>(st, tmA, tmB, args, ctas, b_is_kn, BM); break;

@@ -79,6 +79,37 @@ def test_zgemm_matches_numpy(M, N, K, kn, ca, cb, beta):
     assert rel(Cd.cpu().numpy(), ref) < 1e-13
 
 
+@pytest.mark.parametrize("M,N,K,kn,ca,cb,beta", [
+    (640, 100, 300, True, False, False, 0.0), (640, 100, 300, False, True, True, 1.0),
+    (513, 24, 64, True, True, False, 0.5), (1300, 561, 96, True, False, False, 0.0),
+    (1300, 153, 200, False, False, True, -1.0), (5120, 276, 200, True, False, False, 1.0),
+    (700, 10200 // 8, 130, False, False, False, 0.0),
+])
+def test_zgemm_3m_and_4m_modes_match_numpy(M, N, K, kn, ca, cb, beta):
+    """The large-contraction path in both complex-product modes (3M: three real DMMA products per complex one; 4M: four),
+    both tile widths of the 3M kernel (32, 48), both B layouts, conjugations, K-split tail tiles."""
+    cc = _lib()
+    rng = np.random.default_rng(M + N + K)
+    A = rng.normal(size=(M, K)) + 1j * rng.normal(size=(M, K))
+    B = rng.normal(size=(K, N) if kn else (N, K)) + 1j * rng.normal(size=(K, N) if kn else (N, K))
+    C0 = rng.normal(size=(M, N)) + 1j * rng.normal(size=(M, N))
+    alpha = -0.4 + 0.9j
+    opA = A.conj() if ca else A
+    opB = B.conj() if cb else B
+    ref = alpha * (opA @ (opB if kn else opB.T)) + beta * C0
+    try:
+        for mode in (1, 0):
+            cc.cclr_set_gemm_mode(mode)
+            assert cc.cclr_get_gemm_mode() == mode
+            Cd = torch.from_numpy(C0.copy()).cuda()
+            cc.cclr_zgemm(torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda(), Cd, alpha=alpha, beta=beta, conj_a=ca,
+                          conj_b=cb, b_is_kn=kn)
+            torch.cuda.synchronize()
+            assert rel(Cd.cpu().numpy(), ref) < 1e-13, mode
+    finally:
+        cc.cclr_set_gemm_mode(1)
+
+
 def test_zgemm_batched_and_strided():
     cc = _lib()
     rng = np.random.default_rng(5)
