@@ -148,7 +148,7 @@ def run_reference(args):
 
 
 # DRAM traffic of one ladder launch from the ncu captures under profiles/ (bytes; None where no capture exists)
-NCU_LADDER_TRAFFIC = {3: 7.12e9, 4: 43.55e9}
+NCU_LADDER_TRAFFIC = {("4m", 3): 7.12e9, ("4m", 4): 43.55e9, ("3m", 3): 7.21e9, ("3m", 4): 48.10e9}
 
 CONFIGS = {1: dict(o=4, v=20, nvec=1), 2: dict(o=10, v=80, nvec=1), 3: dict(o=24, v=200, nvec=1),
            4: dict(o=34, v=300, nvec=1), 5: dict(o=18, v=150, nvec=3)}
@@ -296,8 +296,9 @@ def run_ours(args):
                     "pipe_frac = executed DMMA flops / peak stays below it",
             "peak_source": "FP64 tensor (DMMA m8n8k4) issue-rate probe cclr_fp64_tensor_peak measured in this run; "
                            "MEASURED_PEAKS.json has no FP64 entry (nominal HGX B200: 37 TFLOP/s)",
-            "traffic": NCU_LADDER_TRAFFIC.get(args.config), "traffic_source": "profiles/r01_config4_sigma_step_ncu.md / "
-            "r01_zgemm_ncu_full_config3.md (dram__bytes_read.sum + dram__bytes_write.sum of the ladder launch)",
+            "traffic": NCU_LADDER_TRAFFIC.get((args.gemm, args.config)),
+            "traffic_source": "profiles/r01_config4_sigma_step_ncu[_3m].md / r01_zgemm_ncu_full_config3.md "
+                              "(dram__bytes_read.sum + dram__bytes_write.sum of the ladder launch)",
             "algorithmic_bytes": 16.0 * (npair(v) ** 2 + 2 * n2), "ms_per_launch": lad_ms,
         }
         tot = max(phases["total"], 1e-9)
