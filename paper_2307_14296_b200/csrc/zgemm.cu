@@ -568,6 +568,14 @@ cudaError_t zgemm(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *
   // the small and skinny ones, where tile padding, not the DMMA count, is the cost
   const bool use3m = g_gemm_3m && M >= 512 && N >= 24 && K >= 64;
   const int BM = use3m ? 128 : ((pad64 * 10 <= pad128 * 9) ? 64 : 128);
+  if (batch > 1 && (sa == 0 || sb == 0)) {   // a shared operand has no batch stride a tensor map could carry: one launch per batch
+    for (int b = 0; b < batch; ++b) {
+      const cudaError_t e = zgemm(st, M, N, K, alpha, A + (size_t)b * sa, lda, conjA, B + (size_t)b * sb, ldb, b_is_kn, conjB, beta,
+                                  C + (size_t)b * sc, ldc, 1, 0, 0, 0, ws);
+      if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
+  }
   if (K <= 0) {  // C = beta * C
     zgemm_reduce_kernel<<<256, 256, 0, st>>>(nullptr, 0, M, N, alpha, beta, C, ldc, sc, batch);
     cclr_count_launch();

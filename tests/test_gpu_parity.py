@@ -121,6 +121,19 @@ def test_zgemm_batched_and_strided():
     assert rel(C.cpu().numpy(), A @ B) < 1e-13
 
 
+def test_zgemm_batched_with_a_shared_operand():
+    """batch > 1 with stride 0 on A (one matrix applied to a block of right-hand sides)."""
+    cc = _lib()
+    rng = np.random.default_rng(6)
+    A = rng.normal(size=(70, 40)) + 1j * rng.normal(size=(70, 40))
+    B = rng.normal(size=(3, 40, 50)) + 1j * rng.normal(size=(3, 40, 50))
+    C = torch.zeros((3, 70, 50), dtype=torch.complex128, device="cuda")
+    cc.cclr_zgemm(torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda(), C, b_is_kn=True, M=70, N=50, K=40, lda=40, ldb=50,
+                  ldc=50, batch=3, sa=0, sb=40 * 50, sc=70 * 50)
+    torch.cuda.synchronize()
+    assert rel(C.cpu().numpy(), np.einsum("mk,bkn->bmn", A, B)) < 1e-13
+
+
 # ---------------------------------------------------------------------------------------------------------------
 INTERMEDIATES = {
     # name -> oracle array in the library's layout (DESIGN.md "Data layout")
