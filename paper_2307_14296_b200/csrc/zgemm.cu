@@ -275,8 +275,10 @@ zgemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CU
       // row n = wn*WN + 4g + nb4 ; (n & 7) = ((g & 1) << 2) | nb4 -> handled per g below
       b_off[s4] = (uint32_t)((wn * WN + nb4) * 128 + (k << 4));
     } else {
-      // row k (inside a box of BK rows: + kb*8*128 per 8-k block), col n = wn*WN + 4g + nb4
-      b_off[s4] = (uint32_t)(k * 128);
+      // row k (inside a box of BK rows: + kb*8*128 per 8-k block), col n = wn*WN + 4g + nb4.  For WN a multiple of 8 the box
+      // of the warp's first column and the lane part (nb4 ^ k) of the swizzled chunk are folded in here; the loop then only
+      // adds compile-time terms and flips bit 6 for odd g
+      b_off[s4] = (WN % 8 == 0) ? (uint32_t)(((wn * WN) >> 3) * (BK * 128) + k * 128 + ((nb4 ^ k) << 4)) : (uint32_t)(k * 128);
     }
   }
 
@@ -304,6 +306,9 @@ zgemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CU
           if (!BKN) {
             const int n7 = (((g & 1) ^ wpar) << 2) | nb4;   // (row & 7) of row = wn*WN + 4g + nb4
             addr = sB + kb * (BN * 128) + g * 512 + (b_off[s4] ^ (uint32_t)(n7 << 4));
+          } else if constexpr (WN % 8 == 0) {
+            // n = wn*WN + 4g + nb4 with wn*WN a multiple of 8: box (n >> 3) = wn*WN/8 + g/2, (n & 7) = 4 (g & 1) + nb4
+            addr = sB + (uint32_t)(g >> 1) * (BK * 128) + kb * 1024 + (b_off[s4] ^ (uint32_t)((g & 1) << 6));
           } else {
             const int n = wn * WN + 4 * g + nb4;
             const int k7 = 4 * s4 + tig;
