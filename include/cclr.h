@@ -200,7 +200,8 @@ int cclr_sigma_host(cclr_ctx *ctx, const cclr_c128 *x1, const cclr_c128 *x2, int
 /* C[M][N] = alpha * opA(A)[M][K] * opB(B) + beta * C, complex128, row-major with leading dimensions in elements.
  * A is always [M][K] (K contiguous).  b_is_kn = 0: B is [N][K] (K contiguous); 1: B is [K][N] (N contiguous).
  * conj_a / conj_b conjugate the operand elementwise.  batch > 1 repeats with element strides sa, sb, sc.
- * The 4M complex product runs on the FP64 tensor cores (DMMA) from TMA-staged shared-memory tiles.
+ * The complex product (4M, or 3M for large shapes: cclr_set_gemm_mode) runs on the FP64 tensor cores (DMMA) from TMA-staged
+ * shared-memory tiles; N = 1 / M = 1 shapes go to bandwidth-bound matrix-vector kernels.
  * alpha, beta are host pointers to one complex number. */
 int cclr_zgemm(void *cuda_stream, int M, int N, int K, const cclr_c128 *alpha, const cclr_c128 *A, long lda,
                int conj_a, const cclr_c128 *B, long ldb, int b_is_kn, int conj_b, const cclr_c128 *beta,

@@ -13,6 +13,8 @@
 //         acc += a.re * (parity ? b.im :  b.re)      acc += a.im * (parity ? b.re : -b.im)
 //     where parity = "this lane feeds an imaginary output column".  conj(A)/conj(B) only flip sign bits.
 //     The C fragment of m8n8k4 (row g, real columns 2t, 2t+1) is then exactly one complex number per lane.
+//   * 3M variant (template flag M3) for the large contractions: T1 = Ar Br, T2 = Ai Bi, T3 = (Ar + Ai)(Br + Bi) on 8 x 8-complex
+//     DMMA tiles with three real accumulator tiles per complex tile -- 3 DMMA per 8 x 8 x 4 complex block instead of 4.
 //   * operands are staged by TMA (cp.async.bulk.tensor, FLOAT64 tensor maps over the interleaved data, boxes of
 //     128 B x rows, SWIZZLE_128B) into a STAGES-deep ring guarded by full/empty mbarriers; one producer warp,
 //     (BM/WM)*(BN/WN) consumer warps.  Fragment loads are single conflict-free LDS.128 per complex element:
@@ -20,7 +22,9 @@
 //         quarter-warp differ in address bit 9 and the swizzle separates them;
 //       - N-contiguous B ([K][N]): the four k rows of a quarter-warp are separated by the swizzle directly.
 //   * ragged M, N, K: TMA zero-fills out-of-bounds loads; stores are guarded.
-//   * optional split-K (partials in a workspace + a deterministic reduce kernel) for tall-K / tiny-MN contractions.
+//   * tile shape per call (BM 128 | 64, BN 32..64), a 1-D tile grid whose last partial wave is split along K (partials in a
+//     workspace + a deterministic reduce kernel; the same mechanism serves tall-K / tiny-MN contractions), and
+//     matrix-vector kernels for N = 1 / M = 1.
 #include "common.cuh"
 #include <mutex>
 
