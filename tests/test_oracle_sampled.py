@@ -37,3 +37,66 @@ def test_ladder_rows_is_term_T11():
     rows = [0, 3, 14]
     got = sampled.ladder_rows(eri["vvvv"].reshape(15, 15)[rows], x2p)
     assert np.abs(got - want[rows]).max() < 1e-14
+
+
+def _small_system_with_T(o, v):
+    eri = {k: x.numpy() for k, x in synth.eri_packed(o, v, seed=o + 3 * v, scale=0.3).items()}
+    f = synth.fock(o, v, seed=2).numpy() + 0.1 * synth.hermitian_operator(o + v, 3, 5)      # f_ov != 0 on purpose
+    t1, t2 = synth.amplitudes(o, v, seed=4, scale=0.4)
+    t1, t2 = t1[0].numpy(), t2[0].numpy()
+    ints = ccsd.Integrals(o, v, f, **packing.unpack_eri(o, v, eri))
+    c = cclr.CCLR(ints, *packing.unpack_amplitudes(t1, t2, o, v))
+    vvvv = eri["vvvv"].reshape(packing.npair(v), -1)
+    s = sampled.SampledCCLR(o, v, f, eri, lambda ab: vvvv[ab], t1, t2)
+    return c, s
+
+
+@pytest.mark.parametrize("o,v", [(3, 5), (4, 6)])
+def test_dressed_intermediate_slices_match_full_oracle(o, v):
+    """Every slice method of SampledCCLR against the full-tensor intermediates of oracle.cclr.CCLR (pinned by the
+    determinant-space definitions), all slices, random complex T: a wrong sign, index or symmetry relation fails here."""
+    c, s = _small_system_with_T(o, v)
+    tol = 1e-13
+    assert np.abs(s.Fme() - c.Fme).max() < tol
+    assert np.abs(s.Fmi() - c.Fmi).max() < tol
+    for a in range(v):
+        assert np.abs(s.Fae_row(a) - c.Fae[a]).max() < tol
+        assert np.abs(s.Wamef_a(a) - c.Wamef[a]).max() < tol
+    for i in range(o):
+        assert np.abs(s.Wmnie_i(i) - c.Wmnie[:, :, i, :]).max() < tol
+        for j in range(o):
+            assert np.abs(s.Wmnij_col(i, j) - c.Wmnij[:, :, i, j]).max() < tol
+    for b in range(v):
+        for j in range(o):
+            assert np.abs(s.Wbar_bj(b, j) - c.Wbar[:, b, :, j]).max() < tol
+            assert np.abs(s.Wmbej_bj(b, j) - c.Wmbej[:, b, :, j]).max() < tol
+            for i in range(o):
+                assert np.abs(s.Wmbij_bij(b, i, j) - c.Wmbij[:, b, i, j]).max() < tol
+    for b in range(v):
+        for a in range(b):
+            assert np.abs(s.Wabef_row(a, b) - c.Wabef[a, b]).max() < tol
+            for j in range(o):
+                assert np.abs(s.Wabej_abj(a, b, j) - c.Wabej[a, b, :, j]).max() < tol
+
+
+@pytest.mark.parametrize("o,v", [(3, 5), (4, 6)])
+def test_sigma_elements_with_T_match_full_oracle(o, v):
+    c, s = _small_system_with_T(o, v)
+    x1, x2 = synth.amplitudes(o, v, seed=6, cls1="x1", cls2="x2")
+    x1, x2 = x1[0].numpy(), x2[0].numpy()
+    z = 0.0773 + 0.0045j
+    w1, w2 = c.sigma(*packing.unpack_amplitudes(x1, x2, o, v), z=z)
+    singles = [(a, i) for a in range(v) for i in range(o)]
+    doubles = [(a, b, i, j) for b in range(v) for a in range(b) for j in range(o) for i in range(j)]
+    g1, g2 = s.sigma_elements(x1, x2, singles, doubles, z=z)
+    assert np.abs(np.array(g1) - np.array([w1[a, i] for a, i in singles])).max() < 1e-12
+    assert np.abs(np.array(g2) - np.array([w2[a, b, i, j] for a, b, i, j in doubles])).max() < 1e-12
+    # and at T = 0 it reduces to the bare-integral definition above
+    eri = {k: x.numpy() for k, x in synth.eri_packed(o, v, seed=o + 3 * v, scale=0.3).items()}
+    vvvv = eri["vvvv"].reshape(packing.npair(v), -1)
+    f = synth.fock(o, v, seed=2).numpy() + 0.1 * synth.hermitian_operator(o + v, 3, 5)
+    s0 = sampled.SampledCCLR(o, v, f, eri, lambda ab: vvvv[ab], np.zeros((v, o), complex),
+                             np.zeros((packing.npair(v), packing.npair(o)), complex))
+    h1, h2 = s0.sigma_elements(x1, x2, singles[:7], doubles[:9], z=z)
+    k1, k2 = sampled.sigma_T0_elements(o, v, f, eri, lambda ab: vvvv[ab], x1, x2, singles[:7], doubles[:9], z=z)
+    assert np.abs(np.array(h1) - np.array(k1)).max() < 1e-13 and np.abs(np.array(h2) - np.array(k2)).max() < 1e-13
