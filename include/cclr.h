@@ -224,6 +224,9 @@ int cclr_ring(cclr_ctx *ctx, const cclr_c128 *x2, cclr_c128 *out2);
 /* Copy a named intermediate to a device buffer of `capacity` elements (tests: block-by-block parity against the
  * oracle).  Names and layouts: see DESIGN.md "Data layout".  Returns the element count, or a negative error. */
 long cclr_get_intermediate(cclr_ctx *ctx, const char *name, cclr_c128 *out, long capacity);
+/* Same for `count` consecutive elements starting at element `offset` of the named intermediate (full-size parity tests: one
+ * row of the 32 GB W_vvvv, one (b,j) slice of W_ovvo, ...).  Returns count, or CCLR_EINVAL if the range is outside the buffer. */
+long cclr_get_intermediate_slice(cclr_ctx *ctx, const char *name, long offset, long count, cclr_c128 *out);
 
 /* Number of CUDA kernels this library has launched in the calling process so far (every GEMM, layout and vector
  * kernel is counted at its launch site; memcpy / memset are not).  bench.py reports the difference over its timed

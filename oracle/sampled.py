@@ -18,7 +18,7 @@ small sizes, all elements, random complex T.
 """
 import numpy as np
 
-from .packing import npair, pairs, unpack_pair_axis
+from .packing import npair, pack_pair_axes, pairs, unpack_pair_axis
 
 
 def pair_index(p, q):
@@ -118,7 +118,7 @@ class SampledCCLR:
         self.o, self.v = o, v
         oo, vv = npair(o), npair(v)
         f = np.asarray(f)
-        self.foo, self.fov, self.fvv = f[:o, :o], f[:o, o:], f[o:, o:]
+        self.foo, self.fov, self.fvo, self.fvv = f[:o, :o], f[:o, o:], f[o:, :o], f[o:, o:]
         self.t1 = np.asarray(t1).reshape(v, o)
         self.t2 = unpack_pair_axis(unpack_pair_axis(np.asarray(t2p).reshape(vv, oo), o, 1), v, 0)
         tt = np.einsum("ai,bj->abij", self.t1, self.t1)
@@ -298,3 +298,237 @@ class SampledCCLR:
             s += 0.5 * np.einsum("ef,ef->", self.Wabef_row(a, b), r2[:, :, i, j])               # T11
             out2.append(s - z * r2[a, b, i, j])
         return out1, out2
+
+    # ========================================================================================================
+    # More slices (other fixed indices) for the left transform, then l (A - z), xi, eta and Omega by elements
+    # ========================================================================================================
+    def with_amplitudes(self, t1, t2p):
+        """A second SampledCCLR on the SAME integrals (shared arrays, nothing copied) at other amplitudes."""
+        import copy
+        s = copy.copy(self)
+        o, v = self.o, self.v
+        s.t1 = np.asarray(t1).reshape(v, o)
+        s.t2 = unpack_pair_axis(unpack_pair_axis(np.asarray(t2p).reshape(npair(v), npair(o)), o, 1), v, 0)
+        tt = np.einsum("ai,bj->abij", s.t1, s.t1)
+        s.tau = s.t2 + tt - tt.transpose(1, 0, 2, 3)
+        s._cache = {k: val for k, val in self._cache.items() if k[0] == "ovvv"}     # bare-integral slices only
+        s._Fme = s._Fmi = None
+        return s
+
+    def ovvv_e(self, e):
+        """<mb||ef> for fixed e -> [m,b,f] (packed over e<f: sign of the pair, zero for f = e)."""
+        def build():
+            v = self.v
+            fidx = np.arange(v)
+            lo, hi = np.minimum(e, fidx), np.maximum(e, fidx)
+            sign = np.where(fidx > e, 1.0, np.where(fidx < e, -1.0, 0.0))
+            idx = np.where(fidx == e, 0, hi * (hi - 1) // 2 + lo)
+            return self.ovvv_packed[:, :, idx] * sign
+        return self._memo(("ovvv_e", e), build)
+
+    def vvvv_ef_col(self, e, f):
+        """<ab||ef> for fixed e < f, all a,b -> [a,b]:  <ab||ef> = conj<ef||ab>."""
+        return np.conj(self.vvvv_ab(e, f))
+
+    def vvvv_e(self, e):
+        """<ab||ef> for fixed e, all a,b,f -> [a,b,f] (v rows of the packed block)."""
+        def build():
+            v = self.v
+            out = np.zeros((v, v, v), complex)
+            for f in range(v):
+                if f != e:
+                    out[:, :, f] = self.vvvv_ef_col(min(e, f), max(e, f)) * (1.0 if e < f else -1.0)
+            return out
+        return self._memo(("vvvv_e", e), build)
+
+    def Fae_col(self, e):
+        """F_ae[a,e] (S-Eq. 16, reading 2) for fixed e -> [a]."""
+        return self._memo(("Fae_col", e), lambda: (
+            self.fvv[:, e] - self.t1 @ self.fov[:, e] - np.einsum("fm,maf->a", self.t1, self.ovvv_e(e))
+            - 0.5 * np.einsum("afmn,mnf->a", self.tau, self.oovv[:, :, e, :], optimize=True)))
+
+    def Wmnij_row(self, m, n):
+        """W_mnij[mn,ij] (S-Eq. 18) for fixed (m,n) -> [i,j]."""
+        def build():
+            q = np.einsum("ej,ie->ij", self.t1, self.ooov[m, n])
+            return (self.oooo[m, n] + q - q.T + 0.5 * np.einsum("efij,ef->ij", self.tau, self.oovv[m, n], optimize=True))
+        return self._memo(("Wmnij_row", m, n), build)
+
+    def Wabef_col(self, e, f):
+        """W_abef[ab,ef] (S-Eq. 22) for fixed (e<f), all a,b -> [a,b]."""
+        def build():
+            q = np.einsum("bm,ma->ab", self.t1, -self.ovvv_packed[:, :, pair_index(e, f)])     # sum_m t1[b,m] <am||ef>
+            return (self.vvvv_ef_col(e, f) - (q - q.T)
+                    + 0.5 * np.einsum("abmn,mn->ab", self.tau, self.oovv[:, :, e, f], optimize=True))
+        return self._memo(("Wabef_col", e, f), build)
+
+    def Wabef_e(self, e):
+        """W_abef[ab,ef] (S-Eq. 22) for fixed e, all a,b,f -> [a,b,f]."""
+        def build():
+            q = np.einsum("bm,maf->abf", self.t1, -self.ovvv_e(e), optimize=True)              # sum_m t1[b,m] <am||ef>
+            return (self.vvvv_e(e) - (q - q.transpose(1, 0, 2))
+                    + 0.5 * np.einsum("abmn,mnf->abf", self.tau, self.oovv[:, :, e, :], optimize=True))
+        return self._memo(("Wabef_e", e), build)
+
+    def Wbar_e(self, e):
+        """Wbar[mb,ej] (S-Eq. 23) for fixed e -> [m,b,j]."""
+        return self._memo(("Wbar_e", e), lambda: (
+            self.ovvo[:, :, e, :] - np.einsum("bfnj,mnf->mbj", self.t2, self.oovv[:, :, e, :], optimize=True)))
+
+    def Wbar_m(self, m):
+        """Wbar[mb,ej] (S-Eq. 23) for fixed m -> [b,e,j]."""
+        return self._memo(("Wbar_m", m), lambda: (
+            self.ovvo[m] - np.einsum("bfnj,nef->bej", self.t2, self.oovv[m], optimize=True)))
+
+    def Wmbej_me(self, m, e):
+        """W_mbej[mb,ej] (S-Eq. 19) for fixed (m,e) -> [b,j]."""
+        return self._memo(("Wmbej_me", m, e), lambda: (
+            self.ovvo[m, :, e, :] + np.einsum("fj,bf->bj", self.t1, self.ovvv_e(e)[m])
+            - np.einsum("bn,nj->bj", self.t1, -self.ooov[m, :, :, e])
+            - np.einsum("fbjn,nf->bj", self.t2, self.oovv[m, :, e, :], optimize=True)
+            - np.einsum("fj,bn,nf->bj", self.t1, self.t1, self.oovv[m, :, e, :], optimize=True)))
+
+    def Wamef_me(self, m, e):
+        """W_amef[am,fe] (S-Eq. 25) for fixed m and fixed LAST index e -> [a,f]  (<am||fe> = -<ma||fe> = <ma||ef>)."""
+        return self.ovvv_e(e)[m] - np.einsum("an,nf->af", self.t1, self.oovv[:, m, :, e])
+
+    def Wamef_mef(self, m, e, f):
+        """W_amef[am,ef] (S-Eq. 25) for fixed (m, e<f) -> [a]."""
+        return -self.ovvv_packed[m, :, pair_index(e, f)] - self.t1 @ self.oovv[:, m, e, f]
+
+    def Wmnie_me(self, m, e):
+        """W_mnie[nm,je] (S-Eq. 24) as a function of (n,j) for fixed second index m and fixed e -> [n,j]."""
+        return self.ooov[:, m, :, e] + np.einsum("fj,nf->nj", self.t1, self.oovv[:, m, :, e])
+
+    def Wmbij_m(self, m):
+        """W_mbij[mb,ij] (S-Eq. 20, reading 3) for fixed m -> [b,i,j]."""
+        def build():
+            o, v = self.o, self.v
+            ovvv_m = unpack_pair_axis(self.ovvv_packed[m], v, 1)                                   # <mb||ef> [b,e,f]
+            wmnij_m = np.stack([self.Wmnij_row(m, n) if n != m else np.zeros((o, o), complex) for n in range(o)])
+            c6 = np.einsum("nie,bejn->bij", self.ooov[m], self.t2, optimize=True)
+            c7 = np.einsum("ei,bej->bij", self.t1, self.Wbar_m(m), optimize=True)
+            return (np.conj(self.ooov[:, :, m, :]).transpose(2, 0, 1)
+                    - np.einsum("e,beij->bij", self.Fme()[m], self.t2, optimize=True)
+                    - np.einsum("bn,nij->bij", self.t1, wmnij_m)
+                    + 0.5 * np.einsum("bef,efij->bij", ovvv_m, self.tau, optimize=True)
+                    + (c6 - c6.transpose(0, 2, 1)) + (c7 - c7.transpose(0, 2, 1)))
+        return self._memo(("Wmbij_m", m), build)
+
+    def Wabej_e(self, e):
+        """W_abej[ab,ej] (S-Eq. 21, reading 4) for fixed e -> [a,b,j]."""
+        def build():
+            o, v = self.o, self.v
+            vvvo_e = -np.conj(self.ovvv_b(e)).transpose(1, 2, 0)                                   # <ab||ej> [a,b,j]
+            c1 = np.einsum("mbf,afmj->abj", self.ovvv_e(e), self.t2, optimize=True)
+            c2 = np.einsum("am,mbj->abj", self.t1, self.Wbar_e(e), optimize=True)
+            return (vvvo_e - np.einsum("m,abmj->abj", self.Fme()[:, e], self.t2, optimize=True)
+                    + np.einsum("fj,abf->abj", self.t1, self.Wabef_e(e), optimize=True)
+                    + 0.5 * np.einsum("mnj,abmn->abj", -self.ooov[:, :, :, e], self.tau, optimize=True)
+                    - (c1 - c1.transpose(1, 0, 2)) - (c2 - c2.transpose(1, 0, 2)))
+        return self._memo(("Wabej_e", e), build)
+
+    def sigma_left_elements(self, y1, y2p, singles, doubles, z=0.0):
+        """Elements of the left transform L = l (A - z) for l1[a,i] = l^i_a, l2 packed [vv][oo] (Eq. 13; S-Eq. 13,
+        PAPER.md:895-901 in reading 5 of DESIGN.md: the term-by-term adjoint of S-Eq. 11-12 -- each  s[out] += W . r[in]  gives
+        L[in] += W . l[out] under <l,s> = sum l1 s1 + 1/4 sum l2 s2, exactly as oracle.cclr.CCLR.sigma_left).
+        singles: list of (e,m); doubles: list of (c,d,k,l) with c<d, k<l."""
+        o, v = self.o, self.v
+        l1 = np.asarray(y1).reshape(v, o)
+        l2 = unpack_pair_axis(unpack_pair_axis(np.asarray(y2p).reshape(npair(v), npair(o)), o, 1), v, 0)
+        GL = np.einsum("abij,afij->bf", l2, self.t2, optimize=True)          # = -2 G^f_b of S-Eq. 26
+        GO = np.einsum("abij,abin->jn", l2, self.t2, optimize=True)          # =  2 G^j_n of S-Eq. 27
+        Fme, Fmi = self.Fme(), self.Fmi()
+        out1 = []
+        for (e, m) in singles:
+            s = l1[:, m] @ self.Fae_col(e) - l1[e, :] @ Fmi[m, :]                                   # S1, S2
+            s += np.einsum("ai,ai->", l1, self.Wmbej_me(m, e))                                      # S4
+            s -= 0.5 * np.einsum("bij,bij->", l2[e], self.Wmbij_m(m))                               # T1
+            s += 0.5 * np.einsum("abj,abj->", l2[:, :, m, :], self.Wabej_e(e))                      # T2
+            s += 0.5 * np.einsum("bf,bf->", GL, self.Wamef_me(m, e))                                # T3
+            s -= 0.5 * np.einsum("jn,nj->", GO, self.Wmnie_me(m, e))                                # T4
+            out1.append(s - z * l1[e, m])
+        out2 = []
+        for (c, d, k, l) in doubles:
+            s = _Pij2(lambda p, q: _Pij2(lambda r, t: l1[p, r] * Fme[t, q], k, l), c, d)            # S3
+            s += _Pij2(lambda r, t: l1[:, r] @ self.Wamef_mef(t, c, d), k, l)                       # S5
+            s -= _Pij2(lambda p, q: l1[p, :] @ (self.ooov[k, l, :, q] + self.t1.T @ self.oovv[k, l, :, q]), c, d)   # S6
+            s += _Pij2(lambda p, q: l2[p, :, k, l] @ self.Fae_col(q), c, d)                         # T5
+            s -= _Pij2(lambda r, t: l2[c, d, r, :] @ Fmi[t, :], k, l)                               # T6
+            s += 0.5 * np.einsum("ij,ij->", l2[c, d], self.Wmnij_row(k, l))                         # T7
+            s += _Pij2(lambda p, q: _Pij2(lambda r, t: np.einsum("bj,bj->", l2[p, :, r, :], self.Wmbej_me(t, q)),
+                                          k, l), c, d)                                              # T8
+            s -= 0.5 * _Pij2(lambda p, q: GL[q, :] @ self.oovv[l, k, :, p], c, d)                   # T9
+            s -= 0.5 * _Pij2(lambda r, t: GO[r, :] @ self.oovv[:, t, c, d], k, l)                   # T10
+            s += 0.5 * np.einsum("ab,ab->", l2[:, :, k, l], self.Wabef_col(c, d))                   # T11
+            out2.append(s - z * l2[c, d, k, l])
+        return out1, out2
+
+    def eta0_elements(self, singles, doubles):
+        """eta0_nu = <R|[Hbar,tau_nu]|R> = (F_me[i,a], <ij||ab>) (right-hand side of lambda A = -eta0, Eq. 13)."""
+        return ([self.Fme()[i, a] for (a, i) in singles], [self.oovv[i, j, a, b] for (a, b, i, j) in doubles])
+
+    # ---- xi^X, S-Eq. 2-3 as printed (PAPER.md:831-836) -----------------------------------------------------
+    def xi_elements(self, X, singles, doubles):
+        o = self.o
+        t1, t2 = self.t1, self.t2
+        Xoo, Xov, Xvo, Xvv = X[:o, :o], X[:o, o:], X[o:, :o], X[o:, o:]
+        Xt = Xov @ t1                                                     # [m,i]
+        tX = t1 @ Xov                                                     # [a,f]
+        out1 = [Xvo[a, i] + Xvv[a] @ t1[:, i] - t1[a] @ Xoo[:, i] - t1[a] @ Xt[:, i] + np.einsum("me,em->", Xov, t2[a, :, i, :])
+                for (a, i) in singles]
+        out2 = []
+        for (a, b, i, j) in doubles:
+            s = _Pij2(lambda p, q: Xvv[q] @ t2[p, :, i, j], a, b)
+            s -= _Pij2(lambda p, q: Xoo[:, q] @ t2[a, b, p, :], i, j)
+            s -= _Pij2(lambda p, q: Xt[:, p] @ t2[a, b, :, q], i, j)
+            s -= _Pij2(lambda p, q: tX[p] @ t2[:, q, i, j], a, b)
+            out2.append(s)
+        return out1, out2
+
+    # ---- eta^X, S-Eq. 5-6 as printed (PAPER.md:844-849), EOM term S-Eq. 7 (PAPER.md:853) ---------------------
+    def eta_elements(self, X, y1, y2p, singles, doubles, eom=False):
+        """lam1[a,i] = lambda^i_a, lam2 packed; X^p_q = X[p,q].  eom: add sum_bj lam2[ab,ij] xi1[b,j] to the singles."""
+        o, v = self.o, self.v
+        t1, t2 = self.t1, self.t2
+        lam1 = np.asarray(y1).reshape(v, o)
+        lam2 = unpack_pair_axis(unpack_pair_axis(np.asarray(y2p).reshape(npair(v), npair(o)), o, 1), v, 0)
+        Xoo, Xov, Xvv = X[:o, :o], X[:o, o:], X[o:, o:]
+        Goo = np.einsum("femn,femi->ni", t2, lam2, optimize=True)
+        Gvv = np.einsum("fenm,fanm->ea", t2, lam2, optimize=True)
+        tl = t1.T @ lam1                                                  # sum_e t1[e,m] lam1[e,i] -> [m,i]
+        lt = lam1 @ t1.T                                                  # sum_m lam1[a,m] t1[e,m] -> [a,e]
+        if eom:
+            xi1 = np.array(self.xi_elements(X, [(b, j) for b in range(v) for j in range(o)], [])[0]).reshape(v, o)
+        out1 = []
+        for (a, i) in singles:
+            s = (Xov[i, a] + Xvv[:, a] @ lam1[:, i] - Xoo[i] @ lam1[a] - Xov[:, a] @ tl[:, i] - Xov[i] @ lt[a]
+                 - 0.5 * Goo[:, i] @ Xov[:, a] - 0.5 * Gvv[:, a] @ Xov[i])
+            if eom:
+                s += np.einsum("bj,bj->", lam2[a, :, i, :], xi1)
+            out1.append(s)
+        tXov = t1 @ Xov                                                   # sum_m t1[e,m] Xov[m,b] -> [e,b]
+        Xovt = Xov @ t1                                                   # sum_e Xov[j,e] t1[e,m] -> [j,m]
+        out2 = []
+        for (a, b, i, j) in doubles:
+            s = _Pij2(lambda k, l: _Pij2(lambda p, q: lam1[p, k] * Xov[l, q], a, b), i, j)
+            s += _Pij2(lambda p, q: lam2[p, :, i, j] @ Xvv[:, q], a, b)
+            s -= _Pij2(lambda k, l: lam2[a, b, k, :] @ Xoo[l], i, j)
+            s -= _Pij2(lambda p, q: lam2[p, :, i, j] @ tXov[:, q], a, b)
+            s -= _Pij2(lambda k, l: lam2[a, b, k, :] @ Xovt[l], i, j)
+            out2.append(s)
+        return out1, out2
+
+    # ---- Omega(t) by the Gauss quadrature of the Jacobian along the ray (SURVEY 8(c) O2) ----------------------
+    def omega_elements(self, singles, doubles):
+        """CCSD residual elements: Omega(t) = Omega(0) + int_0^1 A(s t) . t ds = Omega(0) + 1/2 [A(s1 t).t + A(s2 t).t],
+        s = 1/2 -+ 1/(2 sqrt 3) (2-point Gauss-Legendre is exact: s -> A(s t).t is a cubic), Omega(0) = (f[a,i], <ab||ij>).
+        Uses sigma_elements at the two scaled amplitude sets; <ab||ij> = conj<ij||ab>."""
+        t2p = pack_pair_axes(pack_pair_axes(self.t2, 2), 0)
+        acc1 = np.array([self.fvo[a, i] for (a, i) in singles], complex)
+        acc2 = np.array([np.conj(self.oovv[i, j, a, b]) for (a, b, i, j) in doubles], complex)
+        for s in (0.5 - 0.5 / np.sqrt(3.0), 0.5 + 0.5 / np.sqrt(3.0)):
+            g1, g2 = self.with_amplitudes(s * self.t1, s * t2p).sigma_elements(self.t1, t2p, singles, doubles)
+            acc1 = acc1 + 0.5 * np.array(g1, complex).reshape(acc1.shape)
+            acc2 = acc2 + 0.5 * np.array(g2, complex).reshape(acc2.shape)
+        return list(acc1), list(acc2)

@@ -73,6 +73,15 @@ class Context:
         torch.cuda.current_stream().synchronize()
         return out
 
+    def get_intermediate_slice(self, name, offset, count):
+        """``count`` consecutive elements of the named intermediate starting at element ``offset`` (device tensor)."""
+        out = torch.empty(int(count), dtype=torch.complex128, device="cuda")
+        m = _lib.load().cclr_get_intermediate_slice(self.handle, name.encode(), int(offset), int(count), _dev(out, "out"))
+        if m < 0:
+            raise CclrError(int(m), "cclr_get_intermediate_slice(%s)" % name)
+        torch.cuda.current_stream().synchronize()
+        return out
+
     def set_max_subspace(self, dim):
         _lib.check(_lib.load().cclr_set_max_subspace(self.handle, int(dim)), "cclr_set_max_subspace")
 

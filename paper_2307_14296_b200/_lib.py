@@ -75,6 +75,7 @@ SIGNATURES = {
     "cclr_ladder": (C.c_int, [C.c_void_p, c128_p, C.c_int, c128_p]),
     "cclr_ring": (C.c_int, [C.c_void_p, c128_p, c128_p]),
     "cclr_get_intermediate": (C.c_long, [C.c_void_p, C.c_char_p, c128_p, C.c_long]),
+    "cclr_get_intermediate_slice": (C.c_long, [C.c_void_p, C.c_char_p, C.c_long, C.c_long, c128_p]),
     "cclr_kernel_launches": (C.c_ulonglong, []),
     "cclr_ctx_bytes": (C.c_size_t, [C.c_void_p]),
     "cclr_set_profiling": (C.c_int, [C.c_void_p, C.c_int]),

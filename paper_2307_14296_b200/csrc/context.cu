@@ -405,6 +405,20 @@ extern "C" long cclr_get_intermediate(cclr_ctx *ctx, const char *name, cclr_c128
   return n;
 }
 
+extern "C" long cclr_get_intermediate_slice(cclr_ctx *ctx, const char *name, long offset, long count, cclr_c128 *out) {
+  if (!ctx || !name || !out || offset < 0 || count < 0) return CCLR_EINVAL;
+  const long n = cclr_get_intermediate(ctx, name, nullptr, 0);
+  if (n < 0) return n;
+  if (offset + count > n) {
+    cclr_set_error(std::string("cclr_get_intermediate_slice: range outside ") + name, cudaSuccess);
+    return CCLR_EINVAL;
+  }
+  const c128 *src = ctx->plan->buf(ctx->plan->find(name)).ptr + offset;
+  cudaError_t e = cudaMemcpyAsync(out, src, (size_t)count * sizeof(c128), cudaMemcpyDeviceToDevice, ctx->st);
+  if (e != cudaSuccess) { cclr_set_error("cclr_get_intermediate_slice copy", e); return CCLR_ECUDA; }
+  return count;
+}
+
 extern "C" int cclr_set_max_subspace(cclr_ctx *ctx, int dim) {
   if (!ctx || dim < 0) return CCLR_EINVAL;
   ctx->max_subspace = dim;

@@ -100,3 +100,64 @@ def test_sigma_elements_with_T_match_full_oracle(o, v):
     h1, h2 = s0.sigma_elements(x1, x2, singles[:7], doubles[:9], z=z)
     k1, k2 = sampled.sigma_T0_elements(o, v, f, eri, lambda ab: vvvv[ab], x1, x2, singles[:7], doubles[:9], z=z)
     assert np.abs(np.array(h1) - np.array(k1)).max() < 1e-13 and np.abs(np.array(h2) - np.array(k2)).max() < 1e-13
+
+
+@pytest.mark.parametrize("o,v", [(3, 5), (4, 6)])
+def test_left_transform_slices_and_elements_match_full_oracle(o, v):
+    """The second family of slices (fixed e / fixed m / columns) and every element of l (A - z) against oracle.cclr.CCLR
+    (whose sigma_left is pinned against the transpose of the determinant-space Jacobian)."""
+    c, s = _small_system_with_T(o, v)
+    tol = 1e-13
+    for e in range(v):
+        assert np.abs(s.Fae_col(e) - c.Fae[:, e]).max() < tol
+        assert np.abs(s.Wabej_e(e) - c.Wabej[:, :, e, :]).max() < tol
+        assert np.abs(s.Wabef_e(e) - c.Wabef[:, :, e, :]).max() < tol
+        assert np.abs(s.Wbar_e(e) - c.Wbar[:, :, e, :]).max() < tol
+        for m in range(o):
+            assert np.abs(s.Wmbej_me(m, e) - c.Wmbej[m, :, e, :]).max() < tol
+            assert np.abs(s.Wamef_me(m, e) - c.Wamef[:, m, :, e]).max() < tol
+            assert np.abs(s.Wmnie_me(m, e) - c.Wmnie[:, m, :, e]).max() < tol
+            for f in range(e + 1, v):
+                assert np.abs(s.Wamef_mef(m, e, f) - c.Wamef[:, m, e, f]).max() < tol
+        for f in range(e + 1, v):
+            assert np.abs(s.Wabef_col(e, f) - c.Wabef[:, :, e, f]).max() < tol
+    for m in range(o):
+        assert np.abs(s.Wmbij_m(m) - c.Wmbij[m]).max() < tol
+        assert np.abs(s.Wbar_m(m) - c.Wbar[m]).max() < tol
+        for n in range(o):
+            assert np.abs(s.Wmnij_row(m, n) - c.Wmnij[m, n]).max() < tol
+    y1, y2 = synth.amplitudes(o, v, seed=8, cls1="x1", cls2="x2")
+    y1, y2 = y1[0].numpy(), y2[0].numpy()
+    z = -0.0773 + 0.0045j
+    w1, w2 = c.sigma_left(*packing.unpack_amplitudes(y1, y2, o, v), z=z)
+    singles = [(a, i) for a in range(v) for i in range(o)]
+    doubles = [(a, b, i, j) for b in range(v) for a in range(b) for j in range(o) for i in range(j)]
+    g1, g2 = s.sigma_left_elements(y1, y2, singles, doubles, z=z)
+    assert np.abs(np.array(g1) - np.array([w1[a, i] for a, i in singles])).max() < 1e-12
+    assert np.abs(np.array(g2) - np.array([w2[a, b, i, j] for a, b, i, j in doubles])).max() < 1e-12
+    e1, e2 = c.eta0()
+    h1, h2 = s.eta0_elements(singles, doubles)
+    assert np.abs(np.array(h1) - np.array([e1[a, i] for a, i in singles])).max() < tol
+    assert np.abs(np.array(h2) - np.array([e2[a, b, i, j] for a, b, i, j in doubles])).max() < tol
+
+
+@pytest.mark.parametrize("o,v", [(3, 5), (4, 6)])
+def test_xi_eta_and_omega_elements_match_full_oracle(o, v):
+    c, s = _small_system_with_T(o, v)
+    singles = [(a, i) for a in range(v) for i in range(o)]
+    doubles = [(a, b, i, j) for b in range(v) for a in range(b) for j in range(o) for i in range(j)]
+    pick = lambda w1, w2: (np.array([w1[a, i] for a, i in singles]), np.array([w2[a, b, i, j] for a, b, i, j in doubles]))
+    lam1, lam2 = synth.amplitudes(o, v, seed=9, cls1="x1", cls2="x2")
+    lam1, lam2 = lam1[0].numpy(), lam2[0].numpy()
+    L1, L2 = packing.unpack_amplitudes(lam1, lam2, o, v)
+    for X in (synth.hermitian_operator(o + v, 1, 0), synth.hermitian_operator(o + v, 1, 1, imaginary_antisymmetric=True)):
+        w1, w2 = pick(*c.xi(X))                          # = Omega[f := X, V := 0](t), the definition (pinned)
+        g1, g2 = s.xi_elements(X, singles, doubles)
+        assert np.abs(np.array(g1) - w1).max() < 1e-13 and np.abs(np.array(g2) - w2).max() < 1e-13
+        for eom in (False, True):
+            w1, w2 = pick(*(c.eta_eom(X, L1, L2) if eom else c.eta(X, L1, L2)))
+            g1, g2 = s.eta_elements(X, lam1, lam2, singles, doubles, eom=eom)
+            assert np.abs(np.array(g1) - w1).max() < 1e-12 and np.abs(np.array(g2) - w2).max() < 1e-12
+    w1, w2 = pick(*ccsd.residual(c.I, c.t1, c.t2))
+    g1, g2 = s.omega_elements(singles, doubles)
+    assert np.abs(np.array(g1) - w1).max() < 1e-12 and np.abs(np.array(g2) - w2).max() < 1e-12
