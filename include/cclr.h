@@ -107,7 +107,8 @@ int cclr_eta(cclr_ctx *ctx, const cclr_c128 *X, const cclr_c128 *lam1, const ccl
 
 /* Left equations  l (A - z_k) = -eta_r  for every right-hand side and shift: the same shared-subspace method as cclr_solve on
  * the left transform (arguments as cclr_solve).  cclr_lambda solves the ground-state multiplier equations
- * lambda A = -eta0, eta0 = (F_me[i,a], <ij||ab>) (Eq. 13): lam1 [v*o], lam2 [vv*oo] device outputs. */
+ * lambda A = -eta0, eta0 = (F_me[i,a], <ij||ab>) (Eq. 13): lam1 [v*o], lam2 [vv*oo] device outputs; a converged
+ * solution is also kept in the context, where cclr_response_ci / cclr_response_cc reuse it unless they ask for a tighter tol. */
 int cclr_solve_left(cclr_ctx *ctx, const cclr_c128 *eta1, const cclr_c128 *eta2, int nrhs, const double *omegas, int nomega,
                     double gamma, double tol, int maxiter, cclr_c128 *l1_out, cclr_c128 *l2_out, cclr_solve_info *info);
 int cclr_lambda(cclr_ctx *ctx, double tol, int maxiter, cclr_c128 *lam1, cclr_c128 *lam2, cclr_solve_info *info);

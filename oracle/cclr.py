@@ -293,19 +293,23 @@ class CCLR:
 
     def response_cc_ci(self, solve, X, Y, z, lam1, lam2):
         """CC-CI (EOM-CC) form, Eq. 16 (PAPER.md:142): g(z) = EOMeta^X.t^Y(z) - (lam.t^X(-z))(lam.xi^Y) + (X<->Y, z<->-z)."""
-        def g(zz):
-            tY = solve(*self.xi(Y), zz)
-            tX = solve(*self.xi(X), -zz)
-            return (dot(*self.eta_eom(X, lam1, lam2), *tY) - dot(lam1, lam2, *tX) * dot(lam1, lam2, *self.xi(Y))
-                    + dot(*self.eta_eom(Y, lam1, lam2), *tX) - dot(lam1, lam2, *tY) * dot(lam1, lam2, *self.xi(X)))
-        return 0.5 * (g(z) + np.conj(g(-np.conj(z))))
+        xiX, xiY = self.xi(X), self.xi(Y)
+        zc = -np.conj(z)
+        return cc_ci_from_vectors(lambda u, w: dot(*u, *w), self.eta_eom(X, lam1, lam2), self.eta_eom(Y, lam1, lam2),
+                                  (lam1, lam2), xiX, xiY, solve(*xiY, z), solve(*xiX, -z), solve(*xiY, zc), solve(*xiX, -zc))
+
+
+def cc_ci_from_vectors(d, etaX, etaY, lam, xiX, xiY, tY_z, tX_mz, tY_zc, tX_mzc):
+    """<<X;Y>>_z of Eq. 16 with the symmetriser of Eq. 17 (readings 7-8) from the vectors it is made of:
+    g(w) = EOMeta^X.t^Y(w) - (lam.t^X(-w))(lam.xi^Y) + EOMeta^Y.t^X(-w) - (lam.t^Y(w))(lam.xi^X),
+    <<X;Y>>_z = 1/2 [ g(z) + conj g(zc) ],  zc = -conj(z).  ``d(u, w)`` is the bilinear dot over unique elements; the vectors
+    may be in any representation d understands (full tensors here, packed arrays in the full-size tests)."""
+    def g(tY, tX):
+        return d(etaX, tY) - d(lam, tX) * d(lam, xiY) + d(etaY, tX) - d(lam, tY) * d(lam, xiX)
+    return 0.5 * (g(tY_z, tX_mz) + np.conj(g(tY_zc, tX_mzc)))
 
 
 def dot(a1, a2, b1, b2):
     """Bilinear (no conjugation) dot over unique elements: sum_ai a1 b1 + sum_{a<b,i<j} a2 b2 = ... + 1/4 full sum."""
     return np.sum(a1 * b1) + 0.25 * np.sum(a2 * b2)
 
-
-def vdot(a1, a2, b1, b2):
-    """Sesquilinear dot over unique elements (used for projections / norms, Eq. 29)."""
-    return np.sum(np.conj(a1) * b1) + 0.25 * np.sum(np.conj(a2) * b2)

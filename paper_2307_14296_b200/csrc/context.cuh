@@ -28,6 +28,7 @@ struct cclr_ctx {
   size_t host_stage_elems = 0;
   c128 *lambda = nullptr;         // ground-state multipliers [n1 + n2], solved on first use by cclr_response_ci
   bool have_lambda = false;
+  double lambda_tol = 0.0;        // tolerance the cached multipliers were solved to (a tighter request re-solves)
   int max_subspace = 0;           // cclr_set_max_subspace (0 = automatic)
   size_t extra_bytes = 0;         // device bytes owned outside the plan
 };

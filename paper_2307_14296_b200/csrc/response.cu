@@ -104,12 +104,13 @@ static int response_impl(cclr_ctx *ctx, const cclr_c128 *X, const cclr_c128 *Y, 
       ctx->have_lambda = false;
     }
     cclr_c128 *lam1 = (cclr_c128 *)ctx->lambda, *lam2 = (cclr_c128 *)(ctx->lambda + n1);
-    if (!ctx->have_lambda) {
+    if (!ctx->have_lambda || tol < ctx->lambda_tol) {
       cclr_solve_info li{};
       rc = cclr_lambda(ctx, tol, maxiter, lam1, lam2, &li);
       acc(li);
       if (rc != CCLR_OK && rc != CCLR_ENOTCONV) return rc;
       ctx->have_lambda = rc == CCLR_OK;
+      ctx->lambda_tol = tol;
     }
     DeviceBuf xiX, xiY, eX, eY, tX, tY;
     xiX.alloc(n, "cudaMalloc(xi X)"); xiY.alloc(n, "cudaMalloc(xi Y)"); eX.alloc(n, "cudaMalloc(eta X)"); eY.alloc(n, "cudaMalloc(eta Y)");

@@ -384,8 +384,22 @@ extern "C" int cclr_lambda(cclr_ctx *ctx, double tol, int maxiter, cclr_c128 *la
   const int i1 = ctx->plan->find("FmeT"), i2 = ctx->plan->find("eta02");
   if (i1 < 0 || i2 < 0 || !ctx->plan->buf(i1).ptr || !ctx->plan->buf(i2).ptr) return CCLR_EINVAL;
   const double zero = 0.0;
-  return solve_impl(ctx, (const cclr_c128 *)ctx->plan->buf(i1).ptr, (const cclr_c128 *)ctx->plan->buf(i2).ptr, 1, &zero, 1, 0.0,
-                    tol, maxiter, lam1, lam2, info, true);
+  const int rc = solve_impl(ctx, (const cclr_c128 *)ctx->plan->buf(i1).ptr, (const cclr_c128 *)ctx->plan->buf(i2).ptr, 1, &zero, 1,
+                            0.0, tol, maxiter, lam1, lam2, info, true);
+  // keep a copy in the context: cclr_response_ci / _cc reuse multipliers solved to a tolerance at least as tight
+  if (rc == CCLR_OK && (c128 *)lam1 != ctx->lambda) {
+    const size_t n1 = (size_t)ctx->n1, n2 = (size_t)ctx->n2;
+    if (!ctx->lambda) {
+      if (cudaMalloc(&ctx->lambda, (n1 + n2) * sizeof(c128)) != cudaSuccess) { cudaGetLastError(); ctx->lambda = nullptr; return rc; }
+      ctx->extra_bytes += (n1 + n2) * sizeof(c128);
+    }
+    cudaMemcpyAsync(ctx->lambda, lam1, n1 * sizeof(c128), cudaMemcpyDeviceToDevice, ctx->st);
+    cudaMemcpyAsync(ctx->lambda + n1, lam2, n2 * sizeof(c128), cudaMemcpyDeviceToDevice, ctx->st);
+    cudaStreamSynchronize(ctx->st);
+    ctx->have_lambda = true;
+    ctx->lambda_tol = tol;
+  }
+  return rc;
 }
 
 // Host-only entry point used by the CPU tests of the reduced-space algebra: beta_k = (G - z_k)^{-1} rhs for nz shifts.

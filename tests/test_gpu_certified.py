@@ -1,0 +1,180 @@
+"""Certified solutions and response functions at the full sizes of BASELINE.json configs 3, 4, 5.
+
+At these sizes the oracle cannot solve anything, but it can CERTIFY what the GPU solved: oracle.sampled.SampledCCLR evaluates
+single elements of Omega(t), of (A - z) t + xi, of lambda A + eta0, of xi^X and of EOM-eta^X from the packed inputs (each
+pinned against the full-tensor oracle in tests/test_oracle_sampled.py).  The chain checked here is the paper's workflow
+ end to end:
+
+  step 1  T = cclr_ccsd(...)                          certificate: sampled |Omega(T)| at the level of the convergence threshold
+  step 2  ctx = cclr_create(T, ERI_INPLACE)            (intermediates at T != 0: tests/test_gpu_fullsize.py)
+          lambda = cclr_lambda(ctx)                    certificate: sampled elements of lambda A + eta0
+          xi^X = cclr_xi, EOM-eta^X = cclr_eta         sampled elements against S-Eq. 2-3, 5-7
+  step 3  t^Y(z), t^Y(-z*), t^X(-z), t^X(z*)           certificate: sampled elements of (A - z) t + xi
+  step 4  <<X;Y>>_z (CC-CI, Eq. 16-17)                 oracle.cclr.cc_ci_from_vectors on the certified vectors (numpy dots)
+                                                       against cclr_response_ci, relative 1e-8 (north_star)
+
+Residual certificates: the solvers stop at ||r||_2 <= tol ||rhs||_2 (tol = 1e-10) over unique elements; see
+_certify_residual for what is asserted on the sampled elements.
+"""
+import numpy as np
+import pytest
+import torch
+
+import synth
+from oracle import cclr as occlr
+from oracle import sampled
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-10
+
+
+def _index_sets(o, v, rng, na, ni):
+    A = {0, 1, v - 2, v - 1}
+    while len(A) < na:
+        A.add(int(rng.integers(v)))
+    I = {0, o - 1}
+    while len(I) < ni:
+        I.add(int(rng.integers(o)))
+    return sorted(A), sorted(I)
+
+
+def _np(t):
+    return t.detach().cpu().numpy()
+
+
+def _pick(x1, x2, o, v, singles, doubles):
+    """Sampled elements of a packed device / host vector pair."""
+    P = sampled.pair_index
+    g1 = np.asarray(x1).reshape(v, o)
+    g2 = np.asarray(x2).reshape(synth.npair(v), synth.npair(o))
+    return (np.array([g1[a, i] for a, i in singles]), np.array([g2[P(a, b), P(i, j)] for a, b, i, j in doubles]))
+
+
+def _rms(x):
+    return float(np.sqrt(np.mean(np.abs(np.asarray(x)) ** 2)))
+
+
+def _certify_residual(what, r1, r2, rhs1, rhs2):
+    """r1, r2 = sampled residual elements (singles, doubles); rhs = the whole right-hand side.  The solver's criterion is
+    ||r||_2 <= TOL ||rhs||_2 over unique elements, so (rigorously) no element of a converged residual exceeds TOL ||rhs||_2,
+    and the stratified estimate n1 <|r1|^2> + n2 <|r2|^2> of ||r||^2 must come out at that level too (factor 5 for the
+    sampling noise); a wrong solution shows elements of the size of the right-hand side's, ten orders of magnitude above."""
+    n1, n2 = np.size(rhs1), np.size(rhs2)
+    norm = float(np.sqrt(np.sum(np.abs(rhs1) ** 2) + np.sum(np.abs(rhs2) ** 2)))
+    r = np.concatenate([r1, r2])
+    assert np.abs(r).max() <= 2 * TOL * norm, (what, "max sampled residual", np.abs(r).max(), TOL * norm)
+    est = float(np.sqrt(n1 * np.mean(np.abs(r1) ** 2) + n2 * np.mean(np.abs(r2) ** 2)))
+    assert est <= 5 * TOL * norm, (what, "estimated ||r||", est, TOL * norm)
+    return est / norm
+
+
+def _udot(u, w):
+    """Bilinear dot over unique elements of packed vectors (singles + a<b,i<j)."""
+    return np.sum(u[0] * w[0]) + np.sum(u[1] * w[1])
+
+
+CASES = {
+    # cfg: list of (X component, Y component, Y imaginary-antisymmetric?, omega, gamma)
+    3: [(0, 0, False, 0.0773, 0.0), (0, 1, True, 0.0773, 0.0)],      # alpha_xx(omega); optical-rotation type pair (Eq. 36)
+    4: [(0, 1, False, 0.0773, 0.0)],                                  # mixed dipole pair at the sodium D line
+    5: [(0, 0, False, 0.2, 0.0045)],                                  # damped, inside the sweep window
+}
+
+
+@pytest.mark.parametrize("cfg", [5, 3, 4])
+def test_workflow_certified_by_the_sampled_oracle(cfg):
+    import paper_2307_14296_b200 as cc
+    o, v = synth.CONFIGS[cfg]["o"], synth.CONFIGS[cfg]["v"]
+    vv, oo, n = synth.npair(v), synth.npair(o), o + v
+    scale = synth.sigma_v(v)
+    dev = "cuda"
+    eri = {k: synth.eri_class(k, o, v, seed=0, device=dev) for k in ("oooo", "ooov", "oovv", "ovvo", "ovvv", "vvvv")}
+    f = synth.fock(o, v, seed=0)
+    host = {k: _np(eri[k]) for k in ("oooo", "ooov", "oovv", "ovvo", "ovvv")}
+    row = lambda ab: synth._hermitian_matrix_rows(0, synth.CLASS_ID["vvvv"], vv, ab, ab + 1, scale, "cpu")[0].numpy()
+    rng = np.random.default_rng(200 + cfg)
+    A, I = _index_sets(o, v, rng, 5, 3)
+    singles = [(a, i) for a in A for i in I]
+    doubles = [(a, b, i, j) for bi, b in enumerate(A) for a in A[:bi] for ji, j in enumerate(I) for i in I[:ji]]
+    lsingles = [(A[0], I[0]), (A[-1], I[-1])]                         # the left transform's singles need whole slabs of W
+
+    # ---- step 1: ground state on the device, certified by sampled elements of Omega(T) ----
+    t1, t2 = synth.first_order_amplitudes(o, v, f.to(dev), eri["oovv"])
+    t1, t2, ginfo = cc.cclr_ccsd(o, v, f.to(dev), eri, t1, t2, tol=TOL, maxiter=150)
+    assert ginfo.converged == 1, ("cclr_ccsd", ginfo.iterations, ginfo.residual)
+    S = sampled.SampledCCLR(o, v, f.numpy(), host, row, _np(t1), _np(t2))
+    om1, om2 = S.omega_elements(singles, doubles)
+    om = np.concatenate([om1, om2])
+    assert np.abs(om).max() <= 2 * TOL, ("sampled |Omega(T)|", np.abs(om).max(), ginfo.residual)
+
+    # ---- step 2: intermediates in place, multipliers, xi / eta ----
+    ctx = cc.cclr_create(o, v, f.to(dev), eri, t1, t2, cc.ERI_INPLACE)
+    del eri
+    lam1, lam2, linfo = cc.cclr_lambda(ctx, tol=TOL, maxiter=200)
+    assert linfo.converged == 1
+    hl = (_np(lam1), _np(lam2))
+    L1, L2 = S.sigma_left_elements(hl[0], hl[1], lsingles, doubles)
+    e1, e2 = S.eta0_elements(lsingles, doubles)
+    eta0_all = (S.Fme().T, host["oovv"])                              # eta0 = (F_me[i,a], <ij||ab>): for the rms only
+    rl = _certify_residual("lambda A + eta0", np.array(L1) + np.array(e1), np.array(L2) + np.array(e2), *eta0_all)
+
+    report = {"omega_max": float(np.abs(om).max()), "lambda_res": rl}
+    for (cx, cy, y_imag, omega, gamma) in CASES[cfg]:
+        Xh = synth.hermitian_operator(n, 0, cx)
+        Yh = synth.hermitian_operator(n, 0, cy, imaginary_antisymmetric=y_imag)
+        X, Y = torch.from_numpy(Xh).to(dev), torch.from_numpy(Yh).to(dev)
+        vecs = {}
+        for name, Op, Oph in (("X", X, Xh), ("Y", Y, Yh)):
+            xi = cc.cclr_xi(ctx, Op)
+            eta = cc.cclr_eta(ctx, Op, lam1, lam2, eom=True)
+            hxi, heta = (_np(xi[0]), _np(xi[1])), (_np(eta[0]), _np(eta[1]))
+            w1, w2 = S.xi_elements(Oph, singles, doubles)
+            g1, g2 = _pick(*hxi, o, v, singles, doubles)
+            assert np.abs(g1 - w1).max() <= 1e-11 * _rms(hxi[0]) and np.abs(g2 - w2).max() <= 1e-11 * _rms(hxi[1]), ("xi", name)
+            w1, w2 = S.eta_elements(Oph, hl[0], hl[1], singles, doubles, eom=True)
+            g1, g2 = _pick(*heta, o, v, singles, doubles)
+            assert np.abs(g1 - w1).max() <= 1e-10 * _rms(heta[0]) and np.abs(g2 - w2).max() <= 1e-10 * _rms(heta[1]), ("EOM-eta", name)
+            vecs[name] = dict(xi=xi, hxi=hxi, heta=heta)
+        # ---- step 3: the four response solves of Eq. 16-17, each certified ----
+        z = complex(omega, gamma)
+        tY1, tY2, iY = cc.cclr_solve(ctx, vecs["Y"]["xi"][0][None], vecs["Y"]["xi"][1][None], [omega, -omega], gamma, tol=TOL)
+        tX1, tX2, iX = cc.cclr_solve(ctx, vecs["X"]["xi"][0][None], vecs["X"]["xi"][1][None], [-omega, omega], -gamma, tol=TOL)
+        assert iY.converged == 1 and iX.converged == 1
+        sols = {"tY_z": (tY1[0, 0], tY2[0, 0], z, "Y"), "tY_zc": (tY1[0, 1], tY2[0, 1], -np.conj(z), "Y"),
+                "tX_mz": (tX1[0, 0], tX2[0, 0], -z, "X"), "tX_mzc": (tX1[0, 1], tX2[0, 1], np.conj(z), "X")}
+        hs = {}
+        for key, (a1, a2, zz, op) in sols.items():
+            h = (_np(a1), _np(a2))
+            hs[key] = h
+            s1, s2 = S.sigma_elements(h[0], h[1], singles, doubles, z=zz)
+            x1, x2 = _pick(*vecs[op]["hxi"], o, v, singles, doubles)
+            report[key] = _certify_residual(key, np.array(s1) + x1, np.array(s2) + x2, *vecs[op]["hxi"])
+        # ---- step 4: the response function assembled by the oracle from the certified vectors vs the library, 1e-8 ----
+        want = occlr.cc_ci_from_vectors(_udot, vecs["X"]["heta"], vecs["Y"]["heta"], hl, vecs["X"]["hxi"], vecs["Y"]["hxi"],
+                                        hs["tY_z"], hs["tX_mz"], hs["tY_zc"], hs["tX_mzc"])
+        got, rinfo = cc.cclr_response_ci(ctx, X, Y, omega, gamma, tol=TOL)
+        assert rinfo.converged == 1
+        assert abs(got - want) <= 1e-8 * abs(want), ("<<X;Y>>", cfg, cx, cy, y_imag, omega, gamma, got, want)
+        if y_imag:   # optical-rotation type: G' = -Im <<mu; m>> (Eq. 36) is the measured quantity
+            assert abs(got.imag - want.imag) <= 1e-8 * abs(want)
+        report["<<%d;%d%s>>(%.4f%+.4fi)" % (cx, cy, "m" if y_imag else "", omega, gamma)] = [got.real, got.imag]
+        del tY1, tY2, tX1, tX2
+    print("certified cfg %d:" % cfg, report)
+
+    if cfg == 5:
+        # ---- the damped sweep (BASELINE config 5): 3 right-hand sides x 64 frequencies in one call, 4 of the 64 certified ----
+        xs = [cc.cclr_xi(ctx, torch.from_numpy(synth.hermitian_operator(n, 0, c)).to(dev)) for c in range(3)]
+        xi1 = torch.stack([x[0] for x in xs]).contiguous()
+        xi2 = torch.stack([x[1] for x in xs]).contiguous()
+        omegas = [float(w) for w in np.linspace(0.05, 0.4, 64)]
+        s1, s2, info = cc.cclr_solve(ctx, xi1, xi2, omegas, 0.0045, tol=TOL, maxiter=200)
+        assert info.converged == 1
+        for r in range(3):
+            hxi = (_np(xi1[r]), _np(xi2[r]))
+            x1, x2 = _pick(*hxi, o, v, singles, doubles)
+            for k in (0, 21, 42, 63):
+                g1, g2 = S.sigma_elements(_np(s1[r, k]), _np(s2[r, k]), singles, doubles, z=complex(omegas[k], 0.0045))
+                _certify_residual(("sweep", r, k), np.array(g1) + x1, np.array(g2) + x2, *hxi)
+    ctx.close()
+    torch.cuda.empty_cache()
