@@ -161,7 +161,7 @@ def workload_name(cfg, o, v):
 # ---------------------------------------------------------------------------------------------------------------
 # the CUDA path
 # ---------------------------------------------------------------------------------------------------------------
-def build_workload(cc, torch, synth, o, v, nvec, seed, ccsd):
+def build_workload(cc, torch, synth, o, v, nvec, seed, ccsd, gemm="3m"):
     """Synthetic inputs generated on the device, context built in place over vvvv."""
     dev = "cuda"
     eri = {k: synth.eri_class(k, o, v, seed=0, device=dev) for k in ("oooo", "ooov", "oovv", "ovvo", "ovvv", "vvvv")}
@@ -175,7 +175,7 @@ def build_workload(cc, torch, synth, o, v, nvec, seed, ccsd):
     torch.cuda.synchronize()
     l0 = cc.cclr_kernel_launches()
     t0 = time.perf_counter()
-    ctx = cc.cclr_create(o, v, f, eri, t1, t2, cc.ERI_INPLACE)
+    ctx = cc.cclr_create(o, v, f, eri, t1, t2, cc.ERI_INPLACE | (cc.GEMM_4M if gemm == "4m" else 0))
     torch.cuda.synchronize()
     create_s = time.perf_counter() - t0
     create_launches = cc.cclr_kernel_launches() - l0
@@ -206,12 +206,11 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    cc.cclr_set_gemm_mode(args.gemm == "3m")
     cfg = CONFIGS[args.config]
     o, v, nvec = cfg["o"], cfg["v"], cfg["nvec"]
     n1, n2 = o * v, npair(o) * npair(v)
     omega, gamma = 0.0773, (0.0045 if args.config in (2, 5) else 0.0)
-    ctx, keep, x1, x2, create_s, create_launches, ground = build_workload(cc, torch, synth, o, v, nvec, rank, args.ccsd)
+    ctx, keep, x1, x2, create_s, create_launches, ground = build_workload(cc, torch, synth, o, v, nvec, rank, args.ccsd, args.gemm)
     out1, out2 = torch.empty_like(x1), torch.empty_like(x2)
     flops_step = sigma_flops(o, v) * nvec
     cm = sigma_cmacs(o, v)

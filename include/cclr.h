@@ -52,6 +52,9 @@ typedef struct {
 #define CCLR_ERI_INPLACE 1u /* the context adopts eri->vvvv and dresses it in place into W_vvvv (S-Eq. 22);
                                the caller must keep the buffer alive until cclr_destroy and not read it again */
 
+#define CCLR_GEMM_4M 4u     /* every contraction of this context uses the 4M complex product (default: the large ones use 3M,
+                               see cclr_zgemm); a per-context choice, nothing process-wide */
+
 #define CCLR_SMALL_CHUNKS 2u /* testing aid: run the chunked intermediate builds with chunks of 3 indices so that small
                                inputs exercise several chunks and a ragged last one (results are unchanged) */
 
@@ -120,6 +123,15 @@ int cclr_lambda(cclr_ctx *ctx, double tol, int maxiter, cclr_c128 *lam1, cclr_c1
  * NULL) accumulates the solver statistics.  Returns CCLR_OK, or CCLR_ENOTCONV if a solve missed tol (result still written). */
 int cclr_response_ci(cclr_ctx *ctx, const cclr_c128 *X, const cclr_c128 *Y, double omega, double gamma, double tol,
                      int maxiter, cclr_c128 *result, cclr_solve_info *info);
+
+/* The whole CC-CI response tensor in one call -- steps 3 and 4 of the paper's workflow for a set of operators and
+ * frequencies: result[k][r][s] = <<X_r; X_s>>_{omegas[k] + i gamma} (HOST, [nomega][nop][nop]) for the nop DEVICE matrices
+ * X [nop][n][n].  All 2 nop nomega (4 nop nomega for gamma != 0) response systems of Eq. 16-17 share one trial space per sign of
+ * gamma (cclr_solve with nop right-hand sides and the shifts +-omegas); lambda is solved once and cached; xi, EOM-eta and every dot
+ * product run on the device.  alpha_rs(omega) = -result (reading 9); sigma_abs(omega) = 4 pi omega / c * Im mean_r alpha_rr (Eq. 22,
+ * PAPER.md:191).  omegas: HOST.  Returns CCLR_OK, or CCLR_ENOTCONV if a solve missed tol (results still written). */
+int cclr_response_ci_tensor(cclr_ctx *ctx, const cclr_c128 *X, int nop, const double *omegas, int nomega, double gamma, double tol,
+                            int maxiter, cclr_c128 *result, cclr_solve_info *info);
 
 /* x . F . y with the CC Hessian F of Table 1 (S-Eq. 8) for amplitude-shaped device vectors x, y and
  * the ground-state multipliers: F is never formed; the contraction is the exact derivative
@@ -201,19 +213,15 @@ int cclr_sigma_host(cclr_ctx *ctx, const cclr_c128 *x1, const cclr_c128 *x2, int
 /* C[M][N] = alpha * opA(A)[M][K] * opB(B) + beta * C, complex128, row-major with leading dimensions in elements.
  * A is always [M][K] (K contiguous).  b_is_kn = 0: B is [N][K] (K contiguous); 1: B is [K][N] (N contiguous).
  * conj_a / conj_b conjugate the operand elementwise.  batch > 1 repeats with element strides sa, sb, sc.
- * The complex product (4M, or 3M for large shapes: cclr_set_gemm_mode) runs on the FP64 tensor cores (DMMA) from TMA-staged
- * shared-memory tiles; N = 1 / M = 1 shapes go to bandwidth-bound matrix-vector kernels.
- * alpha, beta are host pointers to one complex number. */
+ * The complex product runs on the FP64 tensor cores (DMMA) from TMA-staged shared-memory tiles: 4M (four real products per
+ * complex one), or, when three_m != 0 and the shape is large (M >= 512, N >= 24, K >= 64: ladder, ring, W builds), the 3M
+ * product T1 = Ar Br, T2 = Ai Bi, T3 = (Ar+Ai)(Br+Bi), C = (T1 - T2) + i (T3 - T1 - T2) -- three real products instead of four.
+ * Both hold the 1e-10 parity tolerance norm-wise; 3M loses relative accuracy in a component that is much smaller than its
+ * partner (north_star: "3M only if it holds the tolerance").  N = 1 / M = 1 shapes go to
+ * bandwidth-bound matrix-vector kernels.  alpha, beta are host pointers to one complex number. */
 int cclr_zgemm(void *cuda_stream, int M, int N, int K, const cclr_c128 *alpha, const cclr_c128 *A, long lda,
                int conj_a, const cclr_c128 *B, long ldb, int b_is_kn, int conj_b, const cclr_c128 *beta,
-               cclr_c128 *C, long ldc, int batch, long sa, long sb, long sc);
-
-/* Complex-product mode of the GEMM engine (process-wide): 1 (default) = the large contractions (M >= 512, N >= 24, K >= 64:
- * ladder, ring, W builds) use the 3M product -- T1 = Ar Br, T2 = Ai Bi, T3 = (Ar+Ai)(Br+Bi), C = (T1 - T2) + i (T3 - T1 - T2):
- * three real FP64 tensor-core products per complex one instead of four; 0 = 4M everywhere.  Both hold the 1e-10 parity
- * tolerance (north_star: "3M only if it holds the tolerance"). */
-int cclr_set_gemm_mode(int three_m);
-int cclr_get_gemm_mode(void);
+               cclr_c128 *C, long ldc, int batch, long sa, long sb, long sc, int three_m);
 
 /* The particle-particle ladder alone (term T11 of S-Eq. 12):
  * out2[k][ab][ij] = sum_{e<f} W_vvvv[ab][ef] x2[k][ef][ij] for nvec vectors (no shift, no other term). */

@@ -11,7 +11,7 @@ import torch
 from . import _lib
 from ._lib import CclrError, SolveInfo  # noqa: F401
 
-__all__ = ["Context", "cclr_create", "cclr_ccsd", "cclr_response_ci", "cclr_response_cc", "cclr_xfy", "cclr_eom", "cclr_xi", "cclr_eta", "cclr_lambda", "cclr_solve_left", "cclr_sigma_left", "cclr_sigma", "cclr_solve", "cclr_property", "cclr_zgemm", "cclr_ladder",
+__all__ = ["Context", "cclr_create", "cclr_ccsd", "cclr_response_ci", "cclr_response_ci_tensor", "cclr_response_cc", "cclr_xfy", "cclr_eom", "cclr_xi", "cclr_eta", "cclr_lambda", "cclr_solve_left", "cclr_sigma_left", "cclr_sigma", "cclr_solve", "cclr_property", "cclr_zgemm", "cclr_ladder",
            "cclr_ring", "cclr_fp64_tensor_peak", "cclr_hbm_copy_peak", "CclrError"]
 
 
@@ -36,6 +36,8 @@ def _stream():
 
 
 ERI_INPLACE = 1
+SMALL_CHUNKS = 2
+GEMM_4M = 4
 
 
 class Context:
@@ -279,6 +281,23 @@ def cclr_response_ci(ctx, X, Y, omega, gamma=0.0, tol=1e-10, maxiter=200):
     return complex(res.re, res.im), info
 
 
+def cclr_response_ci_tensor(ctx, X, omegas, gamma=0.0, tol=1e-10, maxiter=200):
+    """<<X_r;X_s>>_{omega_k + i gamma} for all operator pairs and frequencies (CC-CI, Eq. 16-17) in one call.
+    X: [nop, n, n] complex128 CUDA tensor.  Returns (list [nomega][nop][nop] of complex, info)."""
+    n = ctx.o + ctx.v
+    nop = X.numel() // (n * n)
+    om = (C.c_double * len(omegas))(*[float(w) for w in omegas])
+    res = (_lib.Complex * (len(omegas) * nop * nop))()
+    info = SolveInfo()
+    rc = _lib.load().cclr_response_ci_tensor(ctx.handle, _dev(X, "X", nop * n * n), nop, om, len(omegas), float(gamma),
+                                             float(tol), int(maxiter), res, C.byref(info))
+    if rc not in (0, -4):
+        _lib.check(rc, "cclr_response_ci_tensor")
+    flat = [complex(r.re, r.im) for r in res]
+    out = [[[flat[(k * nop + r) * nop + s] for s in range(nop)] for r in range(nop)] for k in range(len(omegas))]
+    return out, info
+
+
 def cclr_xfy(o, v, fock, eri, t1, t2, lam1, lam2, x1, x2, y1, y2):
     """x . F . y (CC Hessian contraction) as an exact derivative of the left transform; returns a complex."""
     e = _eri_struct(o, v, eri)
@@ -332,8 +351,9 @@ def cclr_ring(ctx, x2, out2=None):
 
 
 def cclr_zgemm(A, B, C_out, alpha=1.0, beta=0.0, conj_a=False, conj_b=False, b_is_kn=False, M=None, N=None, K=None,
-               lda=None, ldb=None, ldc=None, batch=1, sa=0, sb=0, sc=0):
-    """C = alpha opA(A) opB(B) + beta C on 2-D (or batched 3-D) row-major tensors; see include/cclr.h."""
+               lda=None, ldb=None, ldc=None, batch=1, sa=0, sb=0, sc=0, three_m=True):
+    """C = alpha opA(A) opB(B) + beta C on 2-D (or batched 3-D) row-major tensors; see include/cclr.h.
+    three_m: large shapes use the 3M complex product (False: 4M everywhere)."""
     if M is None:
         M, K = A.shape[-2], A.shape[-1]
         N = B.shape[-1] if b_is_kn else B.shape[-2]
@@ -343,18 +363,10 @@ def cclr_zgemm(A, B, C_out, alpha=1.0, beta=0.0, conj_a=False, conj_b=False, b_i
             sa, sb, sc = A.shape[1] * A.shape[2], B.shape[1] * B.shape[2], C_out.shape[1] * C_out.shape[2]
     al, be = _lib.Complex(complex(alpha).real, complex(alpha).imag), _lib.Complex(complex(beta).real, complex(beta).imag)
     rc = _lib.load().cclr_zgemm(_stream(), M, N, K, C.byref(al), _dev(A, "A"), lda, int(conj_a), _dev(B, "B"), ldb,
-                                int(b_is_kn), int(conj_b), C.byref(be), _dev(C_out, "C"), ldc, batch, sa, sb, sc)
+                                int(b_is_kn), int(conj_b), C.byref(be), _dev(C_out, "C"), ldc, batch, sa, sb, sc,
+                                int(bool(three_m)))
     _lib.check(rc, "cclr_zgemm")
     return C_out
-
-
-def cclr_set_gemm_mode(three_m):
-    """1: large contractions use the 3M complex product (default); 0: 4M everywhere."""
-    _lib.check(_lib.load().cclr_set_gemm_mode(int(bool(three_m))), "cclr_set_gemm_mode")
-
-
-def cclr_get_gemm_mode():
-    return int(_lib.load().cclr_get_gemm_mode())
 
 
 def cclr_kernel_launches():

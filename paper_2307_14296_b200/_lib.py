@@ -48,6 +48,8 @@ SIGNATURES = {
     "cclr_eta": (C.c_int, [C.c_void_p, c128_p, c128_p, c128_p, C.c_int, c128_p, c128_p]),
     "cclr_response_ci": (C.c_int, [C.c_void_p, c128_p, c128_p, C.c_double, C.c_double, C.c_double, C.c_int,
                                    C.POINTER(Complex), C.POINTER(SolveInfo)]),
+    "cclr_response_ci_tensor": (C.c_int, [C.c_void_p, c128_p, C.c_int, C.POINTER(C.c_double), C.c_int, C.c_double, C.c_double,
+                                          C.c_int, C.POINTER(Complex), C.POINTER(SolveInfo)]),
     "cclr_xfy": (C.c_int, [C.c_int, C.c_int, c128_p, C.POINTER(EriPacked), c128_p, c128_p, c128_p, c128_p, c128_p, c128_p,
                            c128_p, c128_p, C.c_void_p, C.POINTER(Complex)]),
     "cclr_response_cc": (C.c_int, [C.c_void_p, c128_p, C.POINTER(EriPacked), c128_p, c128_p, c128_p, c128_p, C.c_double,
@@ -66,11 +68,9 @@ SIGNATURES = {
     "cclr_last_cuda_error": (C.c_int, []),
     "cclr_last_error_message": (C.c_char_p, []),
     "cclr_sigma_host": (C.c_int, [C.c_void_p, c128_p, c128_p, C.c_int, C.c_double, C.c_double, c128_p, c128_p]),
-    "cclr_set_gemm_mode": (C.c_int, [C.c_int]),
-    "cclr_get_gemm_mode": (C.c_int, []),
     "cclr_zgemm": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.POINTER(Complex), c128_p, C.c_long, C.c_int,
                              c128_p, C.c_long, C.c_int, C.c_int, C.POINTER(Complex), c128_p, C.c_long, C.c_int,
-                             C.c_long, C.c_long, C.c_long]),
+                             C.c_long, C.c_long, C.c_long, C.c_int]),
     "cclr_host_shifted_solve": (C.c_int, [C.c_int, c128_p, c128_p, C.c_int, c128_p, c128_p]),
     "cclr_ladder": (C.c_int, [C.c_void_p, c128_p, C.c_int, c128_p]),
     "cclr_ring": (C.c_int, [C.c_void_p, c128_p, c128_p]),

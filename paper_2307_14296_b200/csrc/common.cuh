@@ -33,15 +33,13 @@ void cclr_count_launch(int n = 1);
 struct ZgemmWorkspace {
   c128 *buf = nullptr;   // split-K partial sums
   size_t elems = 0;      // capacity in complex elements
+  int three_m = 1;       // complex product of the large contractions (M >= 512, N >= 24, K >= 64): 1 = 3M, 0 = 4M everywhere
 };
 // C = alpha * opA(A) * opB(B) + beta * C; see include/cclr.h (cclr_zgemm).  ws may be null (no split-K then).
 cudaError_t zgemm(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *A, long lda, bool conjA,
                   const c128 *B, long ldb, bool b_is_kn, bool conjB, c128 beta, c128 *C, long ldc, int batch = 1,
                   long sa = 0, long sb = 0, long sc = 0, const ZgemmWorkspace *ws = nullptr);
 int zgemm_num_sms();
-// 1 (default): contractions with M >= 512, N >= 24, K >= 64 use the 3M complex product; 0: 4M everywhere
-void zgemm_set_mode(int three_m);
-int zgemm_get_mode();
 
 // ---- permute.cu: generic index-permutation / pair (un)packing / antisymmetrising gather-scatter kernel ---------
 // dst(iteration index) (+)= sum_k coef_k * sign_k * [conj] src_k(slots(letters)); see plans.inc for the semantics.

@@ -149,6 +149,7 @@ extern "C" int cclr_create(int o, int v, const cclr_c128 *fock, const cclr_eri_p
     ctx->ws.elems = (size_t)8 << 20;
     check(cudaMalloc(&ctx->ws.buf, ctx->ws.elems * sizeof(c128)), "cudaMalloc(split-K workspace)");
     ctx->extra_bytes += ctx->ws.elems * sizeof(c128);
+    ctx->ws.three_m = (flags & CCLR_GEMM_4M) ? 0 : 1;
     P.set_workspace(&ctx->ws);
 
     // borrowed inputs

@@ -70,12 +70,6 @@ __global__ void copy_kernel(const double2 *__restrict__ src, double2 *__restrict
 
 }  // namespace
 
-extern "C" int cclr_set_gemm_mode(int three_m) {
-  zgemm_set_mode(three_m);
-  return CCLR_OK;
-}
-extern "C" int cclr_get_gemm_mode(void) { return zgemm_get_mode(); }
-
 extern "C" int cclr_last_cuda_error(void) { return g_last_cuda_error; }
 
 extern "C" const char *cclr_strerror(int code) {
@@ -191,7 +185,7 @@ extern "C" int cclr_hbm_copy_peak(void *cuda_stream, size_t bytes, double *gbs) 
 
 extern "C" int cclr_zgemm(void *cuda_stream, int M, int N, int K, const cclr_c128 *alpha, const cclr_c128 *A,
                           long lda, int conj_a, const cclr_c128 *B, long ldb, int b_is_kn, int conj_b,
-                          const cclr_c128 *beta, cclr_c128 *C, long ldc, int batch, long sa, long sb, long sc) {
+                          const cclr_c128 *beta, cclr_c128 *C, long ldc, int batch, long sa, long sb, long sc, int three_m) {
   if (!alpha || !beta || !C || M < 0 || N < 0 || K < 0 || batch < 1) return CCLR_EINVAL;
   if (K > 0 && (!A || !B)) return CCLR_EINVAL;
   if (lda < K || ldc < N || (b_is_kn ? ldb < N : ldb < K)) return CCLR_EINVAL;
@@ -199,10 +193,11 @@ extern "C" int cclr_zgemm(void *cuda_stream, int M, int N, int K, const cclr_c12
   // K-split workspace for this stand-alone entry point (the context keeps its own): room for 3 partial tiles per SM
   ZgemmWorkspace ws;
   ws.elems = (size_t)3 * zgemm_num_sms() * 128 * 64;
+  ws.three_m = three_m != 0;
   if (cudaMalloc(&ws.buf, ws.elems * sizeof(c128)) != cudaSuccess) { ws.buf = nullptr; ws.elems = 0; cudaGetLastError(); }
   cudaError_t e = zgemm(st, M, N, K, make_double2(alpha->re, alpha->im), (const c128 *)A, lda, conj_a != 0,
                         (const c128 *)B, ldb, b_is_kn != 0, conj_b != 0, make_double2(beta->re, beta->im), (c128 *)C,
-                        ldc, batch, sa, sb, sc, ws.buf ? &ws : nullptr);
+                        ldc, batch, sa, sb, sc, &ws);
   if (ws.buf) {
     cudaStreamSynchronize(st);
     cudaFree(ws.buf);

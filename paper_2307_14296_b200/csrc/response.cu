@@ -179,3 +179,107 @@ extern "C" int cclr_response_cc(cclr_ctx *ctx, const cclr_c128 *fock, const cclr
   const GroundState gs{fock, eri, t1, t2};
   return response_impl(ctx, X, Y, omega, gamma, tol, maxiter, result, info, &gs);
 }
+
+
+// The whole CC-CI linear response tensor <<X_r; X_s>>_{z_k}, z_k = omegas[k] + i gamma, for nop one-body operators and nomega
+// frequencies in one call: steps 3 and 4 of the paper's workflow with ONE shared trial space for all
+// operators and frequencies.  Eq. 16 + Eq. 17 (readings 7, 8) need, per operator, t(z_k) and t(-conj z_k) (shifts +-omega_k at
+// +gamma) and t(-z_k), t(conj z_k) (shifts -+omega_k at -gamma); for gamma = 0 the two sets coincide and one solve serves both.
+//   g_rs(w) = EOMeta_r . t_s(w) - (lambda . t_r(-w)) (lambda . xi_s) + EOMeta_s . t_r(-w) - (lambda . t_s(w)) (lambda . xi_r)
+//   <<X_r;X_s>>_z = 1/2 [ g_rs(z) + conj g_rs(-conj z) ]
+extern "C" int cclr_response_ci_tensor(cclr_ctx *ctx, const cclr_c128 *X, int nop, const double *omegas, int nomega, double gamma,
+                                       double tol, int maxiter, cclr_c128 *result, cclr_solve_info *info) {
+  if (!ctx || !X || !omegas || !result || nop < 1 || nomega < 1 || !(tol > 0.0) || maxiter < 1) {
+    cclr_set_error("cclr_response_ci_tensor: null pointer, nop < 1, nomega < 1, tol <= 0 or maxiter < 1", cudaSuccess);
+    return CCLR_EINVAL;
+  }
+  typedef std::complex<double> cplx;
+  cclr_solve_info total{};
+  total.converged = 1;
+  try {
+    const long n1 = ctx->n1, n2 = ctx->n2, n = n1 + n2;
+    const size_t nn = (size_t)(ctx->o + ctx->v) * (size_t)(ctx->o + ctx->v);
+    auto acc = [&](const cclr_solve_info &i) {
+      total.iterations += i.iterations; total.sigma_calls += i.sigma_calls; total.subspace = std::max(total.subspace, i.subspace);
+      total.converged = total.converged && i.converged; total.max_residual = std::max(total.max_residual, i.max_residual);
+      total.seconds += i.seconds;
+    };
+    int rc;
+    if (!ctx->lambda) {
+      check(cudaMalloc(&ctx->lambda, (size_t)n * sizeof(c128)), "cudaMalloc(lambda)");
+      ctx->extra_bytes += (size_t)n * sizeof(c128);
+      ctx->have_lambda = false;
+    }
+    cclr_c128 *lam1 = (cclr_c128 *)ctx->lambda, *lam2 = (cclr_c128 *)(ctx->lambda + n1);
+    if (!ctx->have_lambda || tol < ctx->lambda_tol) {
+      cclr_solve_info li{};
+      rc = cclr_lambda(ctx, tol, maxiter, lam1, lam2, &li);
+      acc(li);
+      if (rc != CCLR_OK && rc != CCLR_ENOTCONV) return rc;
+      ctx->have_lambda = rc == CCLR_OK;
+      ctx->lambda_tol = tol;
+    }
+    // xi and EOM-eta of every operator: [nop][n1] and [nop][n2] blocks
+    DeviceBuf XI, ETA;
+    XI.alloc((size_t)nop * n, "cudaMalloc(xi)");
+    ETA.alloc((size_t)nop * n, "cudaMalloc(eta)");
+    cclr_c128 *xi1 = (cclr_c128 *)XI.p, *xi2 = (cclr_c128 *)(XI.p + (size_t)nop * n1);
+    cclr_c128 *et1 = (cclr_c128 *)ETA.p, *et2 = (cclr_c128 *)(ETA.p + (size_t)nop * n1);
+    for (int r = 0; r < nop; ++r) {
+      if ((rc = cclr_xi(ctx, X + (size_t)r * nn, xi1 + (size_t)r * n1, xi2 + (size_t)r * n2)) != CCLR_OK) return rc;
+      if ((rc = cclr_eta(ctx, X + (size_t)r * nn, lam1, lam2, 1, et1 + (size_t)r * n1, et2 + (size_t)r * n2)) != CCLR_OK) return rc;
+    }
+    // shifts: [w_0 .. w_{K-1}, -w_0 .. -w_{K-1}] at +gamma (set P) and at -gamma (set M)
+    const int ns = 2 * nomega;
+    std::vector<double> sh(ns);
+    for (int k = 0; k < nomega; ++k) { sh[k] = omegas[k]; sh[nomega + k] = -omegas[k]; }
+    const bool two_sets = gamma != 0.0;
+    DeviceBuf TP, TM;
+    TP.alloc((size_t)nop * ns * n, "cudaMalloc(t, +gamma)");
+    cclr_c128 *tp1 = (cclr_c128 *)TP.p, *tp2 = (cclr_c128 *)(TP.p + (size_t)nop * ns * n1);
+    cclr_solve_info si{};
+    rc = cclr_solve(ctx, xi1, xi2, nop, sh.data(), ns, gamma, tol, maxiter, tp1, tp2, &si);
+    acc(si);
+    if (rc != CCLR_OK && rc != CCLR_ENOTCONV) return rc;
+    cclr_c128 *tm1 = tp1, *tm2 = tp2;
+    if (two_sets) {
+      TM.alloc((size_t)nop * ns * n, "cudaMalloc(t, -gamma)");
+      tm1 = (cclr_c128 *)TM.p; tm2 = (cclr_c128 *)(TM.p + (size_t)nop * ns * n1);
+      rc = cclr_solve(ctx, xi1, xi2, nop, sh.data(), ns, -gamma, tol, maxiter, tm1, tm2, &si);
+      acc(si);
+      if (rc != CCLR_OK && rc != CCLR_ENOTCONV) return rc;
+    }
+    // dots: E?[r][s][j] = EOMeta_r . t_s(shift j), L?[s][j] = lambda . t_s(shift j), Lx[s] = lambda . xi_s
+    const int nv = nop * ns;
+    std::vector<cclr_c128> EP((size_t)nop * nv), EM, LP(nv), LM, Lx(nop);
+    for (int r = 0; r < nop; ++r)
+      if ((rc = cclr_property(ctx, et1 + (size_t)r * n1, et2 + (size_t)r * n2, tp1, tp2, nv, EP.data() + (size_t)r * nv)) != CCLR_OK) return rc;
+    if ((rc = cclr_property(ctx, lam1, lam2, tp1, tp2, nv, LP.data())) != CCLR_OK) return rc;
+    if ((rc = cclr_property(ctx, lam1, lam2, xi1, xi2, nop, Lx.data())) != CCLR_OK) return rc;
+    if (two_sets) {
+      EM.resize((size_t)nop * nv); LM.resize(nv);
+      for (int r = 0; r < nop; ++r)
+        if ((rc = cclr_property(ctx, et1 + (size_t)r * n1, et2 + (size_t)r * n2, tm1, tm2, nv, EM.data() + (size_t)r * nv)) != CCLR_OK) return rc;
+      if ((rc = cclr_property(ctx, lam1, lam2, tm1, tm2, nv, LM.data())) != CCLR_OK) return rc;
+    }
+    auto C = [](const cclr_c128 &q) { return cplx(q.re, q.im); };
+    const std::vector<cclr_c128> &EMr = two_sets ? EM : EP, &LMr = two_sets ? LM : LP;
+    for (int k = 0; k < nomega; ++k)
+      for (int r = 0; r < nop; ++r)
+        for (int s = 0; s < nop; ++s) {
+          // shift indices: +gamma set: z_k -> k, -conj z_k -> nomega + k;  -gamma set: -z_k -> nomega + k, conj z_k -> k
+          const int jz = k, jzc = nomega + k;
+          const cplx g0 = C(EP[((size_t)r * nop + s) * ns + jz]) - C(LMr[(size_t)r * ns + jzc]) * C(Lx[s]) +
+                          C(EMr[((size_t)s * nop + r) * ns + jzc]) - C(LP[(size_t)s * ns + jz]) * C(Lx[r]);
+          const cplx g1 = C(EP[((size_t)r * nop + s) * ns + jzc]) - C(LMr[(size_t)r * ns + jz]) * C(Lx[s]) +
+                          C(EMr[((size_t)s * nop + r) * ns + jz]) - C(LP[(size_t)s * ns + jzc]) * C(Lx[r]);
+          const cplx val = 0.5 * (g0 + std::conj(g1));
+          result[((size_t)k * nop + r) * nop + s].re = val.real();
+          result[((size_t)k * nop + r) * nop + s].im = val.imag();
+        }
+  } catch (const PlanError &e) {
+    return cclr_fail(e);
+  }
+  if (info) *info = total;
+  return total.converged ? CCLR_OK : CCLR_ENOTCONV;
+}

@@ -13,7 +13,7 @@
 //         acc += a.re * (parity ? b.im :  b.re)      acc += a.im * (parity ? b.re : -b.im)
 //     where parity = "this lane feeds an imaginary output column".  conj(A)/conj(B) only flip sign bits.
 //     The C fragment of m8n8k4 (row g, real columns 2t, 2t+1) is then exactly one complex number per lane.
-//   * 3M variant (template flag M3) for the large contractions: T1 = Ar Br, T2 = Ai Bi, T3 = (Ar + Ai)(Br + Bi) on 8 x 8-complex
+//   * 3M kernel (zgemm3m_kernel) for the large contractions: T1 = Ar Br, T2 = Ai Bi, T3 = (Ar + Ai)(Br + Bi) on 8 x 8-complex
 //     DMMA tiles with three real accumulator tiles per complex tile -- 3 DMMA per 8 x 8 x 4 complex block instead of 4.
 //   * operands are staged by TMA (cp.async.bulk.tensor, FLOAT64 tensor maps over the interleaved data, boxes of
 //     128 B x rows, SWIZZLE_128B) into a STAGES-deep ring guarded by full/empty mbarriers; one producer warp,
@@ -26,6 +26,8 @@
 //     workspace + a deterministic reduce kernel; the same mechanism serves tall-K / tiny-MN contractions), and
 //     matrix-vector kernels for N = 1 / M = 1.
 #include "common.cuh"
+#include <atomic>
+#include <cmath>
 #include <mutex>
 
 namespace {
@@ -88,15 +90,30 @@ struct ZgemmArgs {
   // wave-quantisation loss of the last partial wave (and is the split-K path of tall-K / tiny-MN contractions when
   // main_tiles == 0).
   int tiles_m, tiles_n;
-  int m_fastest;       // raster order: consecutive CTAs walk tile_m (they share one B column panel) instead of tile_n
+  int group_m;         // raster: tiles are walked in groups of group_m tile rows, tile_m fastest inside a group, then tile_n
+                       // (1 = tile_n fastest over a whole tile row, tiles_m = tile_m fastest over a whole column): the CTAs
+                       // running together cover a group_m x (SMs / group_m) block of tiles and share its panels through L2
   int main_tiles, tail_splits, chunks_per_split;
   c128 *partial;
 };
 
+// tile id -> (batch, tile_m, tile_n) in the raster order of ZgemmArgs::group_m
+__host__ __device__ __forceinline__ void tile_coords(const ZgemmArgs &p, int tile, int &batch, int &tile_m, int &tile_n) {
+  const int tiles_mn = p.tiles_m * p.tiles_n;
+  batch = tile / tiles_mn;
+  const int t = tile - batch * tiles_mn;
+  const int per_group = p.group_m * p.tiles_n;
+  const int grp = t / per_group, r = t - grp * per_group;
+  const int m0 = grp * p.group_m;
+  const int gsz = p.tiles_m - m0 < p.group_m ? p.tiles_m - m0 : p.group_m;
+  tile_m = m0 + r % gsz;
+  tile_n = r / gsz;
+}
+
 // ---------------------------------------------------------------------------------------------------------------
 // kernel
 // ---------------------------------------------------------------------------------------------------------------
-template <int BM, int BN, int BK, int WM, int WN, int STAGES, bool BKN, bool M3>
+template <int BM, int BN, int BK, int WM, int WN, int STAGES, bool BKN>
 __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 32 + 128, 1)
 zgemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const ZgemmArgs p) {
   constexpr int WARPS_M = BM / WM, WARPS_N = BN / WN, NCW = WARPS_M * WARPS_N;
@@ -119,11 +136,8 @@ zgemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CU
     tile = p.main_tiles + r / p.tail_splits;
     split = r % p.tail_splits;
   }
-  const int tiles_mn = p.tiles_m * p.tiles_n;
-  const int batch = tile / tiles_mn;
-  const int trem = tile - batch * tiles_mn;
-  const int tile_m = p.m_fastest ? trem % p.tiles_m : trem / p.tiles_n;
-  const int tile_n = p.m_fastest ? trem / p.tiles_m : trem % p.tiles_n;
+  int batch, tile_m, tile_n;
+  tile_coords(p, tile, batch, tile_m, tile_n);
   const int nchunks_total = (p.K + BK - 1) / BK;
   int chunk0 = 0, nchunks = nchunks_total;
   if (is_tail) {
@@ -176,92 +190,6 @@ zgemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CU
   const int gid = lane >> 2, tig = lane & 3;
   const int rmap = ((gid & 1) << 2) | (gid >> 1);   // row permutation inside an 8-row group (bank-conflict free)
   const int wm = warp / WARPS_N, wn = warp % WARPS_N;
-  if constexpr (M3) {
-    // ===== 3M complex product (Karatsuba): T1 = Ar Br, T2 = Ai Bi, T3 = (Ar + Ai)(Br + Bi); C = (T1 - T2) + i (T3 - T1 - T2).
-    // One DMMA tile is 8 rows x 8 COMPLEX columns here (no re/im doubling of the columns), three real accumulator tiles per
-    // complex tile: 3 DMMA per 8 x 8 x 4 complex block instead of 4.  Physical column of DMMA column g is 8*g3 + rmap(g)
-    // (same permutation as the rows) so that the B fragment loads stay bank-conflict free under the 128-byte swizzle.
-    static_assert(WN % 8 == 0, "3M warp tile");
-    constexpr int NG3 = WN / 8;
-    const uint32_t sa3 = p.conjA ? 0x80000000u : 0u, sb3 = p.conjB ? 0x80000000u : 0u;
-    uint32_t a_off3[2], b_off3[2];
-#pragma unroll
-    for (int s4 = 0; s4 < 2; ++s4) {
-      const int k = 4 * s4 + tig;
-      a_off3[s4] = (uint32_t)((wm * WM + rmap) * 128 + ((k ^ rmap) << 4));
-      b_off3[s4] = !BKN ? (uint32_t)((wn * WN + rmap) * 128 + ((k ^ rmap) << 4))
-                        : (uint32_t)(((wn * WN) >> 3) * (BK * 128) + k * 128 + ((rmap ^ k) << 4));
-    }
-    double acc3[MI][NG3][3][2];
-#pragma unroll
-    for (int i = 0; i < MI; ++i)
-#pragma unroll
-      for (int g = 0; g < NG3; ++g)
-#pragma unroll
-        for (int t = 0; t < 3; ++t) acc3[i][g][t][0] = acc3[i][g][t][1] = 0.0;
-    for (int c = 0; c < nchunks; ++c) {
-      const int s = c % STAGES;
-      const uint32_t ph = (c / STAGES) & 1;
-      mbar_wait(bar_base + 8 * s, ph);
-      const uint32_t sA = smem_base + s * STAGE_BYTES, sB = sA + A_BYTES;
-#pragma unroll
-      for (int kb = 0; kb < BK / 8; ++kb) {
-#pragma unroll
-        for (int s4 = 0; s4 < 2; ++s4) {
-          double ar[MI], ai[MI], as[MI];
-#pragma unroll
-          for (int i = 0; i < MI; ++i) {
-            const double2 a = lds128(sA + kb * (BM * 128) + a_off3[s4] + i * 1024);
-            ar[i] = a.x;
-            ai[i] = flip_sign(a.y, sa3);
-            as[i] = ar[i] + ai[i];
-          }
-#pragma unroll
-          for (int g = 0; g < NG3; ++g) {
-            const uint32_t addr = !BKN ? sB + kb * (BN * 128) + g * 1024 + b_off3[s4]
-                                       : sB + g * (BK * 128) + kb * 1024 + b_off3[s4];
-            const double2 b = lds128(addr);
-            const double br = b.x, bi = flip_sign(b.y, sb3), bs = br + bi;
-#pragma unroll
-            for (int i = 0; i < MI; ++i) dmma884(acc3[i][g][0][0], acc3[i][g][0][1], ar[i], br);
-#pragma unroll
-            for (int i = 0; i < MI; ++i) dmma884(acc3[i][g][1][0], acc3[i][g][1][1], ai[i], bi);
-#pragma unroll
-            for (int i = 0; i < MI; ++i) dmma884(acc3[i][g][2][0], acc3[i][g][2][1], as[i], bs);
-          }
-        }
-      }
-      __syncwarp();
-      if (lane == 0) mbar_arrive(bar_base + 8 * (STAGES + s));
-    }
-    const bool partial3 = is_tail;
-    c128 *Cb3 = partial3 ? p.partial + ((size_t)(blockIdx.x - p.main_tiles)) * (size_t)(BM * BN) -
-                               ((size_t)tile_m * BM * BN + (size_t)tile_n * BN)
-                         : p.C + (size_t)batch * p.sc;
-    const long ldc3 = partial3 ? (long)BN : p.ldc;
-    const c128 alpha3 = partial3 ? make_double2(1.0, 0.0) : p.alpha;
-    const c128 beta3 = partial3 ? make_double2(0.0, 0.0) : p.beta;
-    const bool has_beta3 = (beta3.x != 0.0) || (beta3.y != 0.0);
-#pragma unroll
-    for (int i = 0; i < MI; ++i) {
-      const int row = tile_m * BM + wm * WM + i * 8 + rmap;
-      if (row >= p.M) continue;
-#pragma unroll
-      for (int g = 0; g < NG3; ++g) {
-#pragma unroll
-        for (int cc = 0; cc < 2; ++cc) {
-          const int col = tile_n * BN + wn * WN + g * 8 + (cc ? 4 + tig : tig);
-          if (col >= p.N) continue;
-          const double t1 = acc3[i][g][0][cc], t2 = acc3[i][g][1][cc], t3 = acc3[i][g][2][cc];
-          c128 *dst = Cb3 + (size_t)row * ldc3 + col;
-          c128 r = cmul(alpha3, make_double2(t1 - t2, t3 - t1 - t2));
-          if (has_beta3) r = cadd(r, cmul(beta3, *dst));
-          *dst = r;
-        }
-      }
-    }
-    return;
-  }
   const int par = gid & 1, nb4 = gid >> 1;
   const int wpar = ((wn * WN) >> 2) & 1;            // WN may be an odd multiple of 4: parity of the warp's first 4-row group
   // sign masks (see header comment): f1 = m1 ^ (par ? b.im : b.re), f2 = m2 ^ (par ? b.re : b.im)
@@ -361,6 +289,176 @@ zgemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CU
   }
 }
 
+
+// ---------------------------------------------------------------------------------------------------------------
+// 3M kernel: T1 = Ar Br, T2 = Ai Bi, T3 = (Ar + Ai)(Br + Bi); C = (T1 - T2) + i (T3 - T1 - T2).
+//
+// One DMMA tile is 8 rows x 8 COMPLEX columns (no re/im doubling of the columns), three real accumulator tiles per complex
+// tile: 3 DMMA per 8 x 8 x 4 complex block instead of 4.  CTA tile 128 x BN (BN = 32 | 48), 8 consumer warps (4 x 2, warp tile
+// 32 x BN/2), same TMA ring as the 4M kernel.  The sums Ar + Ai, Br + Bi are formed in registers from the LDS.128 fragments
+// (7 DADD per 36 DMMA and k-step).  Physical column of DMMA column g is 8*g3 + rmap(g) (the row permutation) so that the B
+// fragment loads stay bank-conflict free under the 128-byte swizzle.
+// What the DADDs cost, measured on B200 at config 4 (profiles/r02_3m_sum_experiments.md): ladder 206.4 ms as is, 195.2 ms with
+// the sums deleted (wrong results; the bound), 205.5 ms with the sums formed once per CTA one stage ahead through shared-memory
+// planes (11 DADD per 144 DMMA and warp, nothing in the DMMAs' dependency chain; ring 195 vs 190 ms), 359 ms with the sums
+// formed by the idle producer warps (their DADDs starve behind the consumers' DMMAs).  I.e. the cost is the DADDs' presence on
+// the FP64 datapath shared with DMMA, not their latency; only sum planes that arrive from global memory would remove it.
+// ---------------------------------------------------------------------------------------------------------------
+constexpr int Z3_BM = 128, Z3_BK = 16, Z3_STAGES = 4, Z3_WM = 32, Z3_NCW = 8;
+
+template <int BN, bool BKN>
+__global__ void __launch_bounds__(Z3_NCW * 32 + 128, 1)
+zgemm3m_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const ZgemmArgs p) {
+  constexpr int BM = Z3_BM, BK = Z3_BK, STAGES = Z3_STAGES, WM = Z3_WM, NCW = Z3_NCW;
+  constexpr int WN = BN / 2, WARPS_N = 2, MI = WM / 8, NG3 = WN / 8;
+  constexpr int A_BYTES = BM * BK * 16, B_BYTES = BN * BK * 16, STAGE_BYTES = A_BYTES + B_BYTES;
+  static_assert(BN % 16 == 0, "3M tile shape");
+
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t bar_base = smem_base + STAGES * STAGE_BYTES;   // full[STAGES], empty[STAGES], 8 B each
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  int tile = (int)blockIdx.x, split = 0;
+  const bool is_tail = tile >= p.main_tiles;
+  if (is_tail) {
+    const int r = tile - p.main_tiles;
+    tile = p.main_tiles + r / p.tail_splits;
+    split = r % p.tail_splits;
+  }
+  int batch, tile_m, tile_n;
+  tile_coords(p, tile, batch, tile_m, tile_n);
+  const int nchunks_total = (p.K + BK - 1) / BK;
+  int chunk0 = 0, nchunks = nchunks_total;
+  if (is_tail) {
+    chunk0 = split * p.chunks_per_split;
+    nchunks = nchunks_total - chunk0;
+    if (nchunks > p.chunks_per_split) nchunks = p.chunks_per_split;
+    if (nchunks < 0) nchunks = 0;
+  }
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < STAGES; ++s) {
+      mbar_init(bar_base + 8 * s, 1);                 // full: one arrive (the producer's expect_tx) + tx bytes
+      mbar_init(bar_base + 8 * (STAGES + s), NCW);    // empty: one arrive per consumer warp
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+
+  if (warp >= NCW) {
+    // ===== producer warpgroup: gives its registers to the consumers; one elected lane drives TMA =====
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
+    if (warp == NCW && lane == 0) {
+      for (int c = 0; c < nchunks; ++c) {
+        const int s = c % STAGES;
+        const uint32_t ph = (c / STAGES) & 1;
+        mbar_wait(bar_base + 8 * (STAGES + s), ph ^ 1);
+        const uint32_t full = bar_base + 8 * s;
+        mbar_expect_tx(full, STAGE_BYTES);
+        const uint32_t sA = smem_base + s * STAGE_BYTES, sB = sA + A_BYTES;
+        const int k0 = (chunk0 + c) * BK;
+#pragma unroll
+        for (int kb = 0; kb < BK / 8; ++kb)   // A boxes: [BM rows][8 complex]
+          tma_load_3d(sA + kb * (BM * 128), &tmA, 2 * (k0 + kb * 8), tile_m * BM, batch, full);
+        if (!BKN) {
+#pragma unroll
+          for (int kb = 0; kb < BK / 8; ++kb) // B boxes: [BN rows][8 complex]
+            tma_load_3d(sB + kb * (BN * 128), &tmB, 2 * (k0 + kb * 8), tile_n * BN, batch, full);
+        } else {
+#pragma unroll
+          for (int nb = 0; nb < BN / 8; ++nb) // B boxes: [BK rows][8 complex]
+            tma_load_3d(sB + nb * (BK * 128), &tmB, 2 * (tile_n * BN + nb * 8), k0, batch, full);
+        }
+      }
+    }
+    return;
+  }
+
+  // ===== consumers =====
+  asm volatile("setmaxnreg.inc.sync.aligned.u32 232;");
+  const int gid = lane >> 2, tig = lane & 3;
+  const int rmap = ((gid & 1) << 2) | (gid >> 1);   // row / column permutation inside an 8-group (bank-conflict free)
+  const int wm = warp / WARPS_N, wn = warp % WARPS_N;
+  const uint32_t sa3 = p.conjA ? 0x80000000u : 0u, sb3 = p.conjB ? 0x80000000u : 0u;
+  uint32_t a_off[2], b_off[2];
+#pragma unroll
+  for (int s4 = 0; s4 < 2; ++s4) {
+    const int k = 4 * s4 + tig;
+    a_off[s4] = (uint32_t)((wm * WM + rmap) * 128 + ((k ^ rmap) << 4));
+    b_off[s4] = !BKN ? (uint32_t)((wn * WN + rmap) * 128 + ((k ^ rmap) << 4))
+                     : (uint32_t)(((wn * WN) >> 3) * (BK * 128) + k * 128 + ((rmap ^ k) << 4));
+  }
+  double acc[MI][NG3][3][2];
+#pragma unroll
+  for (int i = 0; i < MI; ++i)
+#pragma unroll
+    for (int g = 0; g < NG3; ++g)
+#pragma unroll
+      for (int t = 0; t < 3; ++t) acc[i][g][t][0] = acc[i][g][t][1] = 0.0;
+  for (int c = 0; c < nchunks; ++c) {
+    const int s = c % STAGES;
+    const uint32_t ph = (c / STAGES) & 1;
+    mbar_wait(bar_base + 8 * s, ph);
+    const uint32_t sA = smem_base + s * STAGE_BYTES, sB = sA + A_BYTES;
+#pragma unroll
+    for (int kb = 0; kb < BK / 8; ++kb) {
+#pragma unroll
+      for (int s4 = 0; s4 < 2; ++s4) {
+        double ar[MI], ai[MI], as[MI];
+#pragma unroll
+        for (int i = 0; i < MI; ++i) {
+          const double2 a = lds128(sA + kb * (BM * 128) + a_off[s4] + i * 1024);
+          ar[i] = a.x;
+          ai[i] = flip_sign(a.y, sa3);
+          as[i] = ar[i] + ai[i];
+        }
+#pragma unroll
+        for (int g = 0; g < NG3; ++g) {
+          const uint32_t addr = !BKN ? sB + kb * (BN * 128) + g * 1024 + b_off[s4]
+                                     : sB + g * (BK * 128) + kb * 1024 + b_off[s4];
+          const double2 b = lds128(addr);
+          const double br = b.x, bi = flip_sign(b.y, sb3), bs = br + bi;
+#pragma unroll
+          for (int i = 0; i < MI; ++i) dmma884(acc[i][g][0][0], acc[i][g][0][1], ar[i], br);
+#pragma unroll
+          for (int i = 0; i < MI; ++i) dmma884(acc[i][g][1][0], acc[i][g][1][1], ai[i], bi);
+#pragma unroll
+          for (int i = 0; i < MI; ++i) dmma884(acc[i][g][2][0], acc[i][g][2][1], as[i], bs);
+        }
+      }
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(bar_base + 8 * (STAGES + s));
+  }
+  // ===== epilogue: tail tiles write raw partial sums to the workspace, main tiles write C =====
+  c128 *Cb = is_tail ? p.partial + ((size_t)(blockIdx.x - p.main_tiles)) * (size_t)(BM * BN) -
+                           ((size_t)tile_m * BM * BN + (size_t)tile_n * BN)
+                     : p.C + (size_t)batch * p.sc;
+  const long ldc = is_tail ? (long)BN : p.ldc;
+  const c128 alpha = is_tail ? make_double2(1.0, 0.0) : p.alpha;
+  const c128 beta = is_tail ? make_double2(0.0, 0.0) : p.beta;
+  const bool has_beta = (beta.x != 0.0) || (beta.y != 0.0);
+#pragma unroll
+  for (int i = 0; i < MI; ++i) {
+    const int row = tile_m * BM + wm * WM + i * 8 + rmap;
+    if (row >= p.M) continue;
+#pragma unroll
+    for (int g = 0; g < NG3; ++g) {
+#pragma unroll
+      for (int cc = 0; cc < 2; ++cc) {
+        const int col = tile_n * BN + wn * WN + g * 8 + (cc ? 4 + tig : tig);
+        if (col >= p.N) continue;
+        const double t1 = acc[i][g][0][cc], t2 = acc[i][g][1][cc], t3 = acc[i][g][2][cc];
+        c128 *dst = Cb + (size_t)row * ldc + col;
+        c128 r = cmul(alpha, make_double2(t1 - t2, t3 - t1 - t2));
+        if (has_beta) r = cadd(r, cmul(beta, *dst));
+        *dst = r;
+      }
+    }
+  }
+}
+
 // C = alpha * sum_s partial[s] + beta * C
 __global__ void zgemm_reduce_kernel(const c128 *__restrict__ partial, int splits, int M, int N, c128 alpha, c128 beta,
                                     c128 *C, long ldc, long sc, int batch) {
@@ -414,17 +512,27 @@ bool make_map(CUtensorMap *tm, const c128 *base, long inner_complex, long rows, 
   return r == CUDA_SUCCESS;
 }
 
-template <int BM, int BN, int BK, int WM, int WN, int STAGES, bool BKN, bool M3 = false>
+// cudaFuncSetAttribute is per device: remember which devices a kernel instantiation has been configured on
+inline cudaError_t configure_smem(const void *kern, int smem, unsigned long long &done_mask) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 64 && (done_mask >> dev) & 1ull) return cudaSuccess;
+  e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  if (e == cudaSuccess && dev < 64) done_mask |= 1ull << dev;
+  return e;
+}
+
+template <int BM, int BN, int BK, int WM, int WN, int STAGES, bool BKN>
 cudaError_t launch(cudaStream_t st, const CUtensorMap &tmA, const CUtensorMap &tmB, const ZgemmArgs &args, int ctas) {
   constexpr int threads = (BM / WM) * (BN / WN) * 32 + 128;
   constexpr int smem = STAGES * (BM + BN) * BK * 16 + 2 * STAGES * 8 + 1024;
-  auto kern = zgemm_kernel<BM, BN, BK, WM, WN, STAGES, BKN, M3>;
-  static bool configured = false;
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (e != cudaSuccess) return e;
-    configured = true;
-  }
+  auto kern = zgemm_kernel<BM, BN, BK, WM, WN, STAGES, BKN>;
+  static std::atomic<unsigned long long> configured{0};
+  unsigned long long mask = configured.load();
+  const cudaError_t e = configure_smem((const void *)kern, smem, mask);
+  if (e != cudaSuccess) return e;
+  configured.fetch_or(mask);
   kern<<<ctas, threads, smem, st>>>(tmA, tmB, args);
   cclr_count_launch();
   return cudaGetLastError();
@@ -441,21 +549,26 @@ cudaError_t launch_ng(cudaStream_t st, const CUtensorMap &tmA, const CUtensorMap
             : launch<64, 8 * NG, ZG_BK, 16, 4 * NG, ZG_STAGES, false>(st, tmA, tmB, args, ctas);
 }
 
-// 3M variant: BN = 16 * NG3 (two warps of NG3 eight-column DMMA groups), 128-row tiles
-template <int NG3>
-cudaError_t launch_3m(cudaStream_t st, const CUtensorMap &tmA, const CUtensorMap &tmB, const ZgemmArgs &args, int ctas, bool kn) {
-  return kn ? launch<128, 16 * NG3, ZG_BK, 32, 8 * NG3, ZG_STAGES, true, true>(st, tmA, tmB, args, ctas)
-            : launch<128, 16 * NG3, ZG_BK, 32, 8 * NG3, ZG_STAGES, false, true>(st, tmA, tmB, args, ctas);
+// 3M kernel: 128 x BN tiles, BN = 32 | 48
+template <int BN, bool BKN>
+cudaError_t launch_3m(cudaStream_t st, const CUtensorMap &tmA, const CUtensorMap &tmB, const ZgemmArgs &args, int ctas) {
+  constexpr int threads = Z3_NCW * 32 + 128;
+  constexpr int smem = Z3_STAGES * (Z3_BM + BN) * Z3_BK * 16 + 2 * Z3_STAGES * 8 + 1024;
+  auto kern = zgemm3m_kernel<BN, BKN>;
+  static std::atomic<unsigned long long> configured{0};
+  unsigned long long mask = configured.load();
+  const cudaError_t e = configure_smem((const void *)kern, smem, mask);
+  if (e != cudaSuccess) return e;
+  configured.fetch_or(mask);
+  kern<<<ctas, threads, smem, st>>>(tmA, tmB, args);
+  cclr_count_launch();
+  return cudaGetLastError();
 }
 
 // C tile = alpha * sum_splits partial + beta * C for the K-split tail tiles
 __global__ void __launch_bounds__(256) zgemm_tail_reduce_kernel(const ZgemmArgs p, int BM, int BN) {
-  const int t = p.main_tiles + (int)blockIdx.x;                 // tile id
-  const int tiles_mn = p.tiles_m * p.tiles_n;
-  const int batch = t / tiles_mn;
-  const int trem = t - batch * tiles_mn;
-  const int tile_m = p.m_fastest ? trem % p.tiles_m : trem / p.tiles_n;
-  const int tile_n = p.m_fastest ? trem / p.tiles_m : trem % p.tiles_n;
+  int batch, tile_m, tile_n;
+  tile_coords(p, p.main_tiles + (int)blockIdx.x, batch, tile_m, tile_n);
   const c128 *part = p.partial + (size_t)blockIdx.x * p.tail_splits * (size_t)(BM * BN);
   const bool has_beta = p.beta.x != 0.0 || p.beta.y != 0.0;
   for (int e = threadIdx.x; e < BM * BN; e += blockDim.x) {
@@ -550,19 +663,34 @@ __global__ void __launch_bounds__(256) zgemv_kernel(int M, int K, c128 alpha, co
 
 }  // namespace
 
-static int g_gemm_3m = 1;   // 1: large contractions use the 3M complex product (zgemm_set_mode)
-void zgemm_set_mode(int three_m) { g_gemm_3m = three_m ? 1 : 0; }
-int zgemm_get_mode() { return g_gemm_3m; }
-
 int zgemm_num_sms() {
-  static int n = 0;
-  if (!n) {
-    int dev = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
-    if (n <= 0) n = 148;
-  }
+  static std::atomic<int> cache[64];   // per device ordinal (zero-initialised)
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return 148;
+  if (dev >= 0 && dev < 64 && cache[dev].load() > 0) return cache[dev].load();
+  int n = 0;
+  cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
+  if (n <= 0) n = 148;
+  if (dev >= 0 && dev < 64) cache[dev].store(n);
   return n;
+}
+
+// Raster (ZgemmArgs::group_m): the CTAs of one wave cover a block of rows x cols tiles and stream rows A panels and cols B
+// panels in k-lockstep; pick the group height that minimises the panel bytes per wave (BM rows + BN cols, per unit of K).
+static int pick_group_m(int tiles_m, int tiles_n, int BM, int BN, int sms) {
+  int best_g = 1;
+  double best = -1.0;
+  for (int g = 1; g <= tiles_m; ++g) {
+    int cols = (sms + g - 1) / g;
+    if (cols > tiles_n) cols = tiles_n;
+    double rows = (double)sms / cols;
+    if (rows < g) rows = g;
+    if (rows > tiles_m) rows = tiles_m;
+    const double bytes = rows * BM + (double)cols * BN;
+    if (best < 0.0 || bytes < best * 0.999) { best = bytes; best_g = g; }
+    if (g >= sms) break;
+  }
+  return best_g;
 }
 
 cudaError_t zgemm(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *A, long lda, bool conjA,
@@ -575,7 +703,7 @@ cudaError_t zgemm(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *
   const long pad128 = (M + 127L) / 128 * 128, pad64 = (M + 63L) / 64 * 64;
   // 3M complex product (3 real DMMA products per complex one instead of 4) for the large contractions; the 4M kernel keeps
   // the small and skinny ones, where tile padding, not the DMMA count, is the cost
-  const bool use3m = g_gemm_3m && M >= 512 && N >= 24 && K >= 64;
+  const bool use3m = (!ws || ws->three_m) && M >= 512 && N >= 24 && K >= 64;
   const int BM = use3m ? 128 : ((pad64 * 10 <= pad128 * 9) ? 64 : 128);
   if (batch > 1 && (sa == 0 || sb == 0)) {   // a shared operand has no batch stride a tensor map could carry: one launch per batch
     for (int b = 0; b < batch; ++b) {
@@ -640,7 +768,7 @@ cudaError_t zgemm(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *
   args.conjA = conjA; args.conjB = conjB;
   args.tiles_m = (M + BM - 1) / BM;
   args.tiles_n = (N + BN - 1) / BN;
-  args.m_fastest = N > M;   // the larger operand's panels are the ones shared through L2 by concurrently running CTAs
+  args.group_m = pick_group_m(args.tiles_m, args.tiles_n, BM, BN, sms);
   const long tiles = (long)args.tiles_m * args.tiles_n * batch;
   if (tiles > 0x7fffffffL / 2) return cudaErrorInvalidValue;
   const int nchunks = (K + BK - 1) / BK;
@@ -681,7 +809,8 @@ cudaError_t zgemm(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *
   }
   cudaError_t e;
   if (use3m) {
-    e = NG3 == 2 ? launch_3m<2>(st, tmA, tmB, args, ctas, b_is_kn) : launch_3m<3>(st, tmA, tmB, args, ctas, b_is_kn);
+    if (NG3 == 2) e = b_is_kn ? launch_3m<32, true>(st, tmA, tmB, args, ctas) : launch_3m<32, false>(st, tmA, tmB, args, ctas);
+    else e = b_is_kn ? launch_3m<48, true>(st, tmA, tmB, args, ctas) : launch_3m<48, false>(st, tmA, tmB, args, ctas);
   } else
   switch (NG) {
     case 4: e = launch_ng<4>(st, tmA, tmB, args, ctas, b_is_kn, BM); break;

@@ -132,3 +132,22 @@ def test_cc_cc_response_function_end_to_end(cfg1, z):
                                              complex(z).imag, tol=1e-11)
         assert info.converged == 1
         assert abs(got - want) <= 1e-8 * abs(want), (z, got, want)
+
+
+@pytest.mark.parametrize("gamma", [0.0, 0.0045])
+def test_response_tensor_in_one_call_matches_the_oracle_and_the_pairwise_entry_point(cfg1, gamma):
+    """cclr_response_ci_tensor (all operator pairs and frequencies from two shared-subspace solves) against the all-oracle
+    CC-CI value of Eq. 16-17 (dense solves) for every pair incl. the imaginary-antisymmetric operator, 1e-8."""
+    s = cfg1
+    cc, c, A = s["cc"], s["c"], s["A"]
+    ops = s["ops"]
+    omegas = [0.0, 0.0773]
+    X = torch.from_numpy(np.stack(ops)).cuda().contiguous()
+    got, info = cc.cclr_response_ci_tensor(s["ctx"], X, omegas, gamma, tol=1e-11, maxiter=300)
+    assert info.converged == 1
+    solve = lambda x1, x2, z: c.solve_dense(A, x1, x2, z)
+    for k, w in enumerate(omegas):
+        for r in range(len(ops)):
+            for q in (r, (r + 1) % len(ops)):
+                want = c.response_cc_ci(solve, ops[r], ops[q], complex(w, gamma), *s["lam"])
+                assert abs(got[k][r][q] - want) <= 1e-8 * max(abs(want), 1e-4), (k, r, q, got[k][r][q], want)
