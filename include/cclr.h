@@ -257,6 +257,17 @@ int cclr_sigma_op_count(const cclr_ctx *ctx);
 const char *cclr_sigma_op_text(const cclr_ctx *ctx, int k);
 int cclr_last_sigma_op_ms(const cclr_ctx *ctx, double *ms, int capacity);
 
+/* The solver's multi-row update (steps 4-5 of PAPER.md:960-967): Y[r][i] = X[r][i] + sum_{j<m} coef[r][j] V[j][i] for R <= 8 rows
+ * in ONE pass over the m vectors V (all DEVICE; leading dimensions in elements; X may be NULL = 0; ldx = 0 shares one X row),
+ * optionally with nrm2[r] = ||Y[r]||_2^2 (DEVICE doubles, or NULL) and the preconditioned rows P[r][i] = Y[r][i] / (z[r] - D[i])
+ * (D = the context's orbital-energy denominators, z DEVICE [R]; P NULL to skip; then n <= v*o + vv*oo). */
+int cclr_vec_block_lincomb(cclr_ctx *ctx, int R, cclr_c128 *Y, long ldy, const cclr_c128 *X, long ldx, const cclr_c128 *coef,
+                           const cclr_c128 *V, long ldv, int m, long n, double *nrm2, const cclr_c128 *z, cclr_c128 *P, long ldp);
+/* Sesquilinear dot block out[ia*nb + ib] = sum_i conj(A[ia][i]) B[ib][i] (Eq. 29) through the path the solver
+ * uses (one split-K DMMA GEMM for blocks, the chunked reduction kernel for single rows): A [na][n], B [nb][n] DEVICE dense rows
+ * (ld must equal n), out HOST [na*nb]. */
+int cclr_vec_dots(cclr_ctx *ctx, const cclr_c128 *A, int na, const cclr_c128 *B, int nb, long n, long ld, cclr_c128 *out);
+
 /* HOST-only: the reduced-space step of cclr_solve: beta[k] = (G - z[k] I)^{-1} rhs for nz shifts sharing one
  * L x L row-major matrix G, through one Hessenberg reduction.  All pointers are host pointers; beta is [nz][L]. */
 int cclr_host_shifted_solve(int L, const cclr_c128 *G, const cclr_c128 *rhs, int nz, const cclr_c128 *z, cclr_c128 *beta);

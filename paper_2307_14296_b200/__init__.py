@@ -369,6 +369,29 @@ def cclr_zgemm(A, B, C_out, alpha=1.0, beta=0.0, conj_a=False, conj_b=False, b_i
     return C_out
 
 
+def cclr_vec_block_lincomb(ctx, Y, X, coef, V, nrm2=None, z=None, P=None):
+    """Y[r] = X[r] + sum_j coef[r][j] V[j] for R <= 8 rows in one pass (Y [R, n], X [R, n] / [n] shared / None, coef [R, m],
+    V [m, n]); optional nrm2 (float64 CUDA tensor [R]) and P [R, n] = Y / (z - D) with z [R] complex."""
+    R, n = Y.shape
+    m = V.shape[0]
+    ldx = 0 if X is None or X.dim() == 1 else X.shape[1]
+    null = C.c_void_p(None)
+    rc = _lib.load().cclr_vec_block_lincomb(ctx.handle, R, _dev(Y, "Y"), n, null if X is None else _dev(X, "X"), ldx, _dev(coef, "coef", R * m),
+                                            _dev(V, "V"), V.shape[1], m, n, null if nrm2 is None else C.c_void_p(nrm2.data_ptr()),
+                                            null if z is None else _dev(z, "z"), null if P is None else _dev(P, "P"), n)
+    _lib.check(rc, "cclr_vec_block_lincomb")
+    return Y
+
+
+def cclr_vec_dots(ctx, A, B):
+    """out[ia][ib] = <A_ia | B_ib> (sesquilinear) for A [na, n], B [nb, n]; returns a list of lists of complex."""
+    na, n = A.shape
+    nb = B.shape[0]
+    res = (_lib.Complex * (na * nb))()
+    _lib.check(_lib.load().cclr_vec_dots(ctx.handle, _dev(A, "A"), na, _dev(B, "B"), nb, n, n, res), "cclr_vec_dots")
+    return [[complex(res[i * nb + j].re, res[i * nb + j].im) for j in range(nb)] for i in range(na)]
+
+
 def cclr_kernel_launches():
     return int(_lib.load().cclr_kernel_launches())
 

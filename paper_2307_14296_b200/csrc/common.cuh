@@ -81,6 +81,14 @@ cudaError_t multi_dot(cudaStream_t st, const c128 *A, long lda, int na, const c1
                       bool conjA, bool diag, c128 *partial, c128 *out);
 // y[i] = beta * y[i] + sum_{j<m} coef[j] * V[j*ldv + i]   (coef: DEVICE array of m complex numbers)
 cudaError_t lincomb(cudaStream_t st, c128 *y, c128 beta, const c128 *coef, const c128 *V, long ldv, int m, long n);
+// Y[r][i] = xs * X[r][i] + sum_j coef[r][j] V0[j][i] + sum_j coef[r][m0+j] V1[j][i] for R <= BLOCK_LINCOMB_MAX rows in one pass
+// over the m0 + m1 vectors, with optional fused squared norms (nrm2: device [R]; nrm_scratch: block_lincomb_grid(n) * R doubles)
+// and optional preconditioned output P[r][i] = Y[r][i] / (z[r] - D[i]) (z: device [R]); see vecops.cu
+constexpr int BLOCK_LINCOMB_MAX = 8;
+int block_lincomb_grid(long n);
+cudaError_t block_lincomb(cudaStream_t st, int R, c128 *Y, long ldy, const c128 *X, long ldx, c128 xs, const c128 *coef, int ldc,
+                          const c128 *V0, long ldv0, int m0, const c128 *V1, long ldv1, int m1, long n, double *nrm2,
+                          double *nrm_scratch, const double *D, const c128 *z, c128 *P, long ldp);
 // y[i] = alpha * x[i] / (z - D[i])      (orbital-energy preconditioner)
 cudaError_t precondition(cudaStream_t st, c128 *y, const c128 *x, const double *D, c128 z, c128 alpha, long n);
 cudaError_t scale_vec(cudaStream_t st, c128 *y, c128 alpha, long n);

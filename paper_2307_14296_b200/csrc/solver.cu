@@ -24,7 +24,11 @@ using subspace::DeviceBuf;
 
 struct Solver : subspace::Space {
   int rcap = 0;
-  DeviceBuf XI, R, tmp;
+  DeviceBuf XI, R, tmp, PC, NV, zdev;
+  double *nrm = nullptr, *nrm_scratch = nullptr;   // fused residual norms (device)
+  ~Solver() { if (nrm) cudaFree(nrm); if (nrm_scratch) cudaFree(nrm_scratch); }
+  c128 *pc(int i) { return PC.p + (size_t)i * n; }
+  c128 *nv(int i) { return NV.p + (size_t)i * n; }
   std::vector<cplx> c;        // maxdim x nrhs: c[j][r] = b_j^H xi_r
   int nrhs = 0;
 
@@ -71,7 +75,8 @@ static int solve_impl(cclr_ctx *ctx, const cclr_c128 *xi1, const cclr_c128 *xi2,
     for (;; rhs_block = (rhs_block + 1) / 2) {
       const int nsys_b = rhs_block * nomega;
       rcap = std::min(nsys_b, 256);
-      double left = budget - (double)(rhs_block + rcap + 1) * vec_b;
+      // right-hand sides, residual block, tmp, preconditioned residuals (<= 15 rows) and the block of new trial vectors
+      double left = budget - (double)(rhs_block + rcap + 1 + std::min(rcap, 15) + 4 * rhs_block) * vec_b;
       while (left < 8 * vec_b && rcap > 1) {            // shrink the residual block before the subspace
         left += (rcap - rcap / 2) * vec_b;
         rcap /= 2;
@@ -97,7 +102,13 @@ static int solve_impl(cclr_ctx *ctx, const cclr_c128 *xi1, const cclr_c128 *xi2,
       S.XI.alloc((size_t)nr * n, "cudaMalloc(xi)");
       S.R.alloc((size_t)rcap * n, "cudaMalloc(residual block)");
       S.tmp.alloc((size_t)n, "cudaMalloc(tmp)");
-      S.coef.alloc((size_t)std::max(maxdim, 1) * std::max(rcap, 1) * 2, "cudaMalloc(coefficients)");
+      const int pc_rows = std::min(rcap, 15), per_rhs_max = nomega >= 16 ? 4 : std::min(nomega, 2);
+      S.PC.alloc((size_t)pc_rows * n, "cudaMalloc(preconditioned residuals)");
+      S.NV.alloc((size_t)per_rhs_max * nr * n, "cudaMalloc(new trial vectors)");
+      S.zdev.alloc(BLOCK_LINCOMB_MAX, "cudaMalloc(shifts)");
+      check(cudaMalloc(&S.nrm, (size_t)std::max(rcap, 1) * sizeof(double)), "cudaMalloc(norms)");
+      check(cudaMalloc(&S.nrm_scratch, (size_t)block_lincomb_grid(n) * BLOCK_LINCOMB_MAX * sizeof(double)), "cudaMalloc(norm scratch)");
+      S.coef.alloc((size_t)std::max(maxdim, 1) * std::max(rcap, BLOCK_LINCOMB_MAX) * 2, "cudaMalloc(coefficients)");
       S.G.assign((size_t)maxdim * maxdim, cplx(0.0));
       S.c.assign((size_t)maxdim * nr, cplx(0.0));
 
@@ -116,6 +127,29 @@ static int solve_impl(cclr_ctx *ctx, const cclr_c128 *xi1, const cclr_c128 *xi2,
       std::vector<double> relres(nsys, 0.0);
       auto out1 = [&](int r, int k) { return (c128 *)t1_out + ((size_t)(r0 + r) * nomega + k) * n1; };
       auto out2 = [&](int r, int k) { return (c128 *)t2_out + ((size_t)(r0 + r) * nomega + k) * n2; };
+      small_dense::Hessenberg hess;
+      std::vector<cplx> beta((size_t)nsys * maxdim, cplx(0.0));
+      // t = sum_j beta_j b_j (step 5) for the listed systems; runs of consecutive shifts of one right-hand side
+      // are contiguous rows of the output arrays and are written by one multi-row pass over the basis
+      auto write_solutions = [&](const std::vector<int> &list, int Lb) {
+        for (size_t p0 = 0; p0 < list.size();) {
+          int R = 1;
+          while (p0 + R < list.size() && R < BLOCK_LINCOMB_MAX && list[p0 + R] == list[p0] + R &&
+                 list[p0 + R] / nomega == list[p0] / nomega)
+            ++R;
+          std::vector<cplx> co((size_t)R * Lb);
+          for (int i = 0; i < R; ++i)
+            for (int j = 0; j < Lb; ++j) co[(size_t)i * Lb + j] = beta[(size_t)list[p0 + i] * maxdim + j];
+          S.upload(co, S.coef.p);
+          const int r = list[p0] / nomega, k = list[p0] % nomega;
+          check(block_lincomb(st, R, out1(r, k), n1, nullptr, 0, make_double2(0.0, 0.0), S.coef.p, Lb, S.Bm.p, n, Lb, nullptr, 0, 0,
+                              n1, nullptr, nullptr, nullptr, nullptr, nullptr, 0), "block_lincomb(t1)");
+          check(block_lincomb(st, R, out2(r, k), n2, nullptr, 0, make_double2(0.0, 0.0), S.coef.p, Lb, S.Bm.p + n1, n, Lb, nullptr, 0, 0,
+                              n2, nullptr, nullptr, nullptr, nullptr, nullptr, 0), "block_lincomb(t2)");
+          check(cudaStreamSynchronize(st), "sync");
+          p0 += R;
+        }
+      };
       for (int r = 0; r < nr; ++r) {
         if (norm_xi[r] == 0.0) {
           for (int k = 0; k < nomega; ++k) {
@@ -135,8 +169,6 @@ static int solve_impl(cclr_ctx *ctx, const cclr_c128 *xi1, const cclr_c128 *xi2,
       int L0 = 0;
       int iter = 0;
       bool all_done = std::all_of(done.begin(), done.end(), [](int d) { return d != 0; });
-      small_dense::Hessenberg hess;
-      std::vector<cplx> beta((size_t)nsys * maxdim, cplx(0.0));
 
       while (!all_done) {
         ++iter;
@@ -160,14 +192,50 @@ static int solve_impl(cclr_ctx *ctx, const cclr_c128 *xi1, const cclr_c128 *xi2,
             for (int j = 0; j < L; ++j) beta[(size_t)sidx * maxdim + j] = 0.0;
         }
         // ---- step 4: residuals r = xi + sum_j beta_j (sigma_j - z b_j), in blocks of rcap systems ----
+        // fewer than 16 systems: multi-row bandwidth kernel, groups of <= 8 systems of one right-hand side, with the norm and
+        // the preconditioned residual r / (z - D) produced in the same pass over the 2L subspace vectors;
+        // more: the residual block as two DMMA GEMMs, norms by the reduction kernel
         const bool single_block = (int)active.size() <= rcap;
+        bool have_pc = false;               // preconditioned residuals of the (single) block are in PC
         for (size_t a0 = 0; a0 < active.size(); a0 += rcap) {
           const int nb = (int)std::min<size_t>(rcap, active.size() - a0);
+          if (nb < 16) {
+            const bool want_pc = single_block && nb <= pc_rows;
+            for (int g0 = 0; g0 < nb;) {
+              const int r = active[a0 + g0] / nomega;
+              int R = 1;
+              while (g0 + R < nb && R < BLOCK_LINCOMB_MAX && active[a0 + g0 + R] / nomega == r) ++R;
+              std::vector<cplx> co((size_t)R * 2 * L), zz(BLOCK_LINCOMB_MAX, cplx(0.0));
+              for (int i = 0; i < R; ++i) {
+                const int sidx = active[a0 + g0 + i];
+                zz[i] = z[sidx % nomega];
+                for (int j = 0; j < L; ++j) {
+                  co[(size_t)i * 2 * L + j] = beta[(size_t)sidx * maxdim + j];
+                  co[(size_t)i * 2 * L + L + j] = -zz[i] * beta[(size_t)sidx * maxdim + j];
+                }
+              }
+              S.upload(zz, S.zdev.p);
+              S.upload(co, S.coef.p);
+              check(block_lincomb(st, R, S.r(g0), n, S.xi(r), 0, make_double2(1.0, 0.0), S.coef.p, 2 * L, S.Sm.p, n, L, S.Bm.p, n, L,
+                                  n, S.nrm + g0, S.nrm_scratch, want_pc ? ctx->D : nullptr, S.zdev.p, want_pc ? S.pc(g0) : nullptr, n),
+                    "block_lincomb(residual)");
+              g0 += R;
+            }
+            std::vector<double> nr2(nb);
+            check(cudaMemcpyAsync(nr2.data(), S.nrm, (size_t)nb * sizeof(double), cudaMemcpyDeviceToHost, st), "D2H norms");
+            check(cudaStreamSynchronize(st), "sync norms");
+            for (int i = 0; i < nb; ++i) {
+              const int sidx = active[a0 + i];
+              relres[sidx] = std::sqrt(std::max(0.0, nr2[i])) / norm_xi[sidx / nomega];
+            }
+            have_pc = want_pc;
+            continue;
+          }
           for (int i = 0; i < nb; ++i) {
             const int r = active[a0 + i] / nomega;
             check(cudaMemcpyAsync(S.r(i), S.xi(r), (size_t)n * sizeof(c128), cudaMemcpyDeviceToDevice, st), "copy xi");
           }
-          if (nb >= 16) {
+          {
             std::vector<cplx> co((size_t)2 * nb * L);
             for (int i = 0; i < nb; ++i) {
               const int sidx = active[a0 + i];
@@ -179,18 +247,8 @@ static int solve_impl(cclr_ctx *ctx, const cclr_c128 *xi1, const cclr_c128 *xi2,
             }
             S.upload(co, S.coef.p);
             const c128 one = make_double2(1.0, 0.0);
-            check(zgemm(st, nb, (int)n, L, one, S.coef.p, L, false, S.Sm.p, n, true, false, one, S.R.p, n), "zgemm(residual sigma)");
-            check(zgemm(st, nb, (int)n, L, one, S.coef.p + (size_t)nb * L, L, false, S.Bm.p, n, true, false, one, S.R.p, n), "zgemm(residual b)");
-          } else {
-            for (int i = 0; i < nb; ++i) {
-              const int sidx = active[a0 + i];
-              const cplx zz = z[sidx % nomega];
-              std::vector<cplx> co(L);
-              for (int j = 0; j < L; ++j) co[j] = beta[(size_t)sidx * maxdim + j];
-              S.add_combination(S.r(i), make_double2(1.0, 0.0), co, S.Sm.p, L, n, n);
-              for (int j = 0; j < L; ++j) co[j] = -zz * beta[(size_t)sidx * maxdim + j];
-              S.add_combination(S.r(i), make_double2(1.0, 0.0), co, S.Bm.p, L, n, n);
-            }
+            check(zgemm(st, nb, (int)n, L, one, S.coef.p, L, false, S.Sm.p, n, true, false, one, S.R.p, n, 1, 0, 0, 0, &ctx->ws), "zgemm(residual sigma)");
+            check(zgemm(st, nb, (int)n, L, one, S.coef.p + (size_t)nb * L, L, false, S.Bm.p, n, true, false, one, S.R.p, n, 1, 0, 0, 0, &ctx->ws), "zgemm(residual b)");
           }
           std::vector<cplx> nr2 = S.dots(S.R.p, nb, S.R.p, nb, true);
           for (int i = 0; i < nb; ++i) {
@@ -200,17 +258,13 @@ static int solve_impl(cclr_ctx *ctx, const cclr_c128 *xi1, const cclr_c128 *xi2,
         }
         // ---- convergence and step 5: solutions t = sum_j beta_j b_j of the converged systems ----
         const bool last = iter >= maxiter;
-        for (int sidx : active) {
-          if (relres[sidx] <= tol || last) {
-            const int r = sidx / nomega, k = sidx % nomega;
-            std::vector<cplx> co(L);
-            for (int j = 0; j < L; ++j) co[j] = beta[(size_t)sidx * maxdim + j];
-            S.upload(co, S.coef.p);
-            check(lincomb(st, out1(r, k), make_double2(0.0, 0.0), S.coef.p, S.Bm.p, n, L, n1), "lincomb(t1)");
-            check(lincomb(st, out2(r, k), make_double2(0.0, 0.0), S.coef.p, S.Bm.p + n1, n, L, n2), "lincomb(t2)");
-            check(cudaStreamSynchronize(st), "sync");
+        {
+          std::vector<int> wr;
+          for (int sidx : active)
+            if (relres[sidx] <= tol || last) wr.push_back(sidx);
+          write_solutions(wr, L);
+          for (int sidx : wr)
             if (relres[sidx] <= tol) done[sidx] = 1;
-          }
         }
         all_done = std::all_of(done.begin(), done.end(), [](int d) { return d != 0; });
         if (all_done || last) break;
@@ -265,9 +319,14 @@ static int solve_impl(cclr_ctx *ctx, const cclr_c128 *xi1, const cclr_c128 *xi2,
           // b' = B C and sigma' = S C, staged in the residual block (m <= rcap), then copied to the front rows
           for (int pass = 0; pass < 2; ++pass) {
             c128 *src = pass == 0 ? S.Bm.p : S.Sm.p;
-            for (int i = 0; i < m; ++i) {
-              S.upload(Cc[i], S.coef.p);
-              check(lincomb(st, S.r(i), make_double2(0.0, 0.0), S.coef.p, src, n, L, n), "lincomb(collapse)");
+            for (int i0 = 0; i0 < m; i0 += BLOCK_LINCOMB_MAX) {
+              const int R = std::min(BLOCK_LINCOMB_MAX, m - i0);
+              std::vector<cplx> co((size_t)R * L);
+              for (int i = 0; i < R; ++i)
+                for (int j = 0; j < L; ++j) co[(size_t)i * L + j] = Cc[i0 + i][j];
+              S.upload(co, S.coef.p);
+              check(block_lincomb(st, R, S.r(i0), n, nullptr, 0, make_double2(0.0, 0.0), S.coef.p, L, src, n, L, nullptr, 0, 0, n,
+                                  nullptr, nullptr, nullptr, nullptr, nullptr, 0), "block_lincomb(collapse)");
             }
             check(cudaMemcpyAsync(src, S.R.p, (size_t)m * n * sizeof(c128), cudaMemcpyDeviceToDevice, st), "copy collapsed");
           }
@@ -309,37 +368,42 @@ static int solve_impl(cclr_ctx *ctx, const cclr_c128 *xi1, const cclr_c128 *xi2,
           Lc = m;
           have_residuals = false;          // the residual block was used as scratch
         }
-        int added = 0;
+        // the preconditioned residuals r / (z - D) of the picks, gathered into one block, then orthonormalised against the
+        // trial space and among themselves in one block Gram-Schmidt step
+        if ((int)picks.size() > maxdim - S.L) picks.resize(std::max(0, maxdim - S.L));
+        int np = 0;
         for (int sidx : picks) {
-          if (S.L >= maxdim) break;
           const int r = sidx / nomega, k = sidx % nomega;
-          c128 *rv;
-          if (have_residuals) {
-            rv = S.r((int)(std::find(active.begin(), active.end(), sidx) - active.begin()));
+          const int pos = (int)(std::find(active.begin(), active.end(), sidx) - active.begin());
+          if (have_residuals && have_pc) {
+            check(cudaMemcpyAsync(S.nv(np), S.pc(pos), (size_t)n * sizeof(c128), cudaMemcpyDeviceToDevice, st), "copy correction");
           } else {
-            // r = xi + sum_j beta_j (sigma_j - z b_j) in the current basis
-            rv = S.tmp.p;
-            check(cudaMemcpyAsync(rv, S.xi(r), (size_t)n * sizeof(c128), cudaMemcpyDeviceToDevice, st), "copy xi");
-            std::vector<cplx> co(Lc);
-            for (int j = 0; j < Lc; ++j) co[j] = beta[(size_t)sidx * maxdim + j];
-            S.add_combination(rv, make_double2(1.0, 0.0), co, S.Sm.p, Lc, n, n);
-            for (int j = 0; j < Lc; ++j) co[j] = -z[k] * beta[(size_t)sidx * maxdim + j];
-            S.add_combination(rv, make_double2(1.0, 0.0), co, S.Bm.p, Lc, n, n);
+            const c128 *rv;
+            if (have_residuals) {
+              rv = S.r(pos);
+            } else {
+              // r = xi + sum_j beta_j (sigma_j - z b_j) in the current basis
+              std::vector<cplx> co((size_t)2 * Lc);
+              for (int j = 0; j < Lc; ++j) {
+                co[j] = beta[(size_t)sidx * maxdim + j];
+                co[Lc + j] = -z[k] * beta[(size_t)sidx * maxdim + j];
+              }
+              S.upload(co, S.coef.p);
+              check(block_lincomb(st, 1, S.tmp.p, n, S.xi(r), 0, make_double2(1.0, 0.0), S.coef.p, 2 * Lc, S.Sm.p, n, Lc, S.Bm.p, n, Lc,
+                                  n, nullptr, nullptr, nullptr, nullptr, nullptr, 0), "block_lincomb(residual)");
+              rv = S.tmp.p;
+            }
+            check(precondition(st, S.nv(np), rv, ctx->D, make_double2(z[k].real(), z[k].imag()), make_double2(1.0, 0.0), n), "precondition");
           }
-          check(precondition(st, rv, rv, ctx->D, make_double2(z[k].real(), z[k].imag()), make_double2(1.0, 0.0), n), "precondition");
-          if (S.append(rv)) ++added;
+          ++np;
         }
+        const int added = S.append_block(S.NV.p, np);
         if (added == 0 && S.L == L0) {
           // no new direction could be added (numerically dependent corrections): stop with what we have
           rc = CCLR_ENOTCONV;
           for (int sidx : active)
             if (!done[sidx]) {
-              const int r = sidx / nomega, k = sidx % nomega;
-              std::vector<cplx> co(Lc);
-              for (int j = 0; j < Lc; ++j) co[j] = beta[(size_t)sidx * maxdim + j];
-              S.upload(co, S.coef.p);
-              check(lincomb(st, out1(r, k), make_double2(0.0, 0.0), S.coef.p, S.Bm.p, n, Lc, n1), "lincomb(t1)");
-              check(lincomb(st, out2(r, k), make_double2(0.0, 0.0), S.coef.p, S.Bm.p + n1, n, Lc, n2), "lincomb(t2)");
+              write_solutions(std::vector<int>{sidx}, Lc);
             }
           break;
         }
@@ -411,5 +475,40 @@ extern "C" int cclr_host_shifted_solve(int L, const cclr_c128 *G, const cclr_c12
   for (int k = 0; k < nz; ++k)
     if (!h.solve(cplx(z[k].re, z[k].im), reinterpret_cast<const cplx *>(rhs), reinterpret_cast<cplx *>(beta) + (size_t)k * L))
       return CCLR_EINVAL;
+  return CCLR_OK;
+}
+
+
+// ---- kernel-level entry points of the solver's bandwidth kernels (unit tests, HBM-roofline measurement in bench.py) ----------
+extern "C" int cclr_vec_block_lincomb(cclr_ctx *ctx, int R, cclr_c128 *Y, long ldy, const cclr_c128 *X, long ldx, const cclr_c128 *coef,
+                                      const cclr_c128 *V, long ldv, int m, long n, double *nrm2, const cclr_c128 *z, cclr_c128 *P,
+                                      long ldp) {
+  if (!ctx || !Y || !coef || !V || R < 1 || R > BLOCK_LINCOMB_MAX || m < 0 || n < 1 || (P && !z) || (P && n > ctx->n1 + ctx->n2))
+    return CCLR_EINVAL;
+  try {
+    double *scratch = nullptr;
+    if (nrm2) check(cudaMalloc(&scratch, (size_t)block_lincomb_grid(n) * BLOCK_LINCOMB_MAX * sizeof(double)), "cudaMalloc(norm scratch)");
+    const cudaError_t e = block_lincomb(ctx->st, R, (c128 *)Y, ldy, (const c128 *)X, ldx, make_double2(1.0, 0.0), (const c128 *)coef, m,
+                                        (const c128 *)V, ldv, m, nullptr, 0, 0, n, nrm2, scratch, P ? ctx->D : nullptr, (const c128 *)z,
+                                        (c128 *)P, ldp);
+    if (scratch) { cudaStreamSynchronize(ctx->st); cudaFree(scratch); }
+    check(e, "block_lincomb");
+  } catch (const PlanError &e) {
+    return cclr_fail(e);
+  }
+  return CCLR_OK;
+}
+
+extern "C" int cclr_vec_dots(cclr_ctx *ctx, const cclr_c128 *A, int na, const cclr_c128 *B, int nb, long n, long ld, cclr_c128 *out) {
+  if (!ctx || !A || !B || !out || na < 1 || nb < 1 || n < 1 || ld < n) return CCLR_EINVAL;
+  try {
+    subspace::Space S;
+    S.ctx = ctx; S.st = ctx->st; S.n = n;
+    if (ld != n) return CCLR_EINVAL;     // the solver's vectors are dense rows
+    std::vector<cplx> h = S.dots((const c128 *)A, na, (const c128 *)B, nb);
+    for (size_t k = 0; k < h.size(); ++k) { out[k].re = h[k].real(); out[k].im = h[k].imag(); }
+  } catch (const PlanError &e) {
+    return cclr_fail(e);
+  }
   return CCLR_OK;
 }

@@ -35,13 +35,19 @@ struct Space {
   c128 *b(int j) { return Bm.p + (size_t)j * n; }
   c128 *s(int j) { return Sm.p + (size_t)j * n; }
 
-  // out[ia*nb+ib] = <A_ia | B_ib> (sesquilinear) on the host
+  // out[ia*nb+ib] = <A_ia | B_ib> (sesquilinear) on the host.  Blocks (na, nb >= 2) run as ONE split-K DMMA GEMM
+  // conj(A)[na x n] . B[nb x n]^T, which reads every vector once; single rows / columns and the diagonal use the chunked
+  // reduction kernel of vecops.cu.  Both are deterministic (fixed split / chunk order).
   std::vector<cplx> dots(const c128 *A, int na, const c128 *Bp, int nb, bool diag = false) {
     const int np = diag ? na : na * nb;
     std::vector<cplx> out(np);
     if (np == 0) return out;
     cclr_ensure_dot_scratch(ctx, np);
-    check(multi_dot(st, A, n, na, Bp, n, nb, n, true, diag, ctx->dot_partial, ctx->dot_out), "multi_dot");
+    if (!diag && na >= 2 && nb >= 2 && n >= 4096)
+      check(zgemm(st, na, nb, (int)n, make_double2(1.0, 0.0), A, n, true, Bp, n, false, false, make_double2(0.0, 0.0),
+                  ctx->dot_out, nb, 1, 0, 0, 0, &ctx->ws), "zgemm(dots)");
+    else
+      check(multi_dot(st, A, n, na, Bp, n, nb, n, true, diag, ctx->dot_partial, ctx->dot_out), "multi_dot");
     check(cudaMemcpyAsync(out.data(), ctx->dot_out, (size_t)np * sizeof(c128), cudaMemcpyDeviceToHost, st), "D2H dots");
     check(cudaStreamSynchronize(st), "sync dots");
     return out;
@@ -59,14 +65,14 @@ struct Space {
     check(lincomb(st, y, beta, coef.p, V, ldv, m, len), "lincomb");
   }
 
-  // orthonormalise v against b_0..b_{L-1} (classical Gram-Schmidt, two passes) and append it; false if dependent
-  bool append(c128 *v) {
-    const double n0 = std::sqrt(std::max(0.0, dots(v, 1, v, 1)[0].real()));
+  // orthonormalise v against b_from..b_{L-1} (Gram-Schmidt, two passes) and append it; false if (numerically) dependent.
+  // n0 = the norm the vector had before any projection (the dependence test is relative to it)
+  bool append_range(c128 *v, int from, double n0) {
     if (!(n0 > 0.0) || !std::isfinite(n0)) return false;
-    for (int pass = 0; pass < 2 && L > 0; ++pass) {
-      std::vector<cplx> h = dots(Bm.p, L, v, 1);
+    for (int pass = 0; pass < 2 && L > from; ++pass) {
+      std::vector<cplx> h = dots(b(from), L - from, v, 1);
       for (auto &x : h) x = -x;
-      add_combination(v, make_double2(1.0, 0.0), h, Bm.p, L, n, n);
+      add_combination(v, make_double2(1.0, 0.0), h, b(from), L - from, n, n);
     }
     const double n1_ = std::sqrt(std::max(0.0, dots(v, 1, v, 1)[0].real()));
     if (!(n1_ > 1e-10 * n0)) return false;
@@ -74,6 +80,34 @@ struct Space {
     check(cudaMemcpyAsync(b(L), v, (size_t)n * sizeof(c128), cudaMemcpyDeviceToDevice, st), "copy trial vector");
     ++L;
     return true;
+  }
+
+  bool append(c128 *v) { return append_range(v, 0, std::sqrt(std::max(0.0, dots(v, 1, v, 1)[0].real()))); }
+
+  // Block version (step 5 of PAPER.md:966 for all new correction vectors of an iteration at once): V holds nv vectors
+  // (leading dimension n).  Two passes of block classical Gram-Schmidt against the current basis -- H = b^H V as one GEMM,
+  // V -= b H as one multi-row update, each reading the basis once for all nv vectors -- then the vectors are orthonormalised
+  // among themselves one by one and appended.  Returns how many were accepted.
+  int append_block(c128 *V, int nv) {
+    if (nv <= 0) return 0;
+    std::vector<cplx> nn0 = dots(V, nv, V, nv, true);
+    const int L_old = L;
+    for (int pass = 0; pass < 2 && L_old > 0; ++pass) {
+      std::vector<cplx> H = dots(Bm.p, L_old, V, nv);                       // [L_old][nv]
+      for (int r0 = 0; r0 < nv; r0 += BLOCK_LINCOMB_MAX) {
+        const int R = std::min(BLOCK_LINCOMB_MAX, nv - r0);
+        std::vector<cplx> co((size_t)R * L_old);
+        for (int r = 0; r < R; ++r)
+          for (int j = 0; j < L_old; ++j) co[(size_t)r * L_old + j] = -H[(size_t)j * nv + r0 + r];
+        upload(co, coef.p);
+        check(block_lincomb(st, R, V + (size_t)r0 * n, n, V + (size_t)r0 * n, n, make_double2(1.0, 0.0), coef.p, L_old, Bm.p, n,
+                            L_old, nullptr, 0, 0, n, nullptr, nullptr, nullptr, nullptr, nullptr, 0), "block_lincomb(GS)");
+      }
+    }
+    int added = 0;
+    for (int k = 0; k < nv && L < maxdim; ++k)
+      if (append_range(V + (size_t)k * n, L_old, std::sqrt(std::max(0.0, nn0[k].real())))) ++added;
+    return added;
   }
 
   // sigma_j = A b_j for j in [L0, L) and the new rows / columns of G

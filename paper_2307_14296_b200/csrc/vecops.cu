@@ -125,6 +125,109 @@ __global__ void __launch_bounds__(256) denominators_kernel(const c128 *__restric
   }
 }
 
+// Y[r][i] = xs * X[r][i] + sum_{j<m0} coef[r][j] V0[j][i] + sum_{j<m1} coef[r][m0+j] V1[j][i]   for r < R rows at once:
+// every element of the m0 + m1 subspace vectors is read ONCE for all R outputs (the per-row kernel above reads them R times).
+// This is the residual block r_k = xi + sum_j beta_kj (sigma_j - z_k b_j) (step 4), the solutions t_k = sum_j
+// beta_kj b_j (step 5), the subspace collapse and the block Gram-Schmidt update of PAPER.md:966.  Fused outputs
+// (each optional): nrm2[r] = sum_i |Y[r][i]|^2 (deterministic two-level reduction: per-CTA partials in fixed order), and the
+// preconditioned vector P[r][i] = Y[r][i] / (z[r] - D[i]) -- residual, norm and correction in one pass.
+constexpr int BL_JT = 32;   // coefficient tile (columns j) staged in shared memory
+struct BlockLincombArgs {
+  c128 *Y; long ldy;
+  const c128 *X; long ldx; c128 xs;
+  const c128 *coef; int ldc;               // device [R][ldc]
+  const c128 *V0; long ldv0; int m0;
+  const c128 *V1; long ldv1; int m1;
+  long n;
+  double *nrm_partial;                      // [gridDim.x][R] or null
+  const double *D; const c128 *z;           // preconditioner (z: device [R]) or null
+  c128 *P; long ldp;
+};
+
+template <int R, int BL_E>
+__global__ void __launch_bounds__(256) block_lincomb_kernel(const BlockLincombArgs a) {
+  __shared__ c128 cs[R][BL_JT];
+  const int m = a.m0 + a.m1;
+  double nr[R];
+#pragma unroll
+  for (int r = 0; r < R; ++r) nr[r] = 0.0;
+  const long tile = 256L * BL_E;
+  for (long t0 = (long)blockIdx.x * tile; t0 < a.n; t0 += (long)gridDim.x * tile) {
+    c128 acc[R][BL_E];
+    long idx[BL_E];
+#pragma unroll
+    for (int e = 0; e < BL_E; ++e) {
+      idx[e] = t0 + e * 256 + threadIdx.x;
+#pragma unroll
+      for (int r = 0; r < R; ++r)
+        acc[r][e] = (a.X && idx[e] < a.n) ? cmul(a.xs, a.X[(size_t)r * a.ldx + idx[e]]) : czero();
+    }
+    for (int j0 = 0; j0 < m; j0 += BL_JT) {
+      __syncthreads();
+      for (int q = threadIdx.x; q < R * BL_JT; q += 256) {
+        const int r = q / BL_JT, j = j0 + q % BL_JT;
+        cs[r][q % BL_JT] = j < m ? a.coef[(size_t)r * a.ldc + j] : czero();
+      }
+      __syncthreads();
+      const int jn = m - j0 < BL_JT ? m - j0 : BL_JT;
+#pragma unroll 2
+      for (int jj = 0; jj < jn; ++jj) {
+        const int j = j0 + jj;
+        const c128 *vrow = j < a.m0 ? a.V0 + (size_t)j * a.ldv0 : a.V1 + (size_t)(j - a.m0) * a.ldv1;
+        c128 v[BL_E];
+#pragma unroll
+        for (int e = 0; e < BL_E; ++e) v[e] = idx[e] < a.n ? vrow[idx[e]] : czero();
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+          const c128 c = cs[r][jj];
+#pragma unroll
+          for (int e = 0; e < BL_E; ++e) cfma(acc[r][e], c, v[e]);
+        }
+      }
+    }
+#pragma unroll
+    for (int e = 0; e < BL_E; ++e) {
+      if (idx[e] >= a.n) continue;
+      const double d = a.P ? a.D[idx[e]] : 0.0;
+#pragma unroll
+      for (int r = 0; r < R; ++r) {
+        const c128 y = acc[r][e];
+        a.Y[(size_t)r * a.ldy + idx[e]] = y;
+        nr[r] += y.x * y.x + y.y * y.y;
+        if (a.P) {
+          const c128 z = a.z[r];
+          const double dr = z.x - d, di = z.y, inv = 1.0 / (dr * dr + di * di);
+          a.P[(size_t)r * a.ldp + idx[e]] = make_double2((y.x * dr + y.y * di) * inv, (y.y * dr - y.x * di) * inv);
+        }
+      }
+    }
+  }
+  if (a.nrm_partial) {
+    __shared__ double red[R][8];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+      double w = nr[r];
+#pragma unroll
+      for (int s = 16; s > 0; s >>= 1) w += __shfl_xor_sync(0xffffffffu, w, s);
+      if ((threadIdx.x & 31) == 0) red[r][threadIdx.x >> 5] = w;
+    }
+    __syncthreads();
+    if (threadIdx.x < R) {
+      double w = 0.0;
+      for (int k = 0; k < 8; ++k) w += red[threadIdx.x][k];
+      a.nrm_partial[(size_t)blockIdx.x * R + threadIdx.x] = w;
+    }
+  }
+}
+
+__global__ void block_norm_final_kernel(const double *__restrict__ partial, int nblocks, int R, double *__restrict__ out) {
+  const int r = threadIdx.x;
+  if (r >= R) return;
+  double s = 0.0;
+  for (int b = 0; b < nblocks; ++b) s += partial[(size_t)b * R + r];
+  out[r] = s;
+}
+
 int stream_grid(long n) {
   long blocks = (n + 255) / 256;
   const long cap = (long)zgemm_num_sms() * 16;
@@ -150,14 +253,17 @@ cudaError_t multi_dot(cudaStream_t st, const c128 *A, long lda, int na, const c1
   if (npairs <= 0) return cudaSuccess;
   const int chunks = dot_chunks(n);
   const long chunk_len = (n + chunks - 1) / chunks;
-  // blockIdx.y is limited to 65535 pairs per launch
-  for (int p0 = 0; p0 < npairs; p0 += 32768) {
-    const int np = npairs - p0 < 32768 ? npairs - p0 : 32768;
-    if (!diag && p0 != 0) return cudaErrorInvalidValue;   // callers keep na*nb below the limit
+  // blockIdx.y is limited to 65535: launch in slabs of at most 32768 (ia, ib) pairs -- whole rows ia of the pair matrix in the
+  // general case, consecutive pairs in the diagonal case; every slab writes its partial sums at its own offset
+  if (!diag && nb > 32768) return cudaErrorInvalidValue;
+  const int rows_per = diag ? 32768 : (32768 / nb > 0 ? 32768 / nb : 1);
+  for (int r0 = 0; r0 < na; r0 += rows_per) {
+    const int nr = na - r0 < rows_per ? na - r0 : rows_per;
+    const int np = diag ? nr : nr * nb;
+    const size_t p0 = diag ? (size_t)r0 : (size_t)r0 * nb;
     dim3 grid(chunks, np);
-    const c128 *Ap = diag ? A + (size_t)p0 * lda : A, *Bp = diag ? B + (size_t)p0 * ldb : B;
-    dot_partial_kernel<<<grid, DOT_THREADS, 0, st>>>(Ap, lda, Bp, ldb, nb, n, conjA ? 1 : 0, diag ? 1 : 0, chunk_len,
-                                                     partial + (size_t)p0 * chunks);
+    dot_partial_kernel<<<grid, DOT_THREADS, 0, st>>>(A + (size_t)r0 * lda, lda, diag ? B + (size_t)r0 * ldb : B, ldb, nb, n,
+                                                     conjA ? 1 : 0, diag ? 1 : 0, chunk_len, partial + p0 * chunks);
     cclr_count_launch();
   }
   dot_final_kernel<<<(npairs + 127) / 128, 128, 0, st>>>(partial, chunks, npairs, out);
@@ -191,5 +297,44 @@ cudaError_t denominators(cudaStream_t st, const c128 *fock, int o, int v, double
   const long n = (long)o * v + npair(o) * npair(v);
   denominators_kernel<<<stream_grid(n), 256, 0, st>>>(fock, o, v, D);
   cclr_count_launch();
+  return cudaGetLastError();
+}
+
+static int block_lincomb_e(int R) { return R <= 4 ? 4 : 2; }   // elements per thread: more loads in flight when few accumulators
+
+int block_lincomb_grid(long n) {
+  long tiles = (n + 511) / 512;
+  const long cap = (long)zgemm_num_sms() * 8;
+  if (tiles > cap) tiles = cap;
+  if (tiles < 1) tiles = 1;
+  return (int)tiles;
+}
+
+// see block_lincomb_kernel; R <= BLOCK_LINCOMB_MAX rows per call; nrm2 (device [R]) / nrm_scratch (device, block_lincomb_grid(n) * R
+// doubles) and D / z / P are optional (null)
+cudaError_t block_lincomb(cudaStream_t st, int R, c128 *Y, long ldy, const c128 *X, long ldx, c128 xs, const c128 *coef, int ldc,
+                          const c128 *V0, long ldv0, int m0, const c128 *V1, long ldv1, int m1, long n, double *nrm2,
+                          double *nrm_scratch, const double *D, const c128 *z, c128 *P, long ldp) {
+  if (n <= 0 || R <= 0) return cudaSuccess;
+  if (R > BLOCK_LINCOMB_MAX) return cudaErrorInvalidValue;
+  BlockLincombArgs a{Y, ldy, X, ldx, xs, coef, ldc, V0, ldv0, m0, V1, ldv1, m1, n, nrm2 ? nrm_scratch : nullptr, D, z, P, ldp};
+  int grid = block_lincomb_grid(n);
+  const long tiles = (n + 256L * block_lincomb_e(R) - 1) / (256L * block_lincomb_e(R));
+  if (grid > tiles) grid = (int)tiles;
+  switch (R) {
+    case 1: block_lincomb_kernel<1, 4><<<grid, 256, 0, st>>>(a); break;
+    case 2: block_lincomb_kernel<2, 4><<<grid, 256, 0, st>>>(a); break;
+    case 3: block_lincomb_kernel<3, 4><<<grid, 256, 0, st>>>(a); break;
+    case 4: block_lincomb_kernel<4, 4><<<grid, 256, 0, st>>>(a); break;
+    case 5: block_lincomb_kernel<5, 2><<<grid, 256, 0, st>>>(a); break;
+    case 6: block_lincomb_kernel<6, 2><<<grid, 256, 0, st>>>(a); break;
+    case 7: block_lincomb_kernel<7, 2><<<grid, 256, 0, st>>>(a); break;
+    default: block_lincomb_kernel<8, 2><<<grid, 256, 0, st>>>(a); break;
+  }
+  cclr_count_launch();
+  if (nrm2) {
+    block_norm_final_kernel<<<1, 32, 0, st>>>(nrm_scratch, grid, R, nrm2);
+    cclr_count_launch();
+  }
   return cudaGetLastError();
 }

@@ -159,3 +159,34 @@ def test_xi_built_on_the_device_matches_oracle(cfg1):
         w1, w2 = packing.pack_amplitudes(*s["xis"][k])
         assert np.linalg.norm(g1.cpu().numpy() - w1.reshape(-1)) <= 1e-12 * np.linalg.norm(w1)
         assert np.linalg.norm(g2.cpu().numpy() - w2.reshape(-1)) <= 1e-12 * np.linalg.norm(w2)
+
+
+def test_solver_bandwidth_kernels_match_numpy(cfg1):
+    """The multi-row update (residual / solution / Gram-Schmidt block, with the fused norm and preconditioned output) and the
+    dot block (split-K DMMA GEMM path and single-row path) against numpy, ragged sizes."""
+    s = cfg1
+    cc, ctx = s["cc"], s["ctx"]
+    n = ctx.n1 + ctx.n2
+    rng = np.random.default_rng(5)
+    cplx = lambda *shape: rng.normal(size=shape) + 1j * rng.normal(size=shape)
+    D = flat(s["c"].D1 + 0j, s["c"].D2 + 0j).real                 # orbital-energy differences over unique elements
+    for (R, m, shared_x) in [(1, 3, False), (3, 37, True), (8, 70, False), (5, 1, True)]:
+        V, X, coef = cplx(m, n), cplx(n) if shared_x else cplx(R, n), cplx(R, m)
+        z = cplx(R) * 0.1 + 0.05
+        Y = torch.zeros((R, n), dtype=torch.complex128, device="cuda")
+        P = torch.zeros((R, n), dtype=torch.complex128, device="cuda")
+        nrm = torch.zeros(R, dtype=torch.float64, device="cuda")
+        cc.cclr_vec_block_lincomb(ctx, Y, torch.from_numpy(X).cuda(), torch.from_numpy(coef).cuda().contiguous(),
+                                  torch.from_numpy(V).cuda(), nrm2=nrm, z=torch.from_numpy(z).cuda(), P=P)
+        torch.cuda.synchronize()
+        want = (X[None, :] if shared_x else X) + coef @ V
+        assert np.abs(Y.cpu().numpy() - want).max() <= 1e-13 * np.abs(want).max()
+        assert np.abs(nrm.cpu().numpy() - (np.abs(want) ** 2).sum(1)).max() <= 1e-13 * (np.abs(want) ** 2).sum(1).max()
+        wp = want / (z[:, None] - D[None, :])
+        assert np.abs(P.cpu().numpy() - wp).max() <= 1e-13 * np.abs(wp).max()
+    big = 6000                                                   # long enough for the GEMM dot path
+    A, B = cplx(5, big), cplx(3, big)
+    for (a, b) in [(A, B), (A, B[:1]), (A[:1], B)]:
+        got = np.array(cc.cclr_vec_dots(ctx, torch.from_numpy(np.ascontiguousarray(a)).cuda(), torch.from_numpy(np.ascontiguousarray(b)).cuda()))
+        want = a.conj() @ b.T
+        assert np.abs(got - want).max() <= 1e-13 * np.abs(want).max()
