@@ -55,6 +55,9 @@ typedef struct {
 #define CCLR_GEMM_4M 4u     /* every contraction of this context uses the 4M complex product (default: the large ones use 3M,
                                see cclr_zgemm); a per-context choice, nothing process-wide */
 
+#define CCLR_NO_GRAPH 8u    /* never replay sigma as a CUDA graph (default: contexts with at most 2^21 unique amplitudes capture the sigma
+                               plan once and replay it per trial vector -- they are launch bound; results are identical) */
+
 #define CCLR_SMALL_CHUNKS 2u /* testing aid: run the chunked intermediate builds with chunks of 3 indices so that small
                                inputs exercise several chunks and a ragged last one (results are unchanged) */
 

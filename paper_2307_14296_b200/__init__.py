@@ -38,6 +38,7 @@ def _stream():
 ERI_INPLACE = 1
 SMALL_CHUNKS = 2
 GEMM_4M = 4
+NO_GRAPH = 8
 
 
 class Context:

@@ -73,6 +73,15 @@ struct PermArgs {
 };
 cudaError_t permute(cudaStream_t st, const PermArgs &args);
 
+// ---- layout.cu: the hot layout statements of sigma, specialised (semantics: see the kernels' comments) ----------------
+cudaError_t layout_unpack_rows(cudaStream_t st, const c128 *src, c128 *dst, int n, long len);
+cudaError_t layout_unpack_cols(cudaStream_t st, const c128 *src, c128 *dst, long rows, int o);
+cudaError_t layout_unpack_ring(cudaStream_t st, const c128 *src, c128 *dst, int v, int o);
+cudaError_t layout_transpose_pair(cudaStream_t st, const c128 *src, c128 *dst, long ncol, int o);
+cudaError_t layout_final_pack(cudaStream_t st, c128 *out2, const c128 *x2, c128 nz, const c128 *Y, const c128 *Q, const c128 *Z,
+                              int v, int o);
+constexpr size_t LAYOUT_MAX_SMEM = 200 * 1024;   // final_pack stages 3 o^2 complex numbers (o <= 65)
+
 // ---- vecops.cu: bandwidth kernels of the solver / property contraction ------------------------------------------
 // out[ia*nb+ib] = sum_i op(A[ia][i]) * B[ib][i]  (op = conj if conjA); diag != 0: out[ia] = sum_i op(A[ia][i]) B[ia][i].
 // partial is a device scratch of at least dots_scratch_elems(na*nb) complex numbers; out is a DEVICE array.
@@ -92,5 +101,7 @@ cudaError_t block_lincomb(cudaStream_t st, int R, c128 *Y, long ldy, const c128 
 // y[i] = alpha * x[i] / (z - D[i])      (orbital-energy preconditioner)
 cudaError_t precondition(cudaStream_t st, c128 *y, const c128 *x, const double *D, c128 z, c128 alpha, long n);
 cudaError_t scale_vec(cudaStream_t st, c128 *y, c128 alpha, long n);
+// out[i] = src[i] + alpha * x[i]
+cudaError_t shifted_copy(cudaStream_t st, c128 *out, const c128 *src, c128 alpha, const c128 *x, long n);
 // D1[a,i] = eps_a - eps_i, D2[(ab),(ij)] = eps_a + eps_b - eps_i - eps_j from the diagonal of fock ([n][n])
 cudaError_t denominators(cudaStream_t st, const c128 *fock, int o, int v, double *D);

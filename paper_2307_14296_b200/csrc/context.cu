@@ -91,12 +91,64 @@ void destroy(cclr_ctx *ctx) {
   if (ctx->xblocks) cudaFree(ctx->xblocks);
   if (ctx->lambda) cudaFree(ctx->lambda);
   for (cudaEvent_t ev : ctx->events) cudaEventDestroy(ev);
+  if (ctx->sigma_graph) cudaGraphExecDestroy(ctx->sigma_graph);
+  if (ctx->graph_stream) cudaStreamDestroy(ctx->graph_stream);
+  if (ctx->graph_io) cudaFree(ctx->graph_io);
   delete ctx;
 }
 
 }  // namespace
 
+extern unsigned long long cclr_launch_counter();   // probes.cu
+
+// Capture the sigma plan once into a CUDA graph bound to the staging vectors graph_io (shift 0); false if capture is impossible
+static bool build_sigma_graph(cclr_ctx *ctx) {
+  const size_t n = (size_t)(ctx->n1 + ctx->n2);
+  if (cudaMalloc(&ctx->graph_io, 2 * n * sizeof(c128)) != cudaSuccess) { cudaGetLastError(); ctx->graph_io = nullptr; return false; }
+  ctx->extra_bytes += 2 * n * sizeof(c128);
+  if (cudaStreamCreateWithFlags(&ctx->graph_stream, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); return false; }
+  c128 *g = ctx->graph_io;
+  bind_vectors(ctx, g, g + ctx->n1, g + n, g + n + ctx->n1);
+  ctx->plan->set_scalar(0, make_double2(0.0, 0.0));
+  cudaStreamSynchronize(ctx->st);
+  cudaGraph_t graph = nullptr;
+  bool ok = cudaStreamBeginCapture(ctx->graph_stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+  if (ok) {
+    const unsigned long long c0 = cclr_launch_counter();
+    ctx->plan->set_stream(ctx->graph_stream);
+    try {
+      for (const ResolvedOp &op : ctx->sigma_ops) ctx->plan->launch(op);
+    } catch (const PlanError &) {
+      ok = false;
+    }
+    ctx->plan->set_stream(ctx->st);
+    ctx->graph_kernels = (int)(cclr_launch_counter() - c0);
+    if (cudaStreamEndCapture(ctx->graph_stream, &graph) != cudaSuccess || !graph) ok = false;
+  }
+  if (ok && cudaGraphInstantiate(&ctx->sigma_graph, graph, 0) != cudaSuccess) { ctx->sigma_graph = nullptr; ok = false; }
+  if (graph) cudaGraphDestroy(graph);
+  if (!ok) cudaGetLastError();
+  return ok;
+}
+
 void cclr_sigma_one(cclr_ctx *ctx, const c128 *x1, const c128 *x2, c128 z, c128 *out1, c128 *out2, bool profile, bool left) {
+  if (ctx->graph_enabled && !ctx->graph_failed && !profile && !left) {
+    if (!ctx->sigma_graph && ctx->plain_sigma_calls > 0 && !build_sigma_graph(ctx)) ctx->graph_failed = true;
+    if (ctx->sigma_graph) {
+      // replay: x -> staging, the captured kernels, out = (A x) - z x
+      const size_t n = (size_t)(ctx->n1 + ctx->n2);
+      c128 *g = ctx->graph_io;
+      check(cudaMemcpyAsync(g, x1, (size_t)ctx->n1 * sizeof(c128), cudaMemcpyDeviceToDevice, ctx->st), "stage x1");
+      check(cudaMemcpyAsync(g + ctx->n1, x2, (size_t)ctx->n2 * sizeof(c128), cudaMemcpyDeviceToDevice, ctx->st), "stage x2");
+      check(cudaGraphLaunch(ctx->sigma_graph, ctx->st), "cudaGraphLaunch(sigma)");
+      cclr_count_launch(ctx->graph_kernels);
+      const c128 nz = make_double2(-z.x, -z.y);
+      check(shifted_copy(ctx->st, out1, g + n, nz, x1, ctx->n1), "shift sigma1");
+      check(shifted_copy(ctx->st, out2, g + n + ctx->n1, nz, x2, ctx->n2), "shift sigma2");
+      return;
+    }
+    ++ctx->plain_sigma_calls;
+  }
   bind_vectors(ctx, x1, x2, out1, out2);
   ctx->plan->set_scalar(0, make_double2(-z.x, -z.y));
   run_ops(ctx, left ? ctx->left_ops : ctx->sigma_ops, profile);
@@ -221,6 +273,9 @@ extern "C" int cclr_create(int o, int v, const cclr_c128 *fock, const cclr_eri_p
     P.compile(CCLR_PLAN_ETA, ctx->eta_ops);
     P.compile(CCLR_PLAN_ETA_EOM, ctx->eta_eom_ops);
     cclr_ensure_dot_scratch(ctx, 256);
+    // launch-bound sizes replay the sigma plan as one CUDA graph (configs 1, 2, 5; above ~2M unique elements the ~40 launches
+    // of a sigma evaluation are noise)
+    ctx->graph_enabled = !(flags & CCLR_NO_GRAPH) && (ctx->n1 + ctx->n2) <= (2L << 20);
   } catch (const PlanError &e) {
     destroy(ctx);
     return cclr_fail(e);

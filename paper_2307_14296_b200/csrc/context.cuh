@@ -29,6 +29,13 @@ struct cclr_ctx {
   c128 *lambda = nullptr;         // ground-state multipliers [n1 + n2], solved on first use by cclr_response_ci
   bool have_lambda = false;
   double lambda_tol = 0.0;        // tolerance the cached multipliers were solved to (a tighter request re-solves)
+  // CUDA graph of the sigma plan (small problems are launch bound: ~35 kernels + 2 tensor-map encodes per GEMM per vector)
+  bool graph_enabled = false, graph_failed = false;
+  int plain_sigma_calls = 0;      // the first call runs plainly (it also configures the kernels' shared-memory attributes)
+  cudaStream_t graph_stream = nullptr;
+  cudaGraphExec_t sigma_graph = nullptr;
+  c128 *graph_io = nullptr;       // staging [x1 | x2 | out1 | out2] the captured kernels are bound to
+  int graph_kernels = 0;          // kernels per replay (added to the launch counter)
   int max_subspace = 0;           // cclr_set_max_subspace (0 = automatic)
   size_t extra_bytes = 0;         // device bytes owned outside the plan
 };

@@ -485,7 +485,63 @@ ResolvedOp Plan::resolve_perm(const PlanStmt &s) {
     ++p.nsrc;
   }
   if (p.nsrc == 0) throw PlanError(CCLR_EINVAL, "perm without sources: " + line);
+  classify_special(s, r);
   return r;
+}
+
+// Recognise the hot layout statements of sigma (layout.cu) by the SHAPE of their index specs: letters are renamed A, B, C, ... in
+// order of first appearance in the destination spec, so "Ur[ea(ij)] = 1 x2[(ea)(ij)]" and the same statement in other letters
+// of the same ranges match alike.  Anything else keeps special = 0 (generic gather kernel).
+void Plan::classify_special(const PlanStmt &s, ResolvedOp &r) {
+  r.special = 0;
+  if (s.tok[0] != "perm") return;
+  std::string dname, dspec;
+  split_ref(s.tok[1], dname, dspec);
+  for (char c : dspec)
+    if (std::isupper((unsigned char)c) || c == '1') return;
+  // the final antisymmetrised pack of sigma2, matched literally
+  static const char *const FINAL[] = {"+=", "$nz", "x2[(ab)(ij)]", "1", "Y[ab(ij)]", "-1", "Y[ba(ij)]", "1", "Q[(ab)ij]", "-1", "Q[(ab)ji]",
+                                      "1", "Z[bjai]", "-1", "Z[ajbi]", "-1", "Z[biaj]", "1", "Z[aibj]"};
+  if (s.tok.size() == 2 + sizeof(FINAL) / sizeof(FINAL[0]) && dspec == "(ab)(ij)") {
+    bool same = true;
+    for (size_t k = 0; k < sizeof(FINAL) / sizeof(FINAL[0]); ++k) same = same && s.tok[2 + k] == FINAL[k];
+    const size_t smem = (size_t)3 * o_ * o_ * sizeof(c128);
+    if (same && smem <= LAYOUT_MAX_SMEM) { r.special = 5; r.sp_n = v_; r.sp_o = o_; }
+    return;
+  }
+  if (s.tok.size() != 5 || s.tok[2] != "=" || s.tok[3] != "1") return;
+  std::string sname, sspec;
+  split_ref(s.tok[4], sname, sspec);
+  std::map<char, char> ren;
+  auto canon = [&](const std::string &spec, bool define) {
+    std::string out;
+    for (char c : spec) {
+      if (c == '(' || c == ')') { out += c; continue; }
+      if (!ren.count(c)) {
+        if (!define) return std::string("?");
+        ren[c] = (char)('A' + ren.size());
+      }
+      out += ren[c];
+    }
+    return out;
+  };
+  const std::string d = canon(dspec, true), q = canon(sspec, false);
+  auto letter = [&](char canon_letter) {
+    for (auto &kv : ren)
+      if (kv.second == canon_letter) return kv.first;
+    return 'a';
+  };
+  if (ren.size() != 4) return;
+  const int eA = full_extent(letter('A')), eB = full_extent(letter('B')), eC = full_extent(letter('C')), eD = full_extent(letter('D'));
+  if (d == "AB(CD)" && q == "(AB)(CD)" && eA == eB && eC == eD) {
+    r.special = 1; r.sp_n = eA; r.sp_len = npair(eC);
+  } else if (d == "(AB)CD" && q == "(AB)(CD)" && eA == eB && eC == eD && (size_t)npair(eC) * sizeof(c128) <= 48 * 1024) {
+    r.special = 2; r.sp_len = npair(eA); r.sp_o = eC;
+  } else if (d == "ABCD" && q == "(AC)(BD)" && eA == eC && eB == eD && (size_t)npair(eB) * sizeof(c128) <= 48 * 1024) {
+    r.special = 3; r.sp_n = eA; r.sp_o = eB;
+  } else if (d == "AB(CD)" && q == "(CD)(AB)" && eA == eB && eC == eD) {
+    r.special = 4; r.sp_len = npair(eC); r.sp_o = eA;
+  }
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -498,6 +554,24 @@ void Plan::launch(const ResolvedOp &op) {
     cuda_check(zgemm(st_, op.M, op.N, op.K, alpha, A.ptr + op.aoff, op.lda, op.conjA, B.ptr + op.boff, op.ldb, op.kn,
                      op.conjB, beta, C.ptr + op.coff, op.ldc, 1, 0, 0, 0, ws_),
                "zgemm(" + C.name + ")");
+  } else if (op.special) {
+    const PlanBuf &D = bufs_[op.dst];
+    if (!D.ptr) throw PlanError(CCLR_EINVAL, "perm on an unbound buffer " + D.name);
+    auto src = [&](int k) {
+      const PlanBuf &S = bufs_[op.srcbuf[k]];
+      if (!S.ptr) throw PlanError(CCLR_EINVAL, "perm on an unbound buffer " + S.name);
+      return (const c128 *)S.ptr;
+    };
+    cudaError_t e = cudaSuccess;
+    switch (op.special) {
+      case 1: e = layout_unpack_rows(st_, src(0), D.ptr, op.sp_n, op.sp_len); break;
+      case 2: e = layout_unpack_cols(st_, src(0), D.ptr, op.sp_len, op.sp_o); break;
+      case 3: e = layout_unpack_ring(st_, src(0), D.ptr, op.sp_n, op.sp_o); break;
+      case 4: e = layout_transpose_pair(st_, src(0), D.ptr, op.sp_len, op.sp_o); break;
+      default:   // sources in statement order: x2, Y, Y, Q, Q, Z, Z, Z, Z
+        e = layout_final_pack(st_, D.ptr, src(0), scalars_[0], src(1), src(3), src(5), op.sp_n, op.sp_o);
+    }
+    cuda_check(e, "layout(" + D.name + ")");
   } else {
     PermArgs args = op.args;
     const PlanBuf &D = bufs_[op.dst];

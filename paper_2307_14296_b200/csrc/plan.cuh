@@ -49,6 +49,9 @@ struct ResolvedOp {
   c128 alpha = {1.0, 0.0};
   int alpha_scalar = -1;
   // permute
+  int special = 0;              // 1..5: one of the specialised layout kernels of layout.cu (see Plan::launch), 0: generic gather
+  int sp_n = 0, sp_o = 0;       // their extents
+  long sp_len = 0;
   PermArgs args;
   int dst = -1;
   size_t dstoff = 0;
@@ -85,6 +88,7 @@ class Plan {
   void free_class(int cls);
   size_t owned_bytes() const { return owned_bytes_; }
   cudaStream_t stream() const { return st_; }
+  void set_stream(cudaStream_t st) { st_ = st; }   // CUDA-graph capture of a compiled plan runs on a capture stream
 
  private:
   int o_, v_;
@@ -104,6 +108,7 @@ class Plan {
   void release(int id);
   ResolvedOp resolve_gemm(const PlanStmt &s);
   ResolvedOp resolve_perm(const PlanStmt &s);
+  void classify_special(const PlanStmt &s, ResolvedOp &r);
 
   int full_extent(char letter) const;
   int extent(char letter) const;

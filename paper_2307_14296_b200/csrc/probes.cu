@@ -8,6 +8,7 @@ thread_local int g_last_cuda_error = 0;
 #include <atomic>
 static std::atomic<unsigned long long> g_kernel_launches{0};
 void cclr_count_launch(int n) { g_kernel_launches.fetch_add((unsigned long long)n, std::memory_order_relaxed); }
+unsigned long long cclr_launch_counter() { return g_kernel_launches.load(std::memory_order_relaxed); }
 extern "C" unsigned long long cclr_kernel_launches(void) { return g_kernel_launches.load(std::memory_order_relaxed); }
 
 namespace {

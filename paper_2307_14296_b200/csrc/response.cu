@@ -229,10 +229,18 @@ extern "C" int cclr_response_ci_tensor(cclr_ctx *ctx, const cclr_c128 *X, int no
       if ((rc = cclr_xi(ctx, X + (size_t)r * nn, xi1 + (size_t)r * n1, xi2 + (size_t)r * n2)) != CCLR_OK) return rc;
       if ((rc = cclr_eta(ctx, X + (size_t)r * nn, lam1, lam2, 1, et1 + (size_t)r * n1, et2 + (size_t)r * n2)) != CCLR_OK) return rc;
     }
-    // shifts: [w_0 .. w_{K-1}, -w_0 .. -w_{K-1}] at +gamma (set P) and at -gamma (set M)
-    const int ns = 2 * nomega;
-    std::vector<double> sh(ns);
-    for (int k = 0; k < nomega; ++k) { sh[k] = omegas[k]; sh[nomega + k] = -omegas[k]; }
+    // shifts needed: +-w_k at +gamma (set P) and at -gamma (set M); equal shifts (w = 0, repeated frequencies) are solved once
+    std::vector<double> sh;
+    std::vector<int> idx_pos(nomega), idx_neg(nomega);
+    auto shift_index = [&](double w) {
+      for (size_t q = 0; q < sh.size(); ++q)
+        if (sh[q] == w) return (int)q;
+      sh.push_back(w);
+      return (int)sh.size() - 1;
+    };
+    for (int k = 0; k < nomega; ++k) idx_pos[k] = shift_index(omegas[k]);
+    for (int k = 0; k < nomega; ++k) idx_neg[k] = shift_index(omegas[k] == 0.0 ? 0.0 : -omegas[k]);
+    const int ns = (int)sh.size();
     const bool two_sets = gamma != 0.0;
     DeviceBuf TP, TM;
     TP.alloc((size_t)nop * ns * n, "cudaMalloc(t, +gamma)");
@@ -267,8 +275,8 @@ extern "C" int cclr_response_ci_tensor(cclr_ctx *ctx, const cclr_c128 *X, int no
     for (int k = 0; k < nomega; ++k)
       for (int r = 0; r < nop; ++r)
         for (int s = 0; s < nop; ++s) {
-          // shift indices: +gamma set: z_k -> k, -conj z_k -> nomega + k;  -gamma set: -z_k -> nomega + k, conj z_k -> k
-          const int jz = k, jzc = nomega + k;
+          // shift indices: +gamma set: z_k -> jz, -conj z_k -> jzc;  -gamma set: -z_k -> jzc, conj z_k -> jz
+          const int jz = idx_pos[k], jzc = idx_neg[k];
           const cplx g0 = C(EP[((size_t)r * nop + s) * ns + jz]) - C(LMr[(size_t)r * ns + jzc]) * C(Lx[s]) +
                           C(EMr[((size_t)s * nop + r) * ns + jzc]) - C(LP[(size_t)s * ns + jz]) * C(Lx[r]);
           const cplx g1 = C(EP[((size_t)r * nop + s) * ns + jzc]) - C(LMr[(size_t)r * ns + jz]) * C(Lx[s]) +

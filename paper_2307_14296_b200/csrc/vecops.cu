@@ -101,6 +101,15 @@ __global__ void __launch_bounds__(256) scale_kernel(c128 *__restrict__ y, c128 a
     y[i] = cmul(alpha, y[i]);
 }
 
+__global__ void __launch_bounds__(256) shifted_copy_kernel(c128 *__restrict__ out, const c128 *__restrict__ src, c128 alpha,
+                                                           const c128 *__restrict__ x, long n) {
+  for (long i = (long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long)gridDim.x * blockDim.x) {
+    c128 acc = src[i];
+    cfma(acc, alpha, x[i]);
+    out[i] = acc;
+  }
+}
+
 __global__ void __launch_bounds__(256) denominators_kernel(const c128 *__restrict__ fock, int o, int v,
                                                            double *__restrict__ D) {
   const long nf = o + v, n1 = (long)o * v, oo = npair(o), n2 = npair(v) * oo;
@@ -170,7 +179,7 @@ __global__ void __launch_bounds__(256) block_lincomb_kernel(const BlockLincombAr
       }
       __syncthreads();
       const int jn = m - j0 < BL_JT ? m - j0 : BL_JT;
-#pragma unroll 2
+#pragma unroll 4
       for (int jj = 0; jj < jn; ++jj) {
         const int j = j0 + jj;
         const c128 *vrow = j < a.m0 ? a.V0 + (size_t)j * a.ldv0 : a.V1 + (size_t)(j - a.m0) * a.ldv1;
@@ -336,5 +345,12 @@ cudaError_t block_lincomb(cudaStream_t st, int R, c128 *Y, long ldy, const c128 
     block_norm_final_kernel<<<1, 32, 0, st>>>(nrm_scratch, grid, R, nrm2);
     cclr_count_launch();
   }
+  return cudaGetLastError();
+}
+
+cudaError_t shifted_copy(cudaStream_t st, c128 *out, const c128 *src, c128 alpha, const c128 *x, long n) {
+  if (n <= 0) return cudaSuccess;
+  shifted_copy_kernel<<<stream_grid(n), 256, 0, st>>>(out, src, alpha, x, n);
+  cclr_count_launch();
   return cudaGetLastError();
 }

@@ -29,5 +29,6 @@ def test_reference_arm_prints_one_json_line_with_the_contract_keys(monkeypatch):
                 "vs_baseline", "dtype", "data", "config", "cpu_baseline", "e2e"):
         assert key in d, key
     assert d["impl"] == "reference" and d["vs_baseline"] is None and d["value"] > 0
+    assert d["steps"] == 2 and d["warmup"] == 1                    # the arm honours --steps / --warmup as given
     assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["cores"] >= 1
     assert d["e2e"]["h2d_bytes_per_step"] == 0 and "workload" in d["config"]
