@@ -55,6 +55,9 @@ typedef struct {
 #define CCLR_GEMM_4M 4u     /* every contraction of this context uses the 4M complex product (default: the large ones use 3M,
                                see cclr_zgemm); a per-context choice, nothing process-wide */
 
+#define CCLR_NO_SUM_PLANES 16u /* do not keep / form the "sum planes" Re + Im that feed the 3M product from global memory (default:
+                               a persistent plane of W_vvvv, 1/2 of its size, when memory allows, and per-call planes of operands
+                               that are small next to the product); without them the sums are formed inside the kernel (~5 % slower) */
 #define CCLR_NO_GRAPH 8u    /* never replay sigma as a CUDA graph (default: contexts with at most 2^21 unique amplitudes capture the sigma
                                plan once and replay it per trial vector -- they are launch bound; results are identical) */
 

@@ -39,6 +39,7 @@ ERI_INPLACE = 1
 SMALL_CHUNKS = 2
 GEMM_4M = 4
 NO_GRAPH = 8
+NO_SUM_PLANES = 16
 
 
 class Context:

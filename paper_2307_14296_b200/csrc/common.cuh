@@ -34,12 +34,22 @@ struct ZgemmWorkspace {
   c128 *buf = nullptr;   // split-K partial sums
   size_t elems = 0;      // capacity in complex elements
   int three_m = 1;       // complex product of the large contractions (M >= 512, N >= 24, K >= 64): 1 = 3M, 0 = 4M everywhere
+  // sum planes of the 3M product (zgemm.cu): scratch for the per-call pre-pass over operands that are small next to the
+  // product, and persistent planes registered for operands that are not (W_vvvv)
+  double *plane = nullptr;
+  size_t plane_elems = 0;
+  const c128 *persist_key[2] = {nullptr, nullptr};     // operand base pointer (unconjugated use, full leading dimension)
+  const double *persist_plane[2] = {nullptr, nullptr};
+  long persist_ld[2] = {0, 0};                         // leading dimension of the operand (complex elements) ...
+  long persist_pld[2] = {0, 0};                        // ... and of its plane (doubles, even)
 };
 // C = alpha * opA(A) * opB(B) + beta * C; see include/cclr.h (cclr_zgemm).  ws may be null (no split-K then).
 cudaError_t zgemm(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *A, long lda, bool conjA,
                   const c128 *B, long ldb, bool b_is_kn, bool conjB, c128 beta, c128 *C, long ldc, int batch = 1,
                   long sa = 0, long sb = 0, long sc = 0, const ZgemmWorkspace *ws = nullptr);
 int zgemm_num_sms();
+// plane[r][c] = Re X[r][c] +- Im X[r][c] (the 3M product's sum operand; see ZgemmWorkspace)
+cudaError_t zgemm_sum_plane(cudaStream_t st, const c128 *X, long ld, long rows, long cols, bool conj, double *plane, long ldp);
 
 // ---- permute.cu: generic index-permutation / pair (un)packing / antisymmetrising gather-scatter kernel ---------
 // dst(iteration index) (+)= sum_k coef_k * sign_k * [conj] src_k(slots(letters)); see plans.inc for the semantics.

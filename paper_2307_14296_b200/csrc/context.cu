@@ -84,6 +84,8 @@ void destroy(cclr_ctx *ctx) {
   if (ctx->st) cudaStreamSynchronize(ctx->st);
   delete ctx->plan;
   if (ctx->ws.buf) cudaFree(ctx->ws.buf);
+  if (ctx->ws.plane) cudaFree(ctx->ws.plane);
+  if (ctx->wplane) cudaFree(ctx->wplane);
   if (ctx->D) cudaFree(ctx->D);
   if (ctx->dot_partial) cudaFree(ctx->dot_partial);
   if (ctx->dot_out) cudaFree(ctx->dot_out);
@@ -202,6 +204,18 @@ extern "C" int cclr_create(int o, int v, const cclr_c128 *fock, const cclr_eri_p
     check(cudaMalloc(&ctx->ws.buf, ctx->ws.elems * sizeof(c128)), "cudaMalloc(split-K workspace)");
     ctx->extra_bytes += ctx->ws.elems * sizeof(c128);
     ctx->ws.three_m = (flags & CCLR_GEMM_4M) ? 0 : 1;
+    if (ctx->ws.three_m && !(flags & CCLR_NO_SUM_PLANES)) {
+      // scratch for the per-call sum planes of the 3M product: both operands of the ring-sized contractions
+      const size_t ov = (size_t)o * v;
+      ctx->ws.plane_elems = 2 * ov * (ov + 1);
+      if (cudaMalloc(&ctx->ws.plane, ctx->ws.plane_elems * sizeof(double)) != cudaSuccess) {
+        cudaGetLastError();
+        ctx->ws.plane = nullptr;
+        ctx->ws.plane_elems = 0;
+      } else {
+        ctx->extra_bytes += ctx->ws.plane_elems * sizeof(double);
+      }
+    }
     P.set_workspace(&ctx->ws);
 
     // borrowed inputs
@@ -241,6 +255,26 @@ extern "C" int cclr_create(int o, int v, const cclr_c128 *fock, const cclr_eri_p
 
     P.execute(CCLR_PLAN_CREATE);
     P.free_class(BUF_TEMP);
+
+    // persistent sum plane of W_vvvv (Re + Im, 8 bytes per element): the ladder's big operand cannot be pre-passed per call
+    // (N = oo is small), so the plane is formed once here -- when it fits comfortably (it is 1/2 of W_vvvv)
+    if (ctx->ws.plane && ctx->vv >= 512 && ctx->oo >= 24) {
+      size_t free_b = 0, total_b = 0;
+      const long pld = (ctx->vv + 1) & ~1L;            // TMA needs 16-byte row strides
+      const size_t bytes = (size_t)ctx->vv * pld * sizeof(double);
+      if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess && free_b > 3 * bytes && cudaMalloc(&ctx->wplane, bytes) == cudaSuccess) {
+        const c128 *W = P.buf(P.find("Wabef")).ptr;
+        check(zgemm_sum_plane(ctx->st, W, ctx->vv, ctx->vv, ctx->vv, false, ctx->wplane, pld), "sum plane of W_vvvv");
+        ctx->ws.persist_key[0] = W;
+        ctx->ws.persist_plane[0] = ctx->wplane;
+        ctx->ws.persist_ld[0] = ctx->vv;
+        ctx->ws.persist_pld[0] = pld;
+        ctx->extra_bytes += bytes;
+      } else {
+        cudaGetLastError();
+        ctx->wplane = nullptr;
+      }
+    }
 
     check(cudaMalloc(&ctx->D, (size_t)(ctx->n1 + ctx->n2) * sizeof(double)), "cudaMalloc(D)");
     ctx->extra_bytes += (size_t)(ctx->n1 + ctx->n2) * sizeof(double);

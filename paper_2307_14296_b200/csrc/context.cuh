@@ -11,6 +11,7 @@ struct cclr_ctx {
   cudaStream_t st = nullptr;
   Plan *plan = nullptr;
   ZgemmWorkspace ws;
+  double *wplane = nullptr;       // persistent sum plane Re + Im of W_vvvv for the 3M ladder (ws.persist_*), or null
   std::vector<ResolvedOp> sigma_ops, ladder_ops, ring_ops, xi_ops, left_ops, eta_ops, eta_eom_ops;
   c128 *xblocks = nullptr;        // X_oo, X_ov, X_vo, X_vv of cclr_xi, contiguous
   int x1_id = -1, x2_id = -1, out1_id = -1, out2_id = -1;

@@ -195,13 +195,18 @@ extern "C" int cclr_zgemm(void *cuda_stream, int M, int N, int K, const cclr_c12
   ZgemmWorkspace ws;
   ws.elems = (size_t)3 * zgemm_num_sms() * 128 * 64;
   ws.three_m = three_m != 0;
+  if (ws.three_m && batch == 1 && M >= 512 && N >= 24 && K >= 64) {   // room for the sum planes of both operands (3M product)
+    ws.plane_elems = ((size_t)M + (size_t)N + 16) * ((size_t)K + 2) + ((size_t)K + 16) * ((size_t)N + 2);
+    if (cudaMalloc(&ws.plane, ws.plane_elems * sizeof(double)) != cudaSuccess) { ws.plane = nullptr; ws.plane_elems = 0; cudaGetLastError(); }
+  }
   if (cudaMalloc(&ws.buf, ws.elems * sizeof(c128)) != cudaSuccess) { ws.buf = nullptr; ws.elems = 0; cudaGetLastError(); }
   cudaError_t e = zgemm(st, M, N, K, make_double2(alpha->re, alpha->im), (const c128 *)A, lda, conj_a != 0,
                         (const c128 *)B, ldb, b_is_kn != 0, conj_b != 0, make_double2(beta->re, beta->im), (c128 *)C,
                         ldc, batch, sa, sb, sc, &ws);
-  if (ws.buf) {
+  if (ws.buf || ws.plane) {
     cudaStreamSynchronize(st);
-    cudaFree(ws.buf);
+    if (ws.buf) cudaFree(ws.buf);
+    if (ws.plane) cudaFree(ws.plane);
   }
   if (e != cudaSuccess) { g_last_cuda_error = e; return CCLR_ECUDA; }
   return CCLR_OK;

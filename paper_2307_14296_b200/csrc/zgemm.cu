@@ -26,6 +26,7 @@
 //     workspace + a deterministic reduce kernel; the same mechanism serves tall-K / tiny-MN contractions), and
 //     matrix-vector kernels for N = 1 / M = 1.
 #include "common.cuh"
+#include <algorithm>
 #include <atomic>
 #include <cmath>
 #include <mutex>
@@ -304,15 +305,26 @@ zgemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CU
 // formed by the idle producer warps (their DADDs starve behind the consumers' DMMAs).  I.e. the cost is the DADDs' presence on
 // the FP64 datapath shared with DMMA, not their latency; only sum planes that arrive from global memory would remove it.
 // ---------------------------------------------------------------------------------------------------------------
-constexpr int Z3_BM = 128, Z3_BK = 16, Z3_STAGES = 4, Z3_WM = 32, Z3_NCW = 8;
+// PL = true: the sums arrive from GLOBAL memory as "sum planes" (one double Re + Im per complex element, conjugation applied;
+// a persistent plane registered for the operand, or a pre-pass of zgemm() over an operand that is small next to the product):
+// TMA stages them beside the tiles ([rows][8 doubles] boxes, SWIZZLE_64B, conflict-free LDS.64), the main loop has no DADD at
+// all, and 3 stages of [A | B | SA | SB] replace the 4 stages of [A | B] (two stages already hide the TMA latency).
+constexpr int Z3_BM = 128, Z3_BK = 16, Z3_WM = 32, Z3_NCW = 8;
+__device__ __forceinline__ double lds64(uint32_t addr) {
+  double v;
+  asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
+  return v;
+}
 
-template <int BN, bool BKN>
+template <int BN, bool BKN, bool PL>
 __global__ void __launch_bounds__(Z3_NCW * 32 + 128, 1)
-zgemm3m_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const ZgemmArgs p) {
-  constexpr int BM = Z3_BM, BK = Z3_BK, STAGES = Z3_STAGES, WM = Z3_WM, NCW = Z3_NCW;
+zgemm3m_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
+               const __grid_constant__ CUtensorMap tmSA, const __grid_constant__ CUtensorMap tmSB, const ZgemmArgs p) {
+  constexpr int BM = Z3_BM, BK = Z3_BK, STAGES = PL ? 3 : 4, WM = Z3_WM, NCW = Z3_NCW;
   constexpr int WN = BN / 2, WARPS_N = 2, MI = WM / 8, NG3 = WN / 8;
-  constexpr int A_BYTES = BM * BK * 16, B_BYTES = BN * BK * 16, STAGE_BYTES = A_BYTES + B_BYTES;
-  static_assert(BN % 16 == 0, "3M tile shape");
+  constexpr int A_BYTES = BM * BK * 16, B_BYTES = BN * BK * 16, SA_BYTES = PL ? BM * BK * 8 : 0, SB_BYTES = PL ? BN * BK * 8 : 0;
+  constexpr int STAGE_BYTES = A_BYTES + B_BYTES + SA_BYTES + SB_BYTES;
+  static_assert(BN % 16 == 0 && STAGE_BYTES % 1024 == 0, "3M tile shape");
 
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -370,6 +382,18 @@ zgemm3m_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
           for (int nb = 0; nb < BN / 8; ++nb) // B boxes: [BK rows][8 complex]
             tma_load_3d(sB + nb * (BK * 128), &tmB, 2 * (tile_n * BN + nb * 8), k0, batch, full);
         }
+        if (PL) {   // sum planes: [rows][8 doubles] boxes
+          const uint32_t sSA = sB + B_BYTES, sSB = sSA + SA_BYTES;
+#pragma unroll
+          for (int kb = 0; kb < BK / 8; ++kb) tma_load_3d(sSA + kb * (BM * 64), &tmSA, k0 + kb * 8, tile_m * BM, 0, full);
+          if (!BKN) {
+#pragma unroll
+            for (int kb = 0; kb < BK / 8; ++kb) tma_load_3d(sSB + kb * (BN * 64), &tmSB, k0 + kb * 8, tile_n * BN, 0, full);
+          } else {
+#pragma unroll
+            for (int nb = 0; nb < BN / 8; ++nb) tma_load_3d(sSB + nb * (BK * 64), &tmSB, tile_n * BN + nb * 8, k0, 0, full);
+          }
+        }
       }
     }
     return;
@@ -381,13 +405,17 @@ zgemm3m_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   const int rmap = ((gid & 1) << 2) | (gid >> 1);   // row / column permutation inside an 8-group (bank-conflict free)
   const int wm = warp / WARPS_N, wn = warp % WARPS_N;
   const uint32_t sa3 = p.conjA ? 0x80000000u : 0u, sb3 = p.conjB ? 0x80000000u : 0u;
-  uint32_t a_off[2], b_off[2];
+  uint32_t a_off[2], b_off[2], sa_off[2], sb_off[2];
 #pragma unroll
   for (int s4 = 0; s4 < 2; ++s4) {
     const int k = 4 * s4 + tig;
     a_off[s4] = (uint32_t)((wm * WM + rmap) * 128 + ((k ^ rmap) << 4));
     b_off[s4] = !BKN ? (uint32_t)((wn * WN + rmap) * 128 + ((k ^ rmap) << 4))
                      : (uint32_t)(((wn * WN) >> 3) * (BK * 128) + k * 128 + ((rmap ^ k) << 4));
+    // sum planes under SWIZZLE_64B: 16-byte chunk index ^= bits 7-8 of the address = (row >> 1) & 3 for 64-byte rows
+    sa_off[s4] = (uint32_t)((wm * WM + rmap) * 64 + (((k >> 1) ^ ((rmap >> 1) & 3)) << 4) + (k & 1) * 8);
+    sb_off[s4] = !BKN ? (uint32_t)((wn * WN + rmap) * 64 + (((k >> 1) ^ ((rmap >> 1) & 3)) << 4) + (k & 1) * 8)
+                      : (uint32_t)(((wn * WN) >> 3) * (BK * 64) + k * 64 + (((rmap >> 1) ^ ((k >> 1) & 3)) << 4) + (rmap & 1) * 8);
   }
   double acc[MI][NG3][3][2];
 #pragma unroll
@@ -400,7 +428,7 @@ zgemm3m_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     const int s = c % STAGES;
     const uint32_t ph = (c / STAGES) & 1;
     mbar_wait(bar_base + 8 * s, ph);
-    const uint32_t sA = smem_base + s * STAGE_BYTES, sB = sA + A_BYTES;
+    const uint32_t sA = smem_base + s * STAGE_BYTES, sB = sA + A_BYTES, sSA = sB + B_BYTES, sSB = sSA + SA_BYTES;
 #pragma unroll
     for (int kb = 0; kb < BK / 8; ++kb) {
 #pragma unroll
@@ -411,14 +439,16 @@ zgemm3m_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
           const double2 a = lds128(sA + kb * (BM * 128) + a_off[s4] + i * 1024);
           ar[i] = a.x;
           ai[i] = flip_sign(a.y, sa3);
-          as[i] = ar[i] + ai[i];
+          as[i] = PL ? lds64(sSA + kb * (BM * 64) + sa_off[s4] + i * 512) : ar[i] + ai[i];
         }
 #pragma unroll
         for (int g = 0; g < NG3; ++g) {
           const uint32_t addr = !BKN ? sB + kb * (BN * 128) + g * 1024 + b_off[s4]
                                      : sB + g * (BK * 128) + kb * 1024 + b_off[s4];
           const double2 b = lds128(addr);
-          const double br = b.x, bi = flip_sign(b.y, sb3), bs = br + bi;
+          const double br = b.x, bi = flip_sign(b.y, sb3);
+          const double bs = PL ? lds64(!BKN ? sSB + kb * (BN * 64) + g * 512 + sb_off[s4] : sSB + g * (BK * 64) + kb * 512 + sb_off[s4])
+                               : br + bi;
 #pragma unroll
           for (int i = 0; i < MI; ++i) dmma884(acc[i][g][0][0], acc[i][g][0][1], ar[i], br);
 #pragma unroll
@@ -496,6 +526,34 @@ EncodeTiledFn get_encode() {
   return fn;
 }
 
+// plane[r][c] = Re X[r][c] + (conj ? -1 : +1) Im X[r][c]  (the A_r + A_i / B_r + B_i operand of the 3M product)
+__global__ void __launch_bounds__(256) sum_plane_kernel(const c128 *__restrict__ X, long ld, long rows, long cols, int conj,
+                                                        double *__restrict__ plane, long ldp) {
+  const double sg = conj ? -1.0 : 1.0;
+  for (long r = blockIdx.y; r < rows; r += gridDim.y) {
+    const c128 *x = X + r * ld;
+    double *d = plane + r * ldp;
+    for (long c = (long)blockIdx.x * blockDim.x + threadIdx.x; c < cols; c += (long)gridDim.x * blockDim.x) {
+      const c128 v = x[c];
+      d[c] = v.x + sg * v.y;
+    }
+  }
+}
+
+// tensor map over a [rows][cols doubles] sum plane, box = [box_rows][8 doubles = 64 B], SWIZZLE_64B
+bool make_plane_map(CUtensorMap *tm, const double *base, long cols, long rows, long ldp, int box_rows) {
+  EncodeTiledFn enc = get_encode();
+  if (!enc || (ldp & 1)) return false;
+  cuuint64_t dims[3] = {(cuuint64_t)cols, (cuuint64_t)rows, 1};
+  cuuint64_t strides[2] = {(cuuint64_t)ldp * 8ull, (cuuint64_t)ldp * (cuuint64_t)rows * 8ull};
+  cuuint32_t box[3] = {8u, (cuuint32_t)box_rows, 1u};
+  cuuint32_t es[3] = {1u, 1u, 1u};
+  CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, (void *)base, dims, strides, box, es,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS;
+}
+
 // tensor map over a [rows][inner complex] (x batch) operand viewed as FLOAT64, box = [box_rows][8 complex = 128 B]
 bool make_map(CUtensorMap *tm, const c128 *base, long inner_complex, long rows, long ld, int batch, long stride,
               int box_rows) {
@@ -549,18 +607,20 @@ cudaError_t launch_ng(cudaStream_t st, const CUtensorMap &tmA, const CUtensorMap
             : launch<64, 8 * NG, ZG_BK, 16, 4 * NG, ZG_STAGES, false>(st, tmA, tmB, args, ctas);
 }
 
-// 3M kernel: 128 x BN tiles, BN = 32 | 48
-template <int BN, bool BKN>
-cudaError_t launch_3m(cudaStream_t st, const CUtensorMap &tmA, const CUtensorMap &tmB, const ZgemmArgs &args, int ctas) {
+// 3M kernel: 128 x BN tiles, BN = 32 | 48; PL: with sum planes from global memory
+template <int BN, bool BKN, bool PL>
+cudaError_t launch_3m(cudaStream_t st, const CUtensorMap &tmA, const CUtensorMap &tmB, const CUtensorMap &tmSA,
+                      const CUtensorMap &tmSB, const ZgemmArgs &args, int ctas) {
   constexpr int threads = Z3_NCW * 32 + 128;
-  constexpr int smem = Z3_STAGES * (Z3_BM + BN) * Z3_BK * 16 + 2 * Z3_STAGES * 8 + 1024;
-  auto kern = zgemm3m_kernel<BN, BKN>;
+  constexpr int stages = PL ? 3 : 4;
+  constexpr int smem = stages * (Z3_BM + BN) * Z3_BK * (PL ? 24 : 16) + 2 * stages * 8 + 1024;
+  auto kern = zgemm3m_kernel<BN, BKN, PL>;
   static std::atomic<unsigned long long> configured{0};
   unsigned long long mask = configured.load();
   const cudaError_t e = configure_smem((const void *)kern, smem, mask);
   if (e != cudaSuccess) return e;
   configured.fetch_or(mask);
-  kern<<<ctas, threads, smem, st>>>(tmA, tmB, args);
+  kern<<<ctas, threads, smem, st>>>(tmA, tmB, tmSA, tmSB, args);
   cclr_count_launch();
   return cudaGetLastError();
 }
@@ -662,6 +722,14 @@ __global__ void __launch_bounds__(256) zgemv_kernel(int M, int K, c128 alpha, co
 }
 
 }  // namespace
+
+cudaError_t zgemm_sum_plane(cudaStream_t st, const c128 *X, long ld, long rows, long cols, bool conj, double *plane, long ldp) {
+  if (rows <= 0 || cols <= 0) return cudaSuccess;
+  dim3 grid((unsigned)std::min<long>((cols + 255) / 256, 64), (unsigned)std::min<long>(rows, 32768));
+  sum_plane_kernel<<<grid, 256, 0, st>>>(X, ld, rows, cols, conj ? 1 : 0, plane, ldp);
+  cclr_count_launch();
+  return cudaGetLastError();
+}
 
 int zgemm_num_sms() {
   static std::atomic<int> cache[64];   // per device ordinal (zero-initialised)
@@ -800,7 +868,45 @@ cudaError_t zgemm(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *
   const int tail_tiles = (int)tiles - main_tiles;
   const int ctas = main_tiles + tail_tiles * splits;
 
+  // ---- 3M: sum planes Re + Im of both operands from global memory, when they can be had cheaply ----
+  // an operand's plane is either registered (persistent, unconjugated use) or formed here by a streaming pre-pass, which pays
+  // when the operand is small next to the product (the other output dimension >= 2048: < 1.2 % of the GEMM's time)
+  CUtensorMap tmSA, tmSB;
+  bool planes = false;
+  if (use3m && batch == 1 && ws) {
+    const double *pa = nullptr, *pb = nullptr;
+    long ldpa = 0, ldpb = 0;
+    for (int q = 0; q < 2; ++q) {
+      if (ws->persist_key[q] == A && !conjA && ws->persist_ld[q] == lda) { pa = ws->persist_plane[q]; ldpa = ws->persist_pld[q]; }
+      if (ws->persist_key[q] == B && !conjB && ws->persist_ld[q] == ldb) { pb = ws->persist_plane[q]; ldpb = ws->persist_pld[q]; }
+    }
+    const long rowsB = b_is_kn ? K : N, colsB = b_is_kn ? N : K;
+    const long ldsa = (K + 1) & ~1L, ldsb = (colsB + 1) & ~1L;
+    size_t need = 0;
+    const bool preA = !pa && N >= 2048, preB = !pb && M >= 2048;
+    if (preA) need += (size_t)M * ldsa;
+    if (preB) need += (size_t)rowsB * ldsb;
+    if ((pa || preA) && (pb || preB) && need <= ws->plane_elems) {
+      double *scratch = ws->plane;
+      if (preA) {
+        dim3 grid((unsigned)std::min<long>((K + 255) / 256, 64), (unsigned)std::min<long>(M, 32768));
+        sum_plane_kernel<<<grid, 256, 0, st>>>(A, lda, M, K, conjA ? 1 : 0, scratch, ldsa);
+        cclr_count_launch();
+        pa = scratch; ldpa = ldsa;
+        scratch += (size_t)M * ldsa;
+      }
+      if (preB) {
+        dim3 grid((unsigned)std::min<long>((colsB + 255) / 256, 64), (unsigned)std::min<long>(rowsB, 32768));
+        sum_plane_kernel<<<grid, 256, 0, st>>>(B, ldb, rowsB, colsB, conjB ? 1 : 0, scratch, ldsb);
+        cclr_count_launch();
+        pb = scratch; ldpb = ldsb;
+      }
+      planes = make_plane_map(&tmSA, pa, K, M, ldpa, BM) &&
+               (b_is_kn ? make_plane_map(&tmSB, pb, N, K, ldpb, BK) : make_plane_map(&tmSB, pb, K, N, ldpb, BN));
+    }
+  }
   CUtensorMap tmA, tmB;
+  if (!planes) { tmSA = CUtensorMap{}; tmSB = CUtensorMap{}; }
   if (!make_map(&tmA, A, K, M, lda, batch, sa, BM)) return cudaErrorInvalidValue;
   if (!b_is_kn) {
     if (!make_map(&tmB, B, K, N, ldb, batch, sb, BN)) return cudaErrorInvalidValue;
@@ -809,8 +915,11 @@ cudaError_t zgemm(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *
   }
   cudaError_t e;
   if (use3m) {
-    if (NG3 == 2) e = b_is_kn ? launch_3m<32, true>(st, tmA, tmB, args, ctas) : launch_3m<32, false>(st, tmA, tmB, args, ctas);
-    else e = b_is_kn ? launch_3m<48, true>(st, tmA, tmB, args, ctas) : launch_3m<48, false>(st, tmA, tmB, args, ctas);
+#define CCLR_L3M(BN_, KN_) (planes ? launch_3m<BN_, KN_, true>(st, tmA, tmB, tmSA, tmSB, args, ctas) \
+                                   : launch_3m<BN_, KN_, false>(st, tmA, tmB, tmSA, tmSB, args, ctas))
+    if (NG3 == 2) e = b_is_kn ? CCLR_L3M(32, true) : CCLR_L3M(32, false);
+    else e = b_is_kn ? CCLR_L3M(48, true) : CCLR_L3M(48, false);
+#undef CCLR_L3M
   } else
   switch (NG) {
     case 4: e = launch_ng<4>(st, tmA, tmB, args, ctas, b_is_kn, BM); break;

@@ -84,6 +84,9 @@ def test_zgemm_matches_numpy(M, N, K, kn, ca, cb, beta):
     (513, 24, 64, True, True, False, 0.5), (1300, 561, 96, True, False, False, 0.0),
     (1300, 153, 200, False, False, True, -1.0), (5120, 276, 200, True, False, False, 1.0),
     (700, 10200 // 8, 130, False, False, False, 0.0),
+    # both output dimensions >= 2048: the 3M kernel is fed with sum planes Re + Im formed by a pre-pass (even / odd K, conj)
+    (2100, 2060, 130, False, False, False, 0.0), (2100, 2060, 131, True, True, False, 1.0),
+    (2304, 2100, 96, True, False, True, 0.5), (2050, 2049, 77, False, True, True, 0.0),
 ])
 def test_zgemm_3m_and_4m_modes_match_numpy(M, N, K, kn, ca, cb, beta):
     """The large-contraction path in both complex-product modes (3M: three real DMMA products per complex one; 4M: four),
