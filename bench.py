@@ -166,23 +166,22 @@ def workload_name(cfg, o, v):
 
 
 def measured_ladder_traffic(gemm, config):
-    """DRAM bytes of one ladder launch from an ncu capture of THIS build (profiles/r02_ncu_traffic.json, written from
-    `ncu --set full`; keyed by the sha1 of csrc/zgemm.cu): (bytes, source) or (None, why)."""
-    path = os.path.join(ROOT, "profiles", "r02_ncu_traffic.json")
+    """DRAM bytes of one ladder launch from an ncu capture of THIS build: profiles/r02_ncu_traffic.csv (rows: sha1 of
+    csrc/zgemm.cu, complex product, config, kernel, dram__bytes_read.sum + dram__bytes_write.sum; the command that made it is in
+    profiles/r02_ncu_traffic.md).  Returns (bytes, source) or (None, why): the run itself cannot measure DRAM traffic."""
+    path = os.path.join(ROOT, "profiles", "r02_ncu_traffic.csv")
     src = os.path.join(ROOT, "paper_2307_14296_b200", "csrc", "zgemm.cu")
     try:
-        with open(path) as fh:
-            rec = json.load(fh)
         with open(src, "rb") as fh:
             sha = hashlib.sha1(fh.read()).hexdigest()
-    except (OSError, ValueError):
+        with open(path) as fh:
+            rows = [line.strip().split(",") for line in fh if line.strip() and not line.startswith("#")]
+    except OSError:
         return None, "no ncu capture of this build under profiles/"
-    if rec.get("zgemm_cu_sha1") != sha:
-        return None, "profiles/r02_ncu_traffic.json was captured on another build of csrc/zgemm.cu"
-    val = rec.get("ladder", {}).get("%s:%d" % (gemm, config))
-    if val is None:
-        return None, "profiles/r02_ncu_traffic.json has no capture for this config / product"
-    return float(val), "profiles/r02_ncu_traffic.json (%s): dram__bytes_read.sum + dram__bytes_write.sum of the ladder launch" % rec.get("command", "ncu --set full")
+    for r in rows:
+        if len(r) >= 5 and r[0] == sha and r[1] == gemm and r[2] == str(config) and r[3] == "ladder":
+            return float(r[4]), "profiles/r02_ncu_traffic.csv: dram__bytes_read.sum + dram__bytes_write.sum of the ladder launch, ncu capture of this build"
+    return None, "profiles/r02_ncu_traffic.csv has no capture of this build of csrc/zgemm.cu for this config / product"
 
 
 # ---------------------------------------------------------------------------------------------------------------

@@ -772,7 +772,11 @@ cudaError_t zgemm(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *
   // 3M complex product (3 real DMMA products per complex one instead of 4) for the large contractions; the 4M kernel keeps
   // the small and skinny ones, where tile padding, not the DMMA count, is the cost
   const bool use3m = (!ws || ws->three_m) && M >= 512 && N >= 24 && K >= 64;
-  const int BM = use3m ? 128 : ((pad64 * 10 <= pad128 * 9) ? 64 : 128);
+  // "skinny" reductions of the solver (Gram blocks b^H sigma, Gram-Schmidt projections: a few rows and columns, K = the whole
+  // amplitude vector): 32 x 8 tiles and an 8-deep ring keep the padding waste and the bytes in flight where HBM, not the
+  // tensor pipe, is the limit
+  const bool skinny = !use3m && !b_is_kn && batch == 1 && N <= 16 && M <= 256 && K >= 65536;
+  const int BM = use3m ? 128 : skinny ? 32 : ((pad64 * 10 <= pad128 * 9) ? 64 : 128);
   if (batch > 1 && (sa == 0 || sb == 0)) {   // a shared operand has no batch stride a tensor map could carry: one launch per batch
     for (int b = 0; b < batch; ++b) {
       const cudaError_t e = zgemm(st, M, N, K, alpha, A + (size_t)b * sa, lda, conjA, B + (size_t)b * sb, ldb, b_is_kn, conjB, beta,
@@ -828,7 +832,7 @@ cudaError_t zgemm(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *
     const long p48 = (N + 47L) / 48 * 48, p32 = (N + 31L) / 32 * 32;
     NG3 = (p32 * 100 < p48 * 99) ? 2 : 3;
   }
-  const int BN = use3m ? 16 * NG3 : 8 * NG;
+  const int BN = use3m ? 16 * NG3 : skinny ? 8 : 8 * NG;
   ZgemmArgs args{};
   args.M = M; args.N = N; args.K = K;
   args.C = C; args.ldc = ldc; args.sc = sc;
@@ -920,6 +924,8 @@ cudaError_t zgemm(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *
     if (NG3 == 2) e = b_is_kn ? CCLR_L3M(32, true) : CCLR_L3M(32, false);
     else e = b_is_kn ? CCLR_L3M(48, true) : CCLR_L3M(48, false);
 #undef CCLR_L3M
+  } else if (skinny) {
+    e = launch<32, 8, ZG_BK, 8, 8, 8, false>(st, tmA, tmB, args, ctas);
   } else
   switch (NG) {
     case 4: e = launch_ng<4>(st, tmA, tmB, args, ctas, b_is_kn, BM); break;

@@ -184,9 +184,14 @@ def test_solver_bandwidth_kernels_match_numpy(cfg1):
         assert np.abs(nrm.cpu().numpy() - (np.abs(want) ** 2).sum(1)).max() <= 1e-13 * (np.abs(want) ** 2).sum(1).max()
         wp = want / (z[:, None] - D[None, :])
         assert np.abs(P.cpu().numpy() - wp).max() <= 1e-13 * np.abs(wp).max()
-    big = 6000                                                   # long enough for the GEMM dot path
+    for big, na, nb in [(6000, 5, 3), (70001, 37, 6), (66000, 3, 2)]:   # GEMM dot path; long vectors: the 32 x 8 "skinny" tiles, ragged
+        A, B = cplx(na, big), cplx(nb, big)
+        got = np.array(cc.cclr_vec_dots(ctx, torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda()))
+        want = A.conj() @ B.T
+        assert np.abs(got - want).max() <= 1e-13 * np.abs(want).max(), (big, na, nb)
+    big = 6000
     A, B = cplx(5, big), cplx(3, big)
-    for (a, b) in [(A, B), (A, B[:1]), (A[:1], B)]:
+    for (a, b) in [(A, B[:1]), (A[:1], B)]:
         got = np.array(cc.cclr_vec_dots(ctx, torch.from_numpy(np.ascontiguousarray(a)).cuda(), torch.from_numpy(np.ascontiguousarray(b)).cuda()))
         want = a.conj() @ b.T
         assert np.abs(got - want).max() <= 1e-13 * np.abs(want).max()
