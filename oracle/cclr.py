@@ -247,6 +247,58 @@ class CCLR:
 
         return (4 * D(0.5) - D(1.0)) / 3 / (hx * hy)
 
+    def F_transform(self, lam1, lam2, y1, y2):
+        """(F y)_nu = <Lambda|[[Hbar, tau_nu], Y]|R> (F of Table 1; "only t.F is formed") as the
+        derivative of the left transform along y:  F y = d/db [eta0 + lambda A](t + b y)|0.  eta0 and every term of sigma_left
+        are linear in the intermediates of S-Eq. 15-28, so this is sigma_left with each intermediate replaced by its derivative
+        (product rule on S-Eq. 15-28, term by term in the order of __init__), plus the terms in which t2 appears explicitly
+        (GL, GO of T3, T4, T9, T10).  The printed S-Eq. 8 ff. are unusable (reading 6); pinned
+        against the determinant-space F and against xFy.  Result laid out like amplitudes."""
+        I, t1, t2 = self.I, self.t1, self.t2
+        E = np.einsum
+        vovv = -I.ovvv.transpose(1, 0, 2, 3)
+        oovo = -I.ooov.transpose(0, 1, 3, 2)
+        yt = E("ai,bj->abij", y1, t1) + E("ai,bj->abij", t1, y1)
+        dtau = y2 + yt - yt.transpose(1, 0, 2, 3)                                              # d S-Eq. 28
+        dFme = E("mnef,fn->me", I.oovv, y1)                                                     # d S-Eq. 17
+        dFmi = E("me,ei->mi", I.fov, y1) + E("mnie,en->mi", I.ooov, y1) + 0.5 * E("mnef,efin->mi", I.oovv, dtau)
+        dFae = -E("am,me->ae", y1, I.fov) + E("fm,amef->ae", y1, vovv) - 0.5 * E("afmn,mnef->ae", dtau, I.oovv)
+        dWmnij = _Pij(E("ej,mnie->mnij", y1, I.ooov)) + 0.5 * E("efij,mnef->mnij", dtau, I.oovv)
+        dWabef = -_Pab(E("bm,amef->abef", y1, vovv)) + 0.5 * E("abmn,mnef->abef", dtau, I.oovv)
+        dWbar = -E("bfnj,mnef->mbej", y2, I.oovv)
+        dWmbej = (E("fj,mbef->mbej", y1, I.ovvv) - E("bn,mnej->mbej", y1, oovo)
+                  - E("fbjn,mnef->mbej", y2 + E("fj,bn->fbjn", y1, t1) + E("fj,bn->fbjn", t1, y1), I.oovv))
+        dWmnie = E("fi,mnfe->mnie", y1, I.oovv)
+        dWamef = -E("an,nmef->amef", y1, I.oovv)
+        dWmbij = (-E("me,beij->mbij", dFme, t2) - E("me,beij->mbij", self.Fme, y2)
+                  - E("bn,mnij->mbij", y1, self.Wmnij) - E("bn,mnij->mbij", t1, dWmnij)
+                  + 0.5 * E("mbef,efij->mbij", I.ovvv, dtau)
+                  + _Pij(E("mnie,bejn->mbij", I.ooov, y2))
+                  + _Pij(E("ei,mbej->mbij", y1, self.Wbar)) + _Pij(E("ei,mbej->mbij", t1, dWbar)))
+        dWabej = (-E("me,abmj->abej", dFme, t2) - E("me,abmj->abej", self.Fme, y2)
+                  + E("fj,abef->abej", y1, self.Wabef) + E("fj,abef->abej", t1, dWabef)
+                  + 0.5 * E("mnej,abmn->abej", oovo, dtau)
+                  - _Pab(E("mbef,afmj->abej", I.ovvv, y2))
+                  - _Pab(E("am,mbej->abej", y1, self.Wbar)) - _Pab(E("am,mbej->abej", t1, dWbar)))
+        GL, GO = E("abij,afij->bf", lam2, t2), E("abij,abin->jn", lam2, t2)
+        dGL, dGO = E("abij,afij->bf", lam2, y2), E("abij,abin->jn", lam2, y2)
+        L1 = (dFme.T                                                                              # d eta0
+              + E("ai,ae->ei", lam1, dFae) - E("ai,mi->am", lam1, dFmi) + E("ai,maei->em", lam1, dWmbej)
+              - 0.5 * E("abij,mbij->am", lam2, dWmbij) + 0.5 * E("abij,abej->ei", lam2, dWabej)
+              + 0.5 * E("bf,bmfe->em", GL, dWamef) - 0.5 * E("jn,nmje->em", GO, dWmnie)
+              + 0.5 * E("bf,bmfe->em", dGL, self.Wamef) - 0.5 * E("jn,nmje->em", dGO, self.Wmnie))
+        L2 = _Pab(_Pij(E("ai,me->aeim", lam1, dFme)))
+        L2 += _Pij(E("ai,amef->efim", lam1, dWamef))
+        L2 -= _Pab(E("ai,mnie->aemn", lam1, dWmnie))
+        L2 += _Pab(E("abij,be->aeij", lam2, dFae))
+        L2 -= _Pij(E("abij,mj->abim", lam2, dFmi))
+        L2 += 0.5 * E("abij,mnij->abmn", lam2, dWmnij)
+        L2 += _Pab(_Pij(E("abij,mbej->aeim", lam2, dWmbej)))
+        L2 -= 0.5 * _Pab(E("af,nmfe->eamn", dGL, I.oovv))
+        L2 -= 0.5 * _Pij(E("in,nmfe->feim", dGO, I.oovv))
+        L2 += 0.5 * E("abij,abef->efij", lam2, dWabef)
+        return L1, L2
+
     # ---- response equations and functions ---------------------------------------------------------------------
     def solve_dense(self, A, xi1, xi2, z):
         """t(z) = -(A - z)^-1 xi  (Eq. 19-21) by dense LU."""

@@ -389,3 +389,19 @@ def run_omega(o, v, fock, packed, t1, t2p, chunk_override=None):
     it.bind("fvv", "ae", fock[o:, o:])
     it.run(load_plan("CCLR_PLAN_OMEGA"))
     return it.get("om1").copy(), it.get("om2").copy()
+
+
+def run_fy(it, packed, l1, l2p, y1, y2p):
+    """Execute CCLR_PLAN_FY (after run_sigma and run_sigma_left have declared the shared work buffers): out = F y for the
+    multipliers (l1, l2) and the vector (y1, y2), with the caller's bare ooov / oovv / ovvo / ovvv bound again (vvvv is not)."""
+    o, v = it.o, it.v
+    for name, spec in (("ooov", "(mn)ie"), ("oovv", "(mn)(ef)"), ("ovvo", "mbej"), ("ovvv", "mb(ef)")):
+        it.bind(name, spec, packed[name])
+    it.bind("x1", "ai", l1)
+    it.bind("x2", "(ab)(ij)", l2p)
+    it.bind("y1", "ai", y1)
+    it.bind("y2", "(ab)(ij)", y2p)
+    it.bind("out1", "ai", np.zeros(v * o, complex))
+    it.bind("out2", "(ab)(ij)", np.zeros(npair(v) * npair(o), complex))
+    it.run(load_plan("CCLR_PLAN_FY"))
+    return it.get("out1").copy(), it.get("out2").copy()

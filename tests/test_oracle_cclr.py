@@ -152,6 +152,30 @@ def test_xi_eta_lambda_F_match_definitions(small_lr, o, v):
     assert abs(flat(*x) @ F @ flat(*y) - c.xFy(l1, l2, *x, *y)) < 1e-11
 
 
+@pytest.mark.parametrize("o,v", [(2, 4), (3, 4), (2, 5)])
+def test_F_transform_is_the_determinant_space_F_times_y(o, v):
+    """oracle.cclr.CCLR.F_transform (differentiated intermediates) against the literal F_mu,nu = <Lambda|[[Hbar,tau_mu],tau_nu]|R>
+    of Table 1 built in the determinant space, at random UNCONVERGED complex t and lambda and a non-diagonal Fock
+    matrix (the identity F y = d/db [eta0 + lambda A](t + b y) holds for any t, lambda), every element; plus symmetry
+    x.(F y) = y.(F x) and agreement with the Richardson second derivative of the Lagrangian (xFy)."""
+    f, V = random_system(o, v, seed=31 + v, diag_fock=False)
+    t1, t2 = random_amplitudes(o, v, seed=32)
+    l1, l2 = random_amplitudes(o, v, seed=33, scale=1.0)
+    ints = ccsd.Integrals.from_full(f, V, o)
+    c = cclr.CCLR(ints, t1, t2)
+    bf = bruteforce.BruteForce(f, V, o)
+    F = bf.F(t1, t2, flat(l1, l2))
+    for seed in (34, 35):
+        y = random_amplitudes(o, v, seed, scale=1.0)
+        got = flat(*c.F_transform(l1, l2, *y))
+        want = F @ flat(*y)
+        assert np.abs(got - want).max() < 1e-11 * max(1.0, np.abs(want).max())
+    x, y = random_amplitudes(o, v, 36, scale=1.0), random_amplitudes(o, v, 37, scale=1.0)
+    xFy = cclr.dot(*x, *c.F_transform(l1, l2, *y))
+    assert abs(xFy - cclr.dot(*y, *c.F_transform(l1, l2, *x))) < 1e-11 * abs(xFy)
+    assert abs(xFy - c.xFy(l1, l2, *x, *y)) < 1e-10 * abs(xFy)
+
+
 @pytest.mark.parametrize("z", [0.0, 0.0773, 0.0773 + 0.0045j, 0.83 + 0.0045j])
 def test_two_electron_response_functions_equal_exact_sum_over_states(small_lr, z):
     """CCSD is FCI for two electrons: CC-CC (Eq. 15), CC-CI (Eq. 16) and the exact SOS (Eq. 23-24) coincide;

@@ -115,3 +115,27 @@ def test_omega_plan_reproduces_oracle_residual(o, v, chunk):
     r1, r2 = packing.pack_amplitudes(*ccsd.residual(ints, t1, t2))
     assert np.abs(s1.reshape(-1) - r1.reshape(-1)).max() <= 1e-12 * max(1.0, np.abs(r1).max())
     assert np.abs(s2.reshape(-1) - r2.reshape(-1)).max() <= 1e-12 * max(1.0, np.abs(r2).max())
+
+
+@pytest.mark.parametrize("o,v,chunk", [(3, 5, None), (4, 6, 2), (2, 7, 3)])
+def test_fy_plan_reproduces_oracle_F_transform(o, v, chunk):
+    """The direct F-contraction plan (CCLR_PLAN_FY: derivative of the left transform along y, the two o^2 v^4-sized derivative
+    intermediates contracted from the lambda side) against oracle.cclr.CCLR.F_transform, which is pinned by the determinant-space F
+    (tests/test_oracle_cclr.py); random unconverged t, random lambda, non-diagonal Fock matrix, every element."""
+    f, V = random_system(o, v, seed=110 + v, diag_fock=False)
+    t1, t2 = random_amplitudes(o, v, seed=111)
+    ints = ccsd.Integrals.from_full(f, V, o)
+    full = dict(oooo=ints.oooo, ooov=ints.ooov, oovv=ints.oovv, ovvo=ints.ovvo, ovvv=ints.ovvv, vvvv=ints.vvvv)
+    packed = packing.pack_eri(full)
+    it = plan_interp.run_create(o, v, f, packed, *packing.pack_amplitudes(t1, t2), chunk)
+    c = cclr.CCLR(ints, t1, t2)
+    l1, l2 = random_amplitudes(o, v, seed=112, scale=1.0)
+    lp = packing.pack_amplitudes(l1, l2)
+    plan_interp.run_sigma(it, *lp, 0.0)               # declare the shared work buffers
+    plan_interp.run_sigma_left(it, *lp, 0.0)
+    for seed in (113, 114):
+        y1, y2 = random_amplitudes(o, v, seed=seed, scale=1.0)
+        s1, s2 = plan_interp.run_fy(it, packed, *lp, *packing.pack_amplitudes(y1, y2))
+        r1, r2 = packing.pack_amplitudes(*c.F_transform(l1, l2, y1, y2))
+        assert np.linalg.norm(s1.reshape(-1) - r1.reshape(-1)) <= 1e-12 * np.linalg.norm(r1)
+        assert np.linalg.norm(s2.reshape(-1) - r2.reshape(-1)) <= 1e-12 * np.linalg.norm(r2)
