@@ -139,22 +139,32 @@ int cclr_response_ci(cclr_ctx *ctx, const cclr_c128 *X, const cclr_c128 *Y, doub
 int cclr_response_ci_tensor(cclr_ctx *ctx, const cclr_c128 *X, int nop, const double *omegas, int nomega, double gamma, double tol,
                             int maxiter, cclr_c128 *result, cclr_solve_info *info);
 
-/* x . F . y with the CC Hessian F of Table 1 (S-Eq. 8) for amplitude-shaped device vectors x, y and
- * the ground-state multipliers: F is never formed; the contraction is the exact derivative
+/* out_k = F y_k for nvec amplitude-shaped device vectors y_k [nvec][v*o], [nvec][vv*oo] and the multipliers lam1, lam2:
+ * (F y)_nu = <Lambda| [[Hbar, tau_nu], Y] |R>, F = the CC Hessian of Table 1 (S-Eq. 8).  F is never
+ * formed, only its contraction with a vector.  The printed contraction formulas are
+ * unrecoverable (reading 6); the routine evaluates the derivative of the left transform along y,
+ * F y = d/db [eta0 + lambda A](t + b y)|_0, as one contraction plan over the context's dressed intermediates (csrc/plans.inc,
+ * CCLR_PLAN_FY: one left ladder for all vectors of the call, then three ring-shaped GEMMs and o^3 v^3-class work per vector).
+ * eri: the packed integrals the context was created from -- ooov, oovv, ovvo, ovvv are read (device, borrowed for the call);
+ * oooo and vvvv are NOT (a CCLR_ERI_INPLACE context, whose vvvv block is overwritten, is fine).  out1 [nvec][v*o],
+ * out2 [nvec][vv*oo]: device outputs, must not alias y.  x . F . y = the bilinear dot cclr_property(x, F y). */
+int cclr_f_transform(cclr_ctx *ctx, const cclr_eri_packed *eri, const cclr_c128 *lam1, const cclr_c128 *lam2,
+                     const cclr_c128 *y1, const cclr_c128 *y2, int nvec, cclr_c128 *out1, cclr_c128 *out2);
+
+/* x . F . y by the stencil route, the independent cross-check of cclr_f_transform: the exact derivative
  * d/da [(eta0 + lambda A)(t + a x) . y] at a = 0 (a cubic in a, 4-point stencil), i.e. four cclr_create + cclr_sigma_left
- * evaluations at shifted amplitudes (reading 6: the printed t.F formulas are unrecoverable).  Needs the bare
- * integrals and t (only read).  result: HOST. */
+ * evaluations at shifted amplitudes, without a context.  Needs the bare integrals (all six classes) and t (only read).
+ * result: HOST. */
 int cclr_xfy(int o, int v, const cclr_c128 *fock, const cclr_eri_packed *eri, const cclr_c128 *t1, const cclr_c128 *t2,
              const cclr_c128 *lam1, const cclr_c128 *lam2, const cclr_c128 *x1, const cclr_c128 *x2, const cclr_c128 *y1,
              const cclr_c128 *y2, void *cuda_stream, cclr_c128 *result);
 
 /* <<X;Y>>_z in the symmetric CC-CC (LR-CC) form of PAPER.md:137 Eq. 15 with Eq. 17:
  * g(w) = eta^X . t^Y(w) + eta^Y . t^X(-w) + t^X(-w) . F . t^Y(w),  <<X;Y>>_z = 1/2 [g(z) + conj g(-conj z)].  Same arguments as
- * cclr_response_ci plus the inputs the context was created from (fock, eri, t1, t2: the F contraction rebuilds intermediates
- * at shifted amplitudes, so the context must NOT have been created with CCLR_ERI_INPLACE over this eri->vvvv). */
-int cclr_response_cc(cclr_ctx *ctx, const cclr_c128 *fock, const cclr_eri_packed *eri, const cclr_c128 *t1, const cclr_c128 *t2,
-                     const cclr_c128 *X, const cclr_c128 *Y, double omega, double gamma, double tol, int maxiter,
-                     cclr_c128 *result, cclr_solve_info *info);
+ * cclr_response_ci plus eri, the packed integrals the context was created from (read by cclr_f_transform as described there;
+ * the context may have been created with CCLR_ERI_INPLACE). */
+int cclr_response_cc(cclr_ctx *ctx, const cclr_eri_packed *eri, const cclr_c128 *X, const cclr_c128 *Y, double omega, double gamma,
+                     double tol, int maxiter, cclr_c128 *result, cclr_solve_info *info);
 
 /* result[k] = sum_ai eta1 x1_k + sum_{a<b,i<j} eta2 x2_k  (bilinear, no conjugation; PAPER.md:137 Eq. 15, :203) for
  * nvec vectors x_k; result is a HOST array of nvec complex numbers. */

@@ -11,7 +11,7 @@ import torch
 from . import _lib
 from ._lib import CclrError, SolveInfo  # noqa: F401
 
-__all__ = ["Context", "cclr_create", "cclr_ccsd", "cclr_response_ci", "cclr_response_ci_tensor", "cclr_response_cc", "cclr_xfy", "cclr_eom", "cclr_xi", "cclr_eta", "cclr_lambda", "cclr_solve_left", "cclr_sigma_left", "cclr_sigma", "cclr_solve", "cclr_property", "cclr_zgemm", "cclr_ladder",
+__all__ = ["Context", "cclr_create", "cclr_ccsd", "cclr_response_ci", "cclr_response_ci_tensor", "cclr_response_cc", "cclr_f_transform", "cclr_xfy", "cclr_eom", "cclr_xi", "cclr_eta", "cclr_lambda", "cclr_solve_left", "cclr_sigma_left", "cclr_sigma", "cclr_solve", "cclr_property", "cclr_zgemm", "cclr_ladder",
            "cclr_ring", "cclr_fp64_tensor_peak", "cclr_hbm_copy_peak", "CclrError"]
 
 
@@ -312,14 +312,36 @@ def cclr_xfy(o, v, fock, eri, t1, t2, lam1, lam2, x1, x2, y1, y2):
     return complex(res.re, res.im)
 
 
-def cclr_response_cc(ctx, fock, eri, t1, t2, X, Y, omega, gamma=0.0, tol=1e-10, maxiter=200):
-    """<<X;Y>>_{omega + i gamma} in the symmetric CC-CC form (Eq. 15, 17) on the device; returns (complex, info)."""
+def _eri_struct_partial(o, v, eri, names):
+    """EriPacked with only the classes in `names` set (the others stay NULL: the callee documents which ones it reads)."""
+    oo, vv = o * (o - 1) // 2, v * (v - 1) // 2
+    sizes = dict(oooo=oo * oo, ooov=oo * o * v, oovv=oo * vv, ovvo=o * v * v * o, ovvv=o * v * vv, vvvv=vv * vv)
+    e = _lib.EriPacked()
+    for k in names:
+        setattr(e, k, _dev(eri[k], "eri." + k, sizes[k]))
+    return e
+
+
+def cclr_f_transform(ctx, eri, lam1, lam2, y1, y2):
+    """F y_k for every vector y_k (y1 [nvec, v*o], y2 [nvec, vv*oo]) and the multipliers lam1, lam2; eri: dict holding at
+    least ooov, oovv, ovvo, ovvv of the integrals the context was created from.  Returns (out1, out2) shaped like y."""
+    nvec = y1.numel() // ctx.n1
+    e = _eri_struct_partial(ctx.o, ctx.v, eri, ("ooov", "oovv", "ovvo", "ovvv"))
+    out1, out2 = torch.empty_like(y1), torch.empty_like(y2)
+    _lib.check(_lib.load().cclr_f_transform(ctx.handle, C.byref(e), _dev(lam1, "lam1", ctx.n1), _dev(lam2, "lam2", ctx.n2),
+                                            _dev(y1, "y1", nvec * ctx.n1), _dev(y2, "y2", nvec * ctx.n2), nvec,
+                                            _dev(out1, "out1"), _dev(out2, "out2")), "cclr_f_transform")
+    return out1, out2
+
+
+def cclr_response_cc(ctx, eri, X, Y, omega, gamma=0.0, tol=1e-10, maxiter=200):
+    """<<X;Y>>_{omega + i gamma} in the symmetric CC-CC form (Eq. 15, 17) on the device; eri as for cclr_f_transform.
+    Returns (complex, info)."""
     n = ctx.o + ctx.v
-    e = _eri_struct(ctx.o, ctx.v, eri)
+    e = _eri_struct_partial(ctx.o, ctx.v, eri, ("ooov", "oovv", "ovvo", "ovvv"))
     res = _lib.Complex()
     info = SolveInfo()
-    rc = _lib.load().cclr_response_cc(ctx.handle, _dev(fock, "fock", n * n), C.byref(e), _dev(t1, "t1", ctx.n1),
-                                      _dev(t2, "t2", ctx.n2), _dev(X, "X", n * n), _dev(Y, "Y", n * n), float(omega),
+    rc = _lib.load().cclr_response_cc(ctx.handle, C.byref(e), _dev(X, "X", n * n), _dev(Y, "Y", n * n), float(omega),
                                       float(gamma), float(tol), int(maxiter), C.byref(res), C.byref(info))
     if rc not in (0, -4):
         _lib.check(rc, "cclr_response_cc")

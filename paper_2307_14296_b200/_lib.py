@@ -52,8 +52,9 @@ SIGNATURES = {
                                           C.c_int, C.POINTER(Complex), C.POINTER(SolveInfo)]),
     "cclr_xfy": (C.c_int, [C.c_int, C.c_int, c128_p, C.POINTER(EriPacked), c128_p, c128_p, c128_p, c128_p, c128_p, c128_p,
                            c128_p, c128_p, C.c_void_p, C.POINTER(Complex)]),
-    "cclr_response_cc": (C.c_int, [C.c_void_p, c128_p, C.POINTER(EriPacked), c128_p, c128_p, c128_p, c128_p, C.c_double,
+    "cclr_response_cc": (C.c_int, [C.c_void_p, C.POINTER(EriPacked), c128_p, c128_p, C.c_double,
                                    C.c_double, C.c_double, C.c_int, C.POINTER(Complex), C.POINTER(SolveInfo)]),
+    "cclr_f_transform": (C.c_int, [C.c_void_p, C.POINTER(EriPacked), c128_p, c128_p, c128_p, c128_p, C.c_int, c128_p, c128_p]),
     "cclr_xi": (C.c_int, [C.c_void_p, c128_p, c128_p, c128_p]),
     "cclr_property": (C.c_int, [C.c_void_p, c128_p, c128_p, c128_p, c128_p, C.c_int, C.POINTER(Complex)]),
     "cclr_ccsd": (C.c_int, [C.c_int, C.c_int, c128_p, C.POINTER(EriPacked), c128_p, c128_p, C.c_double, C.c_int, C.c_void_p,

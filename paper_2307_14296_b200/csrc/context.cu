@@ -472,6 +472,47 @@ extern "C" int cclr_eta(cclr_ctx *ctx, const cclr_c128 *X, const cclr_c128 *lam1
   return CCLR_OK;
 }
 
+// out = F y (CCLR_PLAN_FY, csrc/plans.inc) for nvec vectors y and one set of multipliers; the lambda-only left ladder M
+// (CCLR_PLAN_FY_M) is evaluated once per call.  The plan holds chunk loops and frees its temporaries as it goes, so it is
+// executed statement by statement on the context's plan (like cclr_create), not compiled.
+extern "C" int cclr_f_transform(cclr_ctx *ctx, const cclr_eri_packed *eri, const cclr_c128 *lam1, const cclr_c128 *lam2,
+                                const cclr_c128 *y1, const cclr_c128 *y2, int nvec, cclr_c128 *out1, cclr_c128 *out2) {
+  if (!ctx || !eri || !eri->ooov || !eri->oovv || !eri->ovvo || !eri->ovvv || !lam1 || !lam2 || !y1 || !y2 || !out1 || !out2 ||
+      nvec < 1 || y1 == out1 || y2 == out2) {
+    cclr_set_error("cclr_f_transform: null pointer, nvec < 1 or aliased output", cudaSuccess);
+    return CCLR_EINVAL;
+  }
+  Plan &P = *ctx->plan;
+  auto unbind = [&]() {
+    for (const char *name : {"ooov", "oovv", "ovvo", "ovvv", "y1", "y2"}) {
+      const int id = P.find(name);
+      if (id >= 0) P.rebind(id, nullptr);
+    }
+  };
+  try {
+    P.bind("ooov", "(mn)ie", (c128 *)eri->ooov);
+    P.bind("oovv", "(mn)(ef)", (c128 *)eri->oovv);
+    P.bind("ovvo", "mbej", (c128 *)eri->ovvo);
+    P.bind("ovvv", "mb(ef)", (c128 *)eri->ovvv);
+    bind_vectors(ctx, (const c128 *)lam1, (const c128 *)lam2, nullptr, nullptr);
+    P.execute(CCLR_PLAN_FY_M);
+    for (int k = 0; k < nvec; ++k) {
+      P.bind("y1", "ai", (c128 *)y1 + (size_t)k * ctx->n1);
+      P.bind("y2", "(ab)(ij)", (c128 *)y2 + (size_t)k * ctx->n2);
+      bind_vectors(ctx, (const c128 *)lam1, (const c128 *)lam2, (c128 *)out1 + (size_t)k * ctx->n1, (c128 *)out2 + (size_t)k * ctx->n2);
+      P.execute(CCLR_PLAN_FY);
+      P.free_class(BUF_TEMP);
+    }
+    check(cudaStreamSynchronize(ctx->st), "cclr_f_transform sync");   // the borrowed integrals end here
+    unbind();
+  } catch (const PlanError &e) {
+    try { P.free_class(BUF_TEMP); } catch (...) {}
+    unbind();
+    return cclr_fail(e);
+  }
+  return CCLR_OK;
+}
+
 extern "C" long cclr_get_intermediate(cclr_ctx *ctx, const char *name, cclr_c128 *out, long capacity) {
   if (!ctx || !name) return CCLR_EINVAL;
   long n = 0;

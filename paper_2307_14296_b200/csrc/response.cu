@@ -12,14 +12,7 @@
 using subspace::check;
 using subspace::DeviceBuf;
 
-namespace {
-struct GroundState {   // what the F contraction of the CC-CC form needs besides the context
-  const cclr_c128 *fock;
-  const cclr_eri_packed *eri;
-  const cclr_c128 *t1, *t2;
-};
-}  // namespace
-
+// The stencil route to x . F . y, kept as the independent cross-check of the direct plan (cclr_f_transform, CCLR_PLAN_FY):
 // x . F . y = d/da [ (eta0 + lambda A)(t + a x) . y ] at a = 0  (F = CC Hessian of Table 1; S-Eq. 8, PAPER.md:855-857;
 // the printed contraction formulas PAPER.md:861-879 are unrecoverable, reading 6).  The bracket is a cubic polynomial
 // in a (A is cubic in t, eta0 linear), so the 4-point stencil [w(-2h) - 8 w(-h) + 8 w(h) - w(2h)] / 12h is exact; every w is one
@@ -81,7 +74,7 @@ extern "C" int cclr_xfy(int o, int v, const cclr_c128 *fock, const cclr_eri_pack
 }
 
 static int response_impl(cclr_ctx *ctx, const cclr_c128 *X, const cclr_c128 *Y, double omega, double gamma, double tol,
-                         int maxiter, cclr_c128 *result, cclr_solve_info *info, const GroundState *gs) {
+                         int maxiter, cclr_c128 *result, cclr_solve_info *info, const cclr_eri_packed *gs) {
   if (!ctx || !X || !Y || !result || !(tol > 0.0) || maxiter < 1) {
     cclr_set_error("cclr_response: null pointer, tol <= 0 or maxiter < 1", cudaSuccess);
     return CCLR_EINVAL;
@@ -146,11 +139,14 @@ static int response_impl(cclr_ctx *ctx, const cclr_c128 *X, const cclr_c128 *Y, 
       g0 = C(a[0]) - C(c[0]) * C(e) + C(b[0]) - C(d[0]) * C(f);
       g1 = C(a[1]) - C(c[1]) * C(e) + C(b[1]) - C(d[1]) * C(f);
     } else {     // CC-CC, Eq. 15: g(w) = eta^X . t^Y(w) + eta^Y . t^X(-w) + t^X(-w) . F . t^Y(w)
-      for (int k = 0; k < 2; ++k) {
-        rc = cclr_xfy(ctx->o, ctx->v, gs->fock, gs->eri, gs->t1, gs->t2, lam1, lam2, tX1 + (size_t)k * n1, tX2 + (size_t)k * n2,
-                      tY1 + (size_t)k * n1, tY2 + (size_t)k * n2, (void *)ctx->st, &c[k]);
-        if (rc != CCLR_OK) return rc;
-      }
+      // F t^Y for both shifts in one call of the direct plan (one lambda-only ladder, then ~3 sigma-equivalents per vector)
+      DeviceBuf FY;
+      FY.alloc(2 * n, "cudaMalloc(F t)");
+      cclr_c128 *fy1 = (cclr_c128 *)FY.p, *fy2 = (cclr_c128 *)(FY.p + 2 * n1);
+      if ((rc = cclr_f_transform(ctx, gs, lam1, lam2, tY1, tY2, 2, fy1, fy2)) != CCLR_OK) return rc;
+      for (int k = 0; k < 2; ++k)
+        if ((rc = cclr_property(ctx, tX1 + (size_t)k * n1, tX2 + (size_t)k * n2, fy1 + (size_t)k * n1, fy2 + (size_t)k * n2, 1, &c[k])) != CCLR_OK)
+          return rc;
       g0 = C(a[0]) + C(b[0]) + C(c[0]);
       g1 = C(a[1]) + C(b[1]) + C(c[1]);
     }
@@ -169,15 +165,13 @@ extern "C" int cclr_response_ci(cclr_ctx *ctx, const cclr_c128 *X, const cclr_c1
   return response_impl(ctx, X, Y, omega, gamma, tol, maxiter, result, info, nullptr);
 }
 
-extern "C" int cclr_response_cc(cclr_ctx *ctx, const cclr_c128 *fock, const cclr_eri_packed *eri, const cclr_c128 *t1,
-                                const cclr_c128 *t2, const cclr_c128 *X, const cclr_c128 *Y, double omega, double gamma,
-                                double tol, int maxiter, cclr_c128 *result, cclr_solve_info *info) {
-  if (!fock || !eri || !t1 || !t2) {
+extern "C" int cclr_response_cc(cclr_ctx *ctx, const cclr_eri_packed *eri, const cclr_c128 *X, const cclr_c128 *Y, double omega,
+                                double gamma, double tol, int maxiter, cclr_c128 *result, cclr_solve_info *info) {
+  if (!eri) {
     cclr_set_error("cclr_response_cc: null pointer", cudaSuccess);
     return CCLR_EINVAL;
   }
-  const GroundState gs{fock, eri, t1, t2};
-  return response_impl(ctx, X, Y, omega, gamma, tol, maxiter, result, info, &gs);
+  return response_impl(ctx, X, Y, omega, gamma, tol, maxiter, result, info, eri);
 }
 
 

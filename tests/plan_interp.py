@@ -403,5 +403,6 @@ def run_fy(it, packed, l1, l2p, y1, y2p):
     it.bind("y2", "(ab)(ij)", y2p)
     it.bind("out1", "ai", np.zeros(v * o, complex))
     it.bind("out2", "(ab)(ij)", np.zeros(npair(v) * npair(o), complex))
+    it.run(load_plan("CCLR_PLAN_FY_M"))       # the lambda-only ladder, once per set of multipliers
     it.run(load_plan("CCLR_PLAN_FY"))
     return it.get("out1").copy(), it.get("out2").copy()

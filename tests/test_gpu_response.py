@@ -121,6 +121,26 @@ def test_hessian_contraction_matches_oracle(cfg1):
     assert abs(got - want) <= 1e-9 * abs(want), (got, want)
 
 
+def test_f_transform_matches_oracle_and_the_stencil_route(cfg1):
+    """cclr_f_transform (the direct plan CCLR_PLAN_FY) element by element against oracle.cclr.CCLR.F_transform (pinned by the
+    determinant-space F), two vectors in one call; and x . (F y) against cclr_xfy, the library's independent stencil route."""
+    s = cfg1
+    cc, d, o, v = s["cc"], s["dev"], s["o"], s["v"]
+    l1p, l2p = packing.pack_amplitudes(*s["lam"])
+    y1, y2 = synth.amplitudes(o, v, seed=23, cls1="x1", cls2="x2", nvec=2)
+    g1, g2 = cc.cclr_f_transform(s["ctx"], d["eri"], _dev(l1p), _dev(l2p), y1.cuda(), y2.cuda())
+    torch.cuda.synchronize()
+    for k in range(2):
+        w1, w2 = packing.pack_amplitudes(*s["c"].F_transform(*s["lam"], *packing.unpack_amplitudes(y1[k].numpy(), y2[k].numpy(), o, v)))
+        assert np.linalg.norm(g1[k].cpu().numpy() - w1.reshape(-1)) <= 1e-10 * np.linalg.norm(w1)
+        assert np.linalg.norm(g2[k].cpu().numpy() - w2.reshape(-1)) <= 1e-10 * np.linalg.norm(w2)
+    x1, x2 = synth.amplitudes(o, v, seed=24, cls1="x1", cls2="x2")
+    direct = cc.cclr_property(s["ctx"], x1[0].cuda(), x2[0].cuda(), g1[:1].contiguous(), g2[:1].contiguous())[0]
+    stencil = cc.cclr_xfy(o, v, d["f"], d["eri"], d["t1"], d["t2"], _dev(l1p), _dev(l2p), x1[0].cuda(), x2[0].cuda(),
+                          y1[0].cuda(), y2[0].cuda())
+    assert abs(direct - stencil) <= 1e-9 * abs(stencil), (direct, stencil)
+
+
 @pytest.mark.parametrize("z", [0.0, 0.0773 + 0.0045j])
 def test_cc_cc_response_function_end_to_end(cfg1, z):
     s = cfg1
@@ -128,10 +148,24 @@ def test_cc_cc_response_function_end_to_end(cfg1, z):
     dense = lambda a, b, zz: c.solve_dense(A, a, b, zz)
     for (P, Q) in [(ops[0], ops[1]), (ops[2], ops[3])]:
         want = c.response_cc_cc(dense, P, Q, z, l1, l2)
-        got, info = s["cc"].cclr_response_cc(s["ctx"], d["f"], d["eri"], d["t1"], d["t2"], _dev(P), _dev(Q), complex(z).real,
-                                             complex(z).imag, tol=1e-11)
+        got, info = s["cc"].cclr_response_cc(s["ctx"], d["eri"], _dev(P), _dev(Q), complex(z).real, complex(z).imag, tol=1e-11)
         assert info.converged == 1
         assert abs(got - want) <= 1e-8 * abs(want), (z, got, want)
+
+
+def test_cc_cc_response_function_on_an_inplace_context(cfg1):
+    """The F contraction reads W_vvvv only through the dressed block, so the symmetric form works on a context created with
+    ERI_INPLACE (the caller's vvvv array is overwritten by W_abef; its other classes are read again by cclr_response_cc)."""
+    s = cfg1
+    cc, c, A, (l1, l2), ops, d = s["cc"], s["c"], s["A"], s["lam"], s["ops"], s["dev"]
+    eri = {k: x.clone() for k, x in d["eri"].items()}
+    ctx = cc.cclr_create(s["o"], s["v"], d["f"], eri, d["t1"], d["t2"], cc.ERI_INPLACE)
+    z = 0.0773 + 0.0045j
+    want = c.response_cc_cc(lambda a, b, zz: c.solve_dense(A, a, b, zz), ops[0], ops[2], z, l1, l2)
+    got, info = cc.cclr_response_cc(ctx, eri, _dev(ops[0]), _dev(ops[2]), z.real, z.imag, tol=1e-11)
+    ctx.close()
+    assert info.converged == 1
+    assert abs(got - want) <= 1e-8 * abs(want), (got, want)
 
 
 @pytest.mark.parametrize("gamma", [0.0, 0.0045])
