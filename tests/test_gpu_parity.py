@@ -321,7 +321,8 @@ def test_gpu_linearity_and_shift_identity():
 def test_config2_ground_state_sigma_solve_and_response_function_against_full_oracle():
     """BASELINE.json configs[1] (o=10, v=80, damped gamma=0.0045) at full size, everything against the full-tensor oracle:
     the GPU ground state (cclr_ccsd, 1e-10) is certified by ONE oracle residual evaluation, sigma matches norm-wise to 1e-10,
-    and the damped response amplitudes of a dipole perturbation satisfy the oracle's (A - z) t + xi = 0 to 2e-10."""
+    the damped response amplitudes of a dipole perturbation satisfy the oracle's (A - z) t + xi = 0 to 2e-10, and the damped
+    CC-CI response function <<X;X>>_z (Eq. 16-17) equals the oracle's assembly from certified vectors to 1e-8."""
     cc = _lib()
     o, v = 10, 80
     eri = synth.eri_packed(o, v, seed=0)
@@ -359,8 +360,9 @@ def test_config2_ground_state_sigma_solve_and_response_function_against_full_ora
     # four response solves, dots) against the oracle's own assembly of Eq. 16-17 from amplitudes it has CERTIFIED -- lambda and
     # every t(z) come from the GPU, and the oracle checks each against its own residual before using it.
     X = synth.hermitian_operator(o + v, 0, 0)
-    zr = 0.0773            # (real frequency: two distinct response solves instead of four keeps the oracle's part affordable)
-    got, rinfo = cc.cclr_response_ci(ctx, torch.from_numpy(X).cuda(), torch.from_numpy(X).cuda(), zr, 0.0, tol=1e-10)
+    # (damped, gamma = 0.0045 as BASELINE.json configs[1] asks: four distinct response solves t(z), t(-z), t(-z*), t(z*), each
+    # certified by one oracle sigma and cached)
+    got, rinfo = cc.cclr_response_ci(ctx, torch.from_numpy(X).cuda(), torch.from_numpy(X).cuda(), z.real, z.imag, tol=1e-10)
     assert rinfo.converged == 1
     lg1, lg2, linfo = cc.cclr_lambda(ctx, tol=1e-10)
     assert linfo.converged == 1
@@ -383,7 +385,7 @@ def test_config2_ground_state_sigma_solve_and_response_function_against_full_ora
         cache[complex(zz)] = (h1, h2)
         return h1, h2
 
-    want = c.response_cc_ci(certified_gpu_solve, X, X, zr, *lam)
+    want = c.response_cc_ci(certified_gpu_solve, X, X, z, *lam)
     assert abs(got - want) <= 1e-8 * abs(want), (got, want)
     ctx.close()
 
