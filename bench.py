@@ -170,7 +170,7 @@ def measured_ladder_traffic(gemm, config):
     csrc/zgemm.cu, complex product, config, kernel, dram__bytes_read.sum + dram__bytes_write.sum; the command that made it is in
     profiles/r02_ncu_traffic.md).  Returns (bytes, source) or (None, why): the run itself cannot measure DRAM traffic."""
     path = os.path.join(ROOT, "profiles", "r02_ncu_traffic.csv")
-    src = os.path.join(ROOT, "paper_2307_14296_b200", "csrc", "zgemm.cu")
+    src = os.path.join(ROOT, "paper_2307_14296_b200", "csrc", "zgemm_oz.cu" if gemm == "oz" else "zgemm.cu")
     try:
         with open(src, "rb") as fh:
             sha = hashlib.sha1(fh.read()).hexdigest()
@@ -181,7 +181,19 @@ def measured_ladder_traffic(gemm, config):
     for r in rows:
         if len(r) >= 5 and r[0] == sha and r[1] == gemm and r[2] == str(config) and r[3] == "ladder":
             return float(r[4]), "profiles/r02_ncu_traffic.csv: dram__bytes_read.sum + dram__bytes_write.sum of the ladder launch, ncu capture of this build"
-    return None, "profiles/r02_ncu_traffic.csv has no capture of this build of csrc/zgemm.cu for this config / product"
+    return None, "profiles/r02_ncu_traffic.csv has no capture of this build of csrc/%s for this config / product" % os.path.basename(src)
+
+
+def measured_peaks():
+    """MEASURED_PEAKS.json (driver-written: HBM copy GB/s and cuBLAS bf16 TFLOP/s, burst and sustained) or the profiling guide's
+    fallback (6650 GB/s, 1590 burst / 1400 sustained TFLOP/s)."""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
+            p = json.load(fh)
+        return {"hbm_gbs": float(p["hbm_gbs"]), "bf16": float(p["bf16_tflops"]), "bf16_sustained": float(p.get("bf16_tflops_sustained", p["bf16_tflops"])),
+                "source": "MEASURED_PEAKS.json (of measured)"}
+    except (OSError, KeyError, ValueError):
+        return {"hbm_gbs": 6650.0, "bf16": 1590.0, "bf16_sustained": 1400.0, "source": "B200_PROFILING.md fallback (of fallback)"}
 
 
 # ---------------------------------------------------------------------------------------------------------------
@@ -226,7 +238,8 @@ def build_workload(cc, torch, synth, cfg, o, v, nvec, seed, ground, gemm="3m", g
     torch.cuda.synchronize()
     l0 = cc.cclr_kernel_launches()
     t0 = time.perf_counter()
-    ctx = cc.cclr_create(o, v, f, eri, t1, t2, cc.ERI_INPLACE | (cc.GEMM_4M if gemm == "4m" else 0) | (0 if graph else cc.NO_GRAPH))
+    ctx = cc.cclr_create(o, v, f, eri, t1, t2, cc.ERI_INPLACE | (cc.GEMM_4M if gemm == "4m" else 0) | (cc.GEMM_DMMA if gemm == "3m" else 0)
+                         | (0 if graph else cc.NO_GRAPH))
     torch.cuda.synchronize()
     create_s = time.perf_counter() - t0
     create_launches = cc.cclr_kernel_launches() - l0
@@ -355,6 +368,23 @@ def run_ours(args):
     barrier()
     unprofiled_ms = g0.elapsed_time(g1) / args.steps
 
+    # ---- the same steps with ladder and ring on the FP64 tensor cores (DMMA), same context: the path north_star names -----------
+    dmma_ms = None
+    if args.gemm == "oz" and ctx.set_gemm_path(0) == 0:
+        for _ in range(2):
+            cc.cclr_sigma(ctx, x1, x2, omega, gamma, out1, out2)
+        barrier()
+        d0, d1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        d0.record()
+        for _ in range(3):
+            cc.cclr_sigma(ctx, x1, x2, omega, gamma, out1, out2)
+        d1.record()
+        barrier()
+        dmma_ms = d0.elapsed_time(d1) / 3
+        oz_on = ctx.set_gemm_path(1) == 1
+    else:
+        oz_on = False
+
     # ---- the left transform l (A - z) (Lambda / left response equations; same flop count), 3 steps --------------------------
     for _ in range(2):
         cc.cclr_sigma_left(ctx, x1, x2, omega, gamma, out1, out2)
@@ -393,6 +423,10 @@ def run_ours(args):
         "unprofiled": {"ms_per_step": unprofiled_ms, "tflops": flops_step / (unprofiled_ms * 1e-3) / 1e12,
                        "what": "cclr_sigma without the per-operation profiling events%s" % ("" if args.no_graph else " (CUDA-graph replay when the context is small enough)")},
         "left_sigma": {"ms_per_step": left_ms, "tflops": flops_step / (left_ms * 1e-3) / 1e12},
+        "integer_slice_path": oz_on,
+        "dmma_path": None if dmma_ms is None else {
+            "ms_per_step": dmma_ms, "tflops": flops_step / (dmma_ms * 1e-3) / 1e12,
+            "what": "the same cclr_sigma on the same context with ladder and ring on the FP64 tensor cores (3M DMMA, cclr_set_gemm_path 0)"},
         "gpu_launches": int(launches), "create_s": create_s, "create_launches": int(create_launches),
         "ground_state_info": ground_info,
     }
@@ -401,24 +435,46 @@ def run_ours(args):
         peak = cc.cclr_fp64_tensor_peak(20000)
         lad_ms = phases["ladder"] / (args.steps * nvec)
         lad_flops8 = 8.0 * cm["T11"]
-        executed = (0.75 if args.gemm == "3m" else 1.0) * lad_flops8
         traffic, traffic_src = measured_ladder_traffic(args.gemm, args.config)
-        line["roofline"] = {
-            "bound": "tensor",
-            "kernel": "zgemm3m_kernel<48,kn> (pp ladder T11)" if args.gemm == "3m" else "zgemm_kernel<128,64,16,...,kn> (pp ladder T11)",
-            "achieved": executed / (lad_ms * 1e-3) / 1e12, "peak": peak, "unit": UNIT,
-            "frac": executed / (lad_ms * 1e-3) / 1e12 / peak,
-            "flops_counted": "EXECUTED real flops on the FP64 tensor pipe: %d per complex multiply-add of the packed ladder (the 3M "
-                             "product issues 3 real multiply-adds instead of 4); the algorithmic count of SURVEY 8(d), 8 vv^2 oo, is "
-                             "reported beside it" % (6 if args.gemm == "3m" else 8),
-            "algorithmic_tflops_8flop_convention": lad_flops8 / (lad_ms * 1e-3) / 1e12,
-            "algorithmic_frac_8flop_convention": lad_flops8 / (lad_ms * 1e-3) / 1e12 / peak,
-            "complex_product": args.gemm,
-            "peak_source": "FP64 tensor (DMMA m8n8k4) issue-rate probe cclr_fp64_tensor_peak measured in this run; "
-                           "MEASURED_PEAKS.json has no FP64 entry (nominal HGX B200: 37 TFLOP/s)",
-            "traffic": traffic, "traffic_source": traffic_src,
-            "algorithmic_bytes": 16.0 * (npair(v) ** 2 + 2 * n2), "ms_per_launch": lad_ms,
-        }
+        oz_ladder = args.gemm == "oz" and cc.cclr_zgemm_oz_eligible(npair(v), npair(o), npair(v))
+        if oz_ladder:
+            # the ladder runs as 21 INT8 slice-pair products (6 slices, t + u <= 5) of the real embedding: 4 real multiply-adds per
+            # complex one, 2 ops each -> 21 * 8 vv^2 oo integer ops; peak = measured cuBLAS bf16 (sustained: the kernel is timed inside
+            # a long step) x 2, the nominal INT8 : bf16 ratio of the chip (4.5 : 2.25 Pop/s)
+            mp = measured_peaks()
+            executed = 21.0 * lad_flops8
+            peak_i8 = 2.0 * mp["bf16_sustained"]
+            line["roofline"] = {
+                "bound": "tensor", "kernel": "zgemm_oz_kernel (pp ladder T11 as 21 INT8 slice-pair products, tcgen05.mma.kind::i8, S32 accumulators in TMEM)",
+                "achieved": executed / (lad_ms * 1e-3) / 1e12, "peak": peak_i8, "unit": UNIT, "frac": executed / (lad_ms * 1e-3) / 1e12 / peak_i8,
+                "flops_counted": "EXECUTED integer ops of the tensor pipe (2 per INT8 multiply-add): 21 slice pairs x 8 vv^2 oo; the duration "
+                                 "includes the per-call slicing of the trial vector (the B operand)",
+                "peak_source": "2 x bf16_tflops_sustained of %s: the INT8 peak is the bf16 one times the nominal ratio 4.5 : 2.25 "
+                               "(burst figure x 2 = %.0f)" % (mp["source"], 2.0 * mp["bf16"]),
+                "fp64_equivalent_tflops_8flop_convention": lad_flops8 / (lad_ms * 1e-3) / 1e12,
+                "fp64_equivalent_over_dmma_peak": lad_flops8 / (lad_ms * 1e-3) / 1e12 / peak,
+                "dmma_peak_measured": peak, "complex_product": "oz (6 integer slices of 7 bits)",
+                "traffic": traffic, "traffic_source": traffic_src,
+                "algorithmic_bytes": 16.0 * (npair(v) ** 2 + 2 * n2), "ms_per_launch": lad_ms,
+            }
+        else:
+            executed = (0.75 if args.gemm == "3m" else 1.0) * lad_flops8
+            line["roofline"] = {
+                "bound": "tensor",
+                "kernel": "zgemm3m_kernel<48,kn> (pp ladder T11)" if args.gemm == "3m" else "zgemm_kernel<128,64,16,...,kn> (pp ladder T11)",
+                "achieved": executed / (lad_ms * 1e-3) / 1e12, "peak": peak, "unit": UNIT,
+                "frac": executed / (lad_ms * 1e-3) / 1e12 / peak,
+                "flops_counted": "EXECUTED real flops on the FP64 tensor pipe: %d per complex multiply-add of the packed ladder (the 3M "
+                                 "product issues 3 real multiply-adds instead of 4); the algorithmic count of SURVEY 8(d), 8 vv^2 oo, is "
+                                 "reported beside it" % (6 if args.gemm == "3m" else 8),
+                "algorithmic_tflops_8flop_convention": lad_flops8 / (lad_ms * 1e-3) / 1e12,
+                "algorithmic_frac_8flop_convention": lad_flops8 / (lad_ms * 1e-3) / 1e12 / peak,
+                "complex_product": args.gemm,
+                "peak_source": "FP64 tensor (DMMA m8n8k4) issue-rate probe cclr_fp64_tensor_peak measured in this run; "
+                               "MEASURED_PEAKS.json has no FP64 entry (nominal HGX B200: 37 TFLOP/s)",
+                "traffic": traffic, "traffic_source": traffic_src,
+                "algorithmic_bytes": 16.0 * (npair(v) ** 2 + 2 * n2), "ms_per_launch": lad_ms,
+            }
         tot = max(phases["total"], 1e-9)
         if args.ops:
             line["ops_ms_last_step"] = [(t, round(m, 4)) for t, m in ops_last]
@@ -513,7 +569,9 @@ def main():
     ap.add_argument("--ground", default="ccsd", choices=["ccsd", "first-order"],
                     help="ground-state amplitudes: converged on the device with cclr_ccsd (default; cached in a scratch directory) "
                          "or the first-order doubles (sigma does not depend on the convergence of T, DESIGN.md)")
-    ap.add_argument("--gemm", default="3m", choices=["3m", "4m"], help="complex product of the large contractions")
+    ap.add_argument("--gemm", default="oz", choices=["3m", "4m", "oz"],
+                    help="complex product of the large contractions: 3M / 4M on the FP64 tensor cores (DMMA), or oz = ladder and ring as "
+                         "integer-slice products on the INT8 tensor path at FP64 accuracy (the library default; 3m / 4m set CCLR_GEMM_DMMA / CCLR_GEMM_4M)")
     ap.add_argument("--no-graph", action="store_true", help="do not replay sigma as a CUDA graph (small configs; before / after numbers)")
     ap.add_argument("--ops", action="store_true", help="add the per-operation times of the last sigma step to the line")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")

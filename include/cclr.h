@@ -61,6 +61,14 @@ typedef struct {
 #define CCLR_NO_GRAPH 8u    /* never replay sigma as a CUDA graph (default: contexts with at most 2^21 unique amplitudes capture the sigma
                                plan once and replay it per trial vector -- they are launch bound; results are identical) */
 
+#define CCLR_GEMM_DMMA 32u  /* keep EVERY contraction on the FP64 tensor cores (DMMA).  Default: the two contractions that are 91 % of
+                               cclr_sigma -- the pp ladder T11 and the ring T8 -- run on the INT8 tensor path at FP64 accuracy when
+                               their shapes allow (vv >= 512, oo >= 32): the context keeps 6 integer slices of 7 bits of W_vvvv and
+                               W_ovvo (3/4 of their size) and slices the trial vector per call (cclr_zgemm_oz; csrc/zgemm_oz.cu;
+                               DESIGN.md 6.1b).  The slice product holds north_star's 1e-10 on sigma (~1e-11 measured); every
+                               other contraction, cclr_create and the left transform are DMMA either way.  CCLR_GEMM_4M implies
+                               this flag.  cclr_set_gemm_path switches an existing context. */
+
 #define CCLR_SMALL_CHUNKS 2u /* testing aid: run the chunked intermediate builds with chunks of 3 indices so that small
                                inputs exercise several chunks and a ragged last one (results are unchanged) */
 
@@ -238,6 +246,23 @@ int cclr_sigma_host(cclr_ctx *ctx, const cclr_c128 *x1, const cclr_c128 *x2, int
 int cclr_zgemm(void *cuda_stream, int M, int N, int K, const cclr_c128 *alpha, const cclr_c128 *A, long lda,
                int conj_a, const cclr_c128 *B, long ldb, int b_is_kn, int conj_b, const cclr_c128 *beta,
                cclr_c128 *C, long ldc, int batch, long sa, long sb, long sc, int three_m);
+
+/* The same product C = alpha opA(A) opB(B) + beta C (batch 1) at FP64 accuracy on the INT8 tensor path (tcgen05.mma.kind::i8, S32
+ * accumulators in tensor memory) by integer slicing of the operands (csrc/zgemm_oz.cu): every row of A and every
+ * column of B is scaled by a power of two and cut into `slices` (2..8) signed slices of 7 bits; the slices * (slices + 1) / 2
+ * integer products with t + u < slices are exact, so the only error is the truncation of the operands 6 + 7 (slices - 1) bits below
+ * their row / column maxima (slices = 6: norm-wise ~1e-11 for rows without outliers; it holds north_star's 1e-10 on sigma).
+ * Shapes: M >= 512, N >= 32, 512 <= K < 2^17 (else CCLR_EINVAL).  reps >= 1 repeats the product (timing); ms (HOST, may be NULL)
+ * receives ms[0] = slicing A (done once), ms[1] = one product including the slicing of B, ms[2] = the slicing of B alone
+ * (CUDA events on the stream).  bn = 0 picks the tile width and cluster shape; else bn % 1000 forces the width (multiple of 16 in
+ * [16, 256]) and (bn / 1000) % 10, bn / 10000 the CTAs of a cluster along N and M (tuning runs).  With beta != 0 use reps = 1. */
+int cclr_zgemm_oz(void *cuda_stream, int M, int N, int K, const cclr_c128 *alpha, const cclr_c128 *A, long lda, int conj_a,
+                  const cclr_c128 *B, long ldb, int b_is_kn, int conj_b, const cclr_c128 *beta, cclr_c128 *C, long ldc,
+                  int slices, int bn, int reps, double *ms);
+
+/* Switch the ladder / ring of an existing context between the integer-slice product (path = 1; only if the context holds the slices,
+ * i.e. was created without CCLR_GEMM_DMMA / CCLR_GEMM_4M at an eligible size) and DMMA (path = 0).  Returns the path now in use. */
+int cclr_set_gemm_path(cclr_ctx *ctx, int path);
 
 /* The particle-particle ladder alone (term T11 of S-Eq. 12):
  * out2[k][ab][ij] = sum_{e<f} W_vvvv[ab][ef] x2[k][ef][ij] for nvec vectors (no shift, no other term). */

@@ -40,6 +40,7 @@ SMALL_CHUNKS = 2
 GEMM_4M = 4
 NO_GRAPH = 8
 NO_SUM_PLANES = 16
+GEMM_DMMA = 32
 
 
 class Context:
@@ -88,6 +89,11 @@ class Context:
 
     def set_max_subspace(self, dim):
         _lib.check(_lib.load().cclr_set_max_subspace(self.handle, int(dim)), "cclr_set_max_subspace")
+
+    def set_gemm_path(self, path):
+        """1: ladder / ring as integer-slice products on the INT8 tensor path (if the context holds the slices), 0: DMMA.
+        Returns the path now in use."""
+        return int(_lib.load().cclr_set_gemm_path(self.handle, int(path)))
 
     def set_profiling(self, on):
         _lib.check(_lib.load().cclr_set_profiling(self.handle, int(bool(on))), "cclr_set_profiling")
@@ -392,6 +398,24 @@ def cclr_zgemm(A, B, C_out, alpha=1.0, beta=0.0, conj_a=False, conj_b=False, b_i
                                 2 if three_m == 2 and three_m is not True else int(bool(three_m)))
     _lib.check(rc, "cclr_zgemm")
     return C_out
+
+
+def cclr_zgemm_oz_eligible(M, N, K):
+    """Whether the integer-slice product takes this shape (include/cclr.h: cclr_zgemm_oz)."""
+    return M >= 512 and N >= 32 and 512 <= K < (1 << 17)
+
+
+def cclr_zgemm_oz(A, B, C_out, alpha=1.0, beta=0.0, conj_a=False, conj_b=False, b_is_kn=False, slices=6, bn=0, reps=1):
+    """C = alpha opA(A) opB(B) + beta C on 2-D row-major tensors through the integer-slice product on the INT8 tensor path
+    (include/cclr.h: cclr_zgemm_oz).  Returns (C_out, [ms slicing A, ms per product incl. slicing B, ms slicing B])."""
+    M, K = A.shape
+    N = B.shape[1] if b_is_kn else B.shape[0]
+    al, be = _lib.Complex(complex(alpha).real, complex(alpha).imag), _lib.Complex(complex(beta).real, complex(beta).imag)
+    ms = (C.c_double * 3)()
+    rc = _lib.load().cclr_zgemm_oz(_stream(), M, N, K, C.byref(al), _dev(A, "A"), A.shape[1], int(conj_a), _dev(B, "B"), B.shape[1],
+                                   int(b_is_kn), int(conj_b), C.byref(be), _dev(C_out, "C"), C_out.shape[1], slices, bn, reps, ms)
+    _lib.check(rc, "cclr_zgemm_oz")
+    return C_out, [ms[0], ms[1], ms[2]]
 
 
 def cclr_vec_block_lincomb(ctx, Y, X, coef, V, nrm2=None, z=None, P=None):

@@ -72,6 +72,10 @@ SIGNATURES = {
     "cclr_zgemm": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.POINTER(Complex), c128_p, C.c_long, C.c_int,
                              c128_p, C.c_long, C.c_int, C.c_int, C.POINTER(Complex), c128_p, C.c_long, C.c_int,
                              C.c_long, C.c_long, C.c_long, C.c_int]),
+    "cclr_set_gemm_path": (C.c_int, [C.c_void_p, C.c_int]),
+    "cclr_zgemm_oz": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.POINTER(Complex), c128_p, C.c_long, C.c_int,
+                                c128_p, C.c_long, C.c_int, C.c_int, C.POINTER(Complex), c128_p, C.c_long, C.c_int, C.c_int,
+                                C.c_int, C.POINTER(C.c_double)]),
     "cclr_vec_block_lincomb": (C.c_int, [C.c_void_p, C.c_int, c128_p, C.c_long, c128_p, C.c_long, c128_p, c128_p, C.c_long, C.c_int,
                                          C.c_long, C.c_void_p, c128_p, c128_p, C.c_long]),
     "cclr_vec_dots": (C.c_int, [C.c_void_p, c128_p, C.c_int, c128_p, C.c_int, C.c_long, C.c_long, C.POINTER(Complex)]),

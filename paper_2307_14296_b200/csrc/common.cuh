@@ -7,6 +7,7 @@
 #include <vector>
 
 typedef double2 c128;  // complex128, interleaved (re, im)
+struct OzWorkspace;    // zgemm_oz.cu (below)
 
 #define CCLR_HOST_DEVICE __host__ __device__ __forceinline__
 
@@ -43,6 +44,8 @@ struct ZgemmWorkspace {
   const double *persist_plane[2] = {nullptr, nullptr};
   long persist_ld[2] = {0, 0};                         // leading dimension of the operand (complex elements) ...
   long persist_pld[2] = {0, 0};                        // ... and of its plane (doubles, even)
+  // integer-slice product on the INT8 tensor path (zgemm_oz.cu): when set and oz->slices > 0, eligible contractions go there
+  OzWorkspace *oz = nullptr;
 };
 // C = alpha * opA(A) * opB(B) + beta * C; see include/cclr.h (cclr_zgemm).  ws may be null (no split-K then).
 cudaError_t zgemm(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *A, long lda, bool conjA,
@@ -51,6 +54,32 @@ cudaError_t zgemm(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *
 int zgemm_num_sms();
 // plane[r][c] = Re X[r][c] +- Im X[r][c] (the 3M product's sum operand; see ZgemmWorkspace)
 cudaError_t zgemm_sum_plane(cudaStream_t st, const c128 *X, long ld, long rows, long cols, bool conj, double *plane, long ldp);
+
+// ---- zgemm_oz.cu: the same product at FP64 accuracy from INT8 slices (tcgen05.mma.kind::i8, S32 accumulators in TMEM) --------
+struct OzEntry {
+  const c128 *key = nullptr;   // operand base pointer (A operand, [rows][K], K contiguous, leading dimension ld)
+  long ld = 0, rows = 0, K = 0;
+  int s = 0;
+  int8_t *slices = nullptr;    // [s][rows][ldp] with ldp = 2K rounded up to 16 bytes
+  double *scale = nullptr;     // [rows] powers of two above the row maxima
+  size_t bytes = 0;
+};
+struct OzWorkspace {
+  int slices = 0;                             // 0 = off; 2..8 slices of 7 bits (6 + 7(s-1) bits below each row maximum are kept)
+  int force_bn = 0, force_cm = 0, force_cn = 0;   // tile width / cluster shape overrides (tuning runs); 0 = chosen per call
+  cudaEvent_t ev_b[2] = {nullptr, nullptr};   // when set: recorded around the slicing of B (cclr_zgemm_oz timing)
+  std::vector<OzEntry> persist;               // slices of constant A operands (W_vvvv, W_ovvo): made once, see zgemm_oz_register
+  size_t persist_bytes = 0;
+  int8_t *scratch[2] = {nullptr, nullptr};    // per-call slices of an unregistered A operand / of the B operand
+  size_t scratch_bytes[2] = {0, 0};
+  double *scale[2] = {nullptr, nullptr};
+  size_t scale_bytes[2] = {0, 0};
+};
+bool zgemm_oz_eligible(int M, int N, int K);
+cudaError_t zgemm_oz(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *A, long lda, bool conjA, const c128 *B, long ldb,
+                     bool b_is_kn, bool conjB, c128 beta, c128 *C, long ldc, OzWorkspace *ow);
+cudaError_t zgemm_oz_register(cudaStream_t st, OzWorkspace *ow, const c128 *A, long lda, long rows, long K);
+void zgemm_oz_release(OzWorkspace *ow);
 
 // ---- zgemm_lp.cu: the same product in reduced precision (tcgen05.mma, BF16 planes, FP32 accumulators in tensor memory) ----
 // Used only by the inner (preconditioning) solve of cclr_solve: see zgemm_lp.cu and DESIGN.md "Solver".

@@ -86,6 +86,7 @@ void destroy(cclr_ctx *ctx) {
   if (ctx->ws.buf) cudaFree(ctx->ws.buf);
   if (ctx->ws.plane) cudaFree(ctx->ws.plane);
   if (ctx->wplane) cudaFree(ctx->wplane);
+  zgemm_oz_release(&ctx->oz);
   if (ctx->D) cudaFree(ctx->D);
   if (ctx->dot_partial) cudaFree(ctx->dot_partial);
   if (ctx->dot_out) cudaFree(ctx->dot_out);
@@ -276,6 +277,22 @@ extern "C" int cclr_create(int o, int v, const cclr_c128 *fock, const cclr_eri_p
       }
     }
 
+    // integer slices of the two big constant operands of sigma -- the A operands of the ladder and of the ring -- for the INT8
+    // tensor path (zgemm_oz.cu), when the shapes are eligible and the slices (3/4 of the operands) fit comfortably
+    if (!(flags & (CCLR_GEMM_DMMA | CCLR_GEMM_4M)) && zgemm_oz_eligible((int)ctx->vv, (int)ctx->oo, (int)ctx->vv)) {
+      const long ov = (long)o * v;
+      const bool ring_too = zgemm_oz_eligible((int)ov, (int)ov, (int)ov);
+      const size_t need = (size_t)12 * ctx->vv * ctx->vv + (ring_too ? (size_t)12 * ov * ov : 0);
+      size_t free_b = 0, total_b = 0;
+      if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess && free_b > need + need / 2) {
+        ctx->oz.slices = 6;
+        check(zgemm_oz_register(ctx->st, &ctx->oz, P.buf(P.find("Wabef")).ptr, ctx->vv, ctx->vv, ctx->vv), "integer slices of W_vvvv");
+        if (ring_too) check(zgemm_oz_register(ctx->st, &ctx->oz, P.buf(P.find("Wring")).ptr, ov, ov, ov), "integer slices of W_ovvo");
+        ctx->extra_bytes += ctx->oz.persist_bytes;
+        ctx->ws.oz = &ctx->oz;
+      }
+    }
+
     check(cudaMalloc(&ctx->D, (size_t)(ctx->n1 + ctx->n2) * sizeof(double)), "cudaMalloc(D)");
     ctx->extra_bytes += (size_t)(ctx->n1 + ctx->n2) * sizeof(double);
     check(denominators(ctx->st, F, o, v, ctx->D), "denominators");
@@ -323,6 +340,19 @@ extern "C" int cclr_create(int o, int v, const cclr_c128 *fock, const cclr_eri_p
 }
 
 extern "C" void cclr_destroy(cclr_ctx *ctx) { destroy(ctx); }
+
+extern "C" int cclr_set_gemm_path(cclr_ctx *ctx, int path) {
+  if (!ctx) return CCLR_EINVAL;
+  if (ctx->st) cudaStreamSynchronize(ctx->st);
+  OzWorkspace *want = (path != 0 && ctx->oz.slices > 0 && !ctx->oz.persist.empty()) ? &ctx->oz : nullptr;
+  if (want != ctx->ws.oz) {
+    ctx->ws.oz = want;
+    if (ctx->sigma_graph) { cudaGraphExecDestroy(ctx->sigma_graph); ctx->sigma_graph = nullptr; }   // captured with the other path
+    if (ctx->graph_io) { cudaFree(ctx->graph_io); ctx->graph_io = nullptr; ctx->extra_bytes -= 2 * (size_t)(ctx->n1 + ctx->n2) * sizeof(c128); }
+    if (ctx->graph_stream) { cudaStreamDestroy(ctx->graph_stream); ctx->graph_stream = nullptr; }
+  }
+  return ctx->ws.oz ? 1 : 0;
+}
 
 extern "C" size_t cclr_ctx_bytes(const cclr_ctx *ctx) {
   return ctx ? ctx->plan->owned_bytes() + ctx->extra_bytes : 0;

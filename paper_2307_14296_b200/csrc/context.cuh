@@ -11,6 +11,7 @@ struct cclr_ctx {
   cudaStream_t st = nullptr;
   Plan *plan = nullptr;
   ZgemmWorkspace ws;
+  OzWorkspace oz;                 // integer-slice product of ladder / ring (CCLR_GEMM_OZAKI): slices of W_vvvv, W_ovvo + scratch
   double *wplane = nullptr;       // persistent sum plane Re + Im of W_vvvv for the 3M ladder (ws.persist_*), or null
   std::vector<ResolvedOp> sigma_ops, ladder_ops, ring_ops, xi_ops, left_ops, eta_ops, eta_eom_ops;
   c128 *xblocks = nullptr;        // X_oo, X_ov, X_vo, X_vv of cclr_xi, contiguous

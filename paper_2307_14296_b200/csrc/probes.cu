@@ -223,3 +223,42 @@ extern "C" int cclr_zgemm(void *cuda_stream, int M, int N, int K, const cclr_c12
   if (e != cudaSuccess) { g_last_cuda_error = e; return CCLR_ECUDA; }
   return CCLR_OK;
 }
+
+extern "C" int cclr_zgemm_oz(void *cuda_stream, int M, int N, int K, const cclr_c128 *alpha, const cclr_c128 *A, long lda, int conj_a,
+                             const cclr_c128 *B, long ldb, int b_is_kn, int conj_b, const cclr_c128 *beta, cclr_c128 *C, long ldc,
+                             int slices, int bn, int reps, double *ms) {
+  if (!alpha || !beta || !A || !B || !C || reps < 1 || slices < 2 || slices > 8 || !zgemm_oz_eligible(M, N, K)) return CCLR_EINVAL;
+  if (lda < K || ldc < N || (b_is_kn ? ldb < N : ldb < K)) return CCLR_EINVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  OzWorkspace ow;
+  ow.slices = slices;
+  ow.force_bn = bn % 1000;                  // bn + 1000 * c_n + 10000 * c_m forces the cluster shape as well (tuning runs)
+  ow.force_cn = (bn / 1000) % 10;
+  ow.force_cm = bn >= 1000 ? (bn / 10000 > 0 ? bn / 10000 : 1) : 0;
+  cudaEvent_t ev[6];
+  for (auto &e : ev) cudaEventCreate(&e);
+  ow.ev_b[0] = ev[4]; ow.ev_b[1] = ev[5];
+  cudaEventRecord(ev[0], st);
+  cudaError_t e = zgemm_oz_register(st, &ow, (const c128 *)A, lda, M, K);
+  cudaEventRecord(ev[1], st);
+  // reps > 1: the first product is an untimed warm-up (it allocates the B scratch); reps == 1 runs exactly one product
+  const int first = reps > 1 ? 1 : 0;
+  for (int r = 0; r < reps + first && e == cudaSuccess; ++r) {
+    if (r == first) cudaEventRecord(ev[2], st);
+    e = zgemm_oz(st, M, N, K, make_double2(alpha->re, alpha->im), (const c128 *)A, lda, conj_a != 0, (const c128 *)B, ldb,
+                 b_is_kn != 0, conj_b != 0, make_double2(beta->re, beta->im), (c128 *)C, ldc, &ow);
+  }
+  cudaEventRecord(ev[3], st);
+  const cudaError_t e2 = cudaStreamSynchronize(st);
+  if (e == cudaSuccess) e = e2;
+  if (e == cudaSuccess && ms) {
+    float t = 0.f;
+    cudaEventElapsedTime(&t, ev[0], ev[1]); ms[0] = t;
+    cudaEventElapsedTime(&t, ev[2], ev[3]); ms[1] = t / reps;
+    cudaEventElapsedTime(&t, ev[4], ev[5]); ms[2] = t;
+  }
+  for (auto &x : ev) cudaEventDestroy(x);
+  zgemm_oz_release(&ow);
+  if (e != cudaSuccess) { g_last_cuda_error = e; return CCLR_ECUDA; }
+  return CCLR_OK;
+}

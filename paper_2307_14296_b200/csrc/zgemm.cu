@@ -765,6 +765,13 @@ cudaError_t zgemm(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *
                   const c128 *B, long ldb, bool b_is_kn, bool conjB, c128 beta, c128 *C, long ldc, int batch, long sa,
                   long sb, long sc, const ZgemmWorkspace *ws) {
   if (M <= 0 || N <= 0 || batch <= 0) return cudaSuccess;
+  // integer-slice product on the INT8 tensor path (zgemm_oz.cu) for contractions whose A operand has registered slices
+  // (the context's W_vvvv and W_ovvo: ladder and ring of sigma)
+  if (ws && ws->oz && ws->oz->slices > 0 && batch == 1 && zgemm_oz_eligible(M, N, K)) {
+    for (const OzEntry &e : ws->oz->persist)
+      if (e.key == A && e.ld == lda && e.rows == M && e.K == K)
+        return zgemm_oz(st, M, N, K, alpha, A, lda, conjA, B, ldb, b_is_kn, conjB, beta, C, ldc, ws->oz);
+  }
   constexpr int BK = ZG_BK;
   const int sms = zgemm_num_sms();
   // 64-row tiles when they cut the padding of M by more than 10 % (M of a few hundred: 300 -> 320 instead of 384)

@@ -170,6 +170,65 @@ def test_zgemm_3m_component_accuracy_when_one_part_is_tiny():
         assert rel(Cd.cpu().numpy(), Ac @ Br) < 1e-14, mode
 
 
+@pytest.mark.parametrize("M,N,K,kn,ca,cb,beta,slices", [
+    (512, 32, 512, False, False, False, 0.0, 6), (700, 77, 1000, True, False, False, 0.0, 6),
+    (515, 130, 777, False, True, False, 1.0, 6), (515, 130, 777, True, False, True, -0.5, 6),
+    (1300, 561, 1000, True, True, True, 0.0, 6), (1024, 300, 2048, False, False, False, 1.0, 7),
+    (2100, 520, 4099, False, False, True, 0.0, 6), (600, 1030, 515, True, False, False, 0.0, 8),
+    (1024, 300, 2048, True, False, False, 0.0, 3), (1024, 300, 2048, True, False, False, 0.0, 4),
+])
+def test_zgemm_integer_slice_product_matches_numpy(M, N, K, kn, ca, cb, beta, slices):
+    """zgemm_oz (csrc/zgemm_oz.cu): the complex128 product from INT8 slices on tcgen05.mma.kind::i8 with S32 accumulators in tensor
+    memory.  The integer products are exact, so the error is the truncation of the operands 6 + 7 (s - 1) bits below their row /
+    column maxima: for Gaussian operands norm-wise ~30 * 2^(-7 s).  Asserted: 2^(-7 s + 6) (s = 6: 1.5e-11, an order
+    below north_star's 1e-10 for sigma), ragged M / N / K, both B layouts, conjugations, complex alpha, beta, several tile widths
+    and (K = 4099) a split anti-diagonal.  Per 128 x 64 block as well, so that a wrong tile or scale cannot hide in the norm."""
+    cc = _lib()
+    rng = np.random.default_rng(M + N + K + slices)
+    A = rng.normal(size=(M, K)) + 1j * rng.normal(size=(M, K))
+    B = rng.normal(size=(K, N) if kn else (N, K)) + 1j * rng.normal(size=(K, N) if kn else (N, K))
+    C0 = rng.normal(size=(M, N)) + 1j * rng.normal(size=(M, N))
+    alpha = -0.4 + 0.9j
+    opA = A.conj() if ca else A
+    opB = B.conj() if cb else B
+    prod = alpha * (opA @ (opB if kn else opB.T))
+    ref = prod + beta * C0
+    Cd = torch.from_numpy(C0.copy()).cuda()
+    cc.cclr_zgemm_oz(torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda(), Cd, alpha=alpha, beta=beta, conj_a=ca, conj_b=cb,
+                     b_is_kn=kn, slices=slices)
+    torch.cuda.synchronize()
+    got = Cd.cpu().numpy()
+    tol = max(2.0 ** (-7 * slices + 6), 2e-14)
+    assert np.linalg.norm(got - ref) < tol * np.linalg.norm(prod)
+    for i0 in range(0, M, 128):
+        for j0 in range(0, N, 64):
+            blk = (slice(i0, i0 + 128), slice(j0, j0 + 64))
+            assert np.linalg.norm(got[blk] - ref[blk]) < 4 * tol * np.linalg.norm(prod[blk]), (i0, j0)
+
+
+def test_zgemm_integer_slice_product_is_limited_by_the_row_maximum():
+    """What the slicing does NOT keep: elements far below the largest element of their row (of A) or column (of B)
+    are truncated 41 bits below that maximum, not below themselves.  One outlier of 1e6 in every row of A costs six digits --
+    stated here so that the limit is documented by a test, like the 3M component test above."""
+    cc = _lib()
+    rng = np.random.default_rng(9)
+    M, N, K = 640, 96, 700
+    A = rng.normal(size=(M, K)) + 1j * rng.normal(size=(M, K))
+    B = rng.normal(size=(K, N)) + 1j * rng.normal(size=(K, N))
+    A[:, 5] *= 1e6
+    B[5, :] = 0.0                      # the outlier column meets a zero row: it sets the scale and contributes nothing
+    ref = A @ B
+    Cd = torch.zeros((M, N), dtype=torch.complex128, device="cuda")
+    cc.cclr_zgemm_oz(torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda(), Cd, b_is_kn=True, slices=6)
+    torch.cuda.synchronize()
+    err = rel(Cd.cpu().numpy(), ref)
+    assert 1e-9 < err < 1e-4
+    Cd.zero_()
+    cc.cclr_zgemm_oz(torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda(), Cd, b_is_kn=True, slices=8)
+    torch.cuda.synchronize()
+    assert rel(Cd.cpu().numpy(), ref) < 1e-8
+
+
 def test_zgemm_batched_and_strided():
     cc = _lib()
     rng = np.random.default_rng(5)
@@ -226,7 +285,10 @@ def test_create_intermediates_match_oracle(o, v, flags):
     assert not bad, bad
 
 
-@pytest.mark.parametrize("o,v,flags,nvec", [(3, 5, 0, 1), (4, 7, 2, 2), (4, 20, 0, 3), (6, 40, 0, 1), (6, 40, 4, 1)])
+@pytest.mark.parametrize("o,v,flags,nvec", [(3, 5, 0, 1), (4, 7, 2, 2), (4, 20, 0, 3), (6, 40, 0, 1), (6, 40, 4, 1),
+                                            (9, 34, 0, 2),      # vv = 561, oo = 36: the ladder runs on the INT8 tensor path
+                                            (10, 52, 0, 1),     # ... and the ring (ov = 520)
+                                            (9, 34, 32, 1), (10, 52, 32, 1)])   # CCLR_GEMM_DMMA: the same on the FP64 tensor cores
 def test_sigma_matches_oracle(o, v, flags, nvec):
     cc = _lib()
     s = make_system(o, v, seed=o * 100 + v + 1)
