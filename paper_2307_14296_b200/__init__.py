@@ -383,8 +383,7 @@ def cclr_ring(ctx, x2, out2=None):
 def cclr_zgemm(A, B, C_out, alpha=1.0, beta=0.0, conj_a=False, conj_b=False, b_is_kn=False, M=None, N=None, K=None,
                lda=None, ldb=None, ldc=None, batch=1, sa=0, sb=0, sc=0, three_m=True):
     """C = alpha opA(A) opB(B) + beta C on 2-D (or batched 3-D) row-major tensors; see include/cclr.h.
-    three_m: large shapes use the 3M complex product (False: 4M everywhere); the integer 2 selects the reduced-precision
-    product of the inner solver (BF16 tcgen05, FP32 accumulation: ~3 significant digits)."""
+    three_m: large shapes use the 3M complex product (False: 4M everywhere)."""
     if M is None:
         M, K = A.shape[-2], A.shape[-1]
         N = B.shape[-1] if b_is_kn else B.shape[-2]
@@ -395,7 +394,7 @@ def cclr_zgemm(A, B, C_out, alpha=1.0, beta=0.0, conj_a=False, conj_b=False, b_i
     al, be = _lib.Complex(complex(alpha).real, complex(alpha).imag), _lib.Complex(complex(beta).real, complex(beta).imag)
     rc = _lib.load().cclr_zgemm(_stream(), M, N, K, C.byref(al), _dev(A, "A"), lda, int(conj_a), _dev(B, "B"), ldb,
                                 int(b_is_kn), int(conj_b), C.byref(be), _dev(C_out, "C"), ldc, batch, sa, sb, sc,
-                                2 if three_m == 2 and three_m is not True else int(bool(three_m)))
+                                int(bool(three_m)))
     _lib.check(rc, "cclr_zgemm")
     return C_out
 

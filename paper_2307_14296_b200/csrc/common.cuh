@@ -81,28 +81,6 @@ cudaError_t zgemm_oz(cudaStream_t st, int M, int N, int K, c128 alpha, const c12
 cudaError_t zgemm_oz_register(cudaStream_t st, OzWorkspace *ow, const c128 *A, long lda, long rows, long K);
 void zgemm_oz_release(OzWorkspace *ow);
 
-// ---- zgemm_lp.cu: the same product in reduced precision (tcgen05.mma, BF16 planes, FP32 accumulators in tensor memory) ----
-// Used only by the inner (preconditioning) solve of cclr_solve: see zgemm_lp.cu and DESIGN.md "Solver".
-struct LpCacheEntry {
-  const c128 *key = nullptr;   // operand base pointer
-  long rows = 0, kdim = 0, ld = 0;
-  bool transposed = false, conj = false;
-  uint16_t *planes = nullptr;  // BF16 re plane [rows][ldp] followed by the im plane
-  size_t bytes = 0;
-};
-struct LpWorkspace {
-  bool enabled = false;                       // the plan routes eligible GEMMs through zgemm_lp while this is set
-  uint16_t *scratch[2] = {nullptr, nullptr};  // per-call planes of the A / B operand (operands that change between calls)
-  size_t scratch_elems[2] = {0, 0};
-  std::vector<LpCacheEntry> cache;            // planes of constant operands (the context's persistent intermediates)
-  size_t cache_bytes = 0, cache_budget = 0;
-};
-bool zgemm_lp_eligible(int M, int N, int K);
-// a_const / b_const: the operand never changes for the lifetime of lw (its planes are converted once and cached)
-cudaError_t zgemm_lp(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *A, long lda, bool conjA, bool a_const,
-                     const c128 *B, long ldb, bool b_is_kn, bool conjB, bool b_const, c128 beta, c128 *C, long ldc, LpWorkspace *lw);
-void zgemm_lp_release(LpWorkspace *lw);
-
 // ---- permute.cu: generic index-permutation / pair (un)packing / antisymmetrising gather-scatter kernel ---------
 // dst(iteration index) (+)= sum_k coef_k * sign_k * [conj] src_k(slots(letters)); see plans.inc for the semantics.
 constexpr int PERM_MAX_AXES = 6, PERM_MAX_SLOTS = 5, PERM_MAX_SRC = 10, PERM_MAX_LETTERS = 12;

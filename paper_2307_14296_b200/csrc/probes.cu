@@ -191,18 +191,6 @@ extern "C" int cclr_zgemm(void *cuda_stream, int M, int N, int K, const cclr_c12
   if (K > 0 && (!A || !B)) return CCLR_EINVAL;
   if (lda < K || ldc < N || (b_is_kn ? ldb < N : ldb < K)) return CCLR_EINVAL;
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  if (three_m == 2) {   // the reduced-precision product of the inner solver (zgemm_lp.cu): BF16 tcgen05, FP32 accumulation
-    if (batch != 1 || !zgemm_lp_eligible(M, N, K)) return CCLR_EINVAL;
-    LpWorkspace lw;
-    cudaError_t e = zgemm_lp(st, M, N, K, make_double2(alpha->re, alpha->im), (const c128 *)A, lda, conj_a != 0, false,
-                             (const c128 *)B, ldb, b_is_kn != 0, conj_b != 0, false, make_double2(beta->re, beta->im), (c128 *)C,
-                             ldc, &lw);
-    const cudaError_t e2 = cudaStreamSynchronize(st);
-    zgemm_lp_release(&lw);
-    if (e == cudaSuccess) e = e2;
-    if (e != cudaSuccess) { g_last_cuda_error = e; return CCLR_ECUDA; }
-    return CCLR_OK;
-  }
   // K-split workspace for this stand-alone entry point (the context keeps its own): room for 3 partial tiles per SM
   ZgemmWorkspace ws;
   ws.elems = (size_t)3 * zgemm_num_sms() * 128 * 64;

@@ -171,6 +171,14 @@ def test_sigma_T0_sampled_elements_at_full_size(cfg):
     w_rows = np.stack([row(r) for r in rows])
     want = sampled.ladder_rows(w_rows, x2[0].cpu().numpy().reshape(vv, oo))
     got = lad[0].view(vv, oo)[rows].cpu().numpy()
+    # default path at this size: 6 integer slices on the INT8 tensor path, operands truncated 41 bits below their row maxima ->
+    # 2^-35 norm-wise (measured 6e-12); the FP64 tensor-core (DMMA) path of the same context: rounding level
+    assert ctx.set_gemm_path(1) == 1
+    assert np.linalg.norm(got - want) <= 2.0 ** -35 * np.linalg.norm(want)
+    assert ctx.set_gemm_path(0) == 0
+    lad = cc.cclr_ladder(ctx, x2[:1].contiguous())
+    torch.cuda.synchronize()
+    got = lad[0].view(vv, oo)[rows].cpu().numpy()
     assert np.linalg.norm(got - want) <= 1e-12 * np.linalg.norm(want)
     ctx.close()
     del ctx, lad, s1, s2, x1, x2
@@ -190,13 +198,17 @@ def test_properties_at_full_size_with_T(cfg):
     a, b = 0.3 - 1.1j, -0.7 + 0.2j
     y1 = (a * x1[0] + b * x1[1])[None].contiguous()
     y2 = (a * x2[0] + b * x2[1])[None].contiguous()
-    o1, o2 = cc.cclr_sigma(ctx, x1, x2)
-    p1, p2 = cc.cclr_sigma(ctx, y1, y2)
     rel = lambda u, w: float((u - w).abs().pow(2).sum().sqrt() / w.abs().pow(2).sum().sqrt())
-    assert rel(p2[0], a * o2[0] + b * o2[1]) < 1e-12
-    assert rel(p1[0], a * o1[0] + b * o1[1]) < 1e-12
-    zz = 0.0773 + 0.0045j
-    q1, q2 = cc.cclr_sigma(ctx, x1, x2, zz.real, zz.imag)
-    assert rel(q2, o2 - zz * x2) < 1e-14 and rel(q1, o1 - zz * x1) < 1e-14
+    # path 1 (default at this size): ladder and ring as integer-slice products -- the slicing of the trial vector is not a linear
+    # map, so linearity holds to the truncation level (sigma tolerance 1e-10); path 0: DMMA, rounding level
+    for path, tol in ((1, 1e-10), (0, 1e-12)):
+        assert ctx.set_gemm_path(path) == path
+        o1, o2 = cc.cclr_sigma(ctx, x1, x2)
+        p1, p2 = cc.cclr_sigma(ctx, y1, y2)
+        assert rel(p2[0], a * o2[0] + b * o2[1]) < tol, path
+        assert rel(p1[0], a * o1[0] + b * o1[1]) < tol, path
+        zz = 0.0773 + 0.0045j
+        q1, q2 = cc.cclr_sigma(ctx, x1, x2, zz.real, zz.imag)
+        assert rel(q2, o2 - zz * x2) < 1e-14 and rel(q1, o1 - zz * x1) < 1e-14
     ctx.close()
     torch.cuda.empty_cache()
