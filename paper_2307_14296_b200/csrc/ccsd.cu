@@ -56,6 +56,8 @@ struct Engine {
   const cclr_c128 *fock;
   const cclr_eri_packed *eri;
   Plan P;
+  ZgemmWorkspace ws;
+  OzWorkspace oz;      // integer-slice product (zgemm_oz.cu) for the contractions of the residual that dominate an iteration
   Buf fblocks, S, TS, coef;
   const c128 *W0 = nullptr, *fovT = nullptr, *fvo = nullptr;
   int t1_id = -1, t2_id = -1;
@@ -88,8 +90,29 @@ struct Engine {
     t1_id = P.find("t1");
     t2_id = P.find("t2");
     P.execute(PLAN_OMEGA0);
+    P.set_workspace(&ws);
     W0 = P.buf(P.find("W0")).ptr;
     fovT = P.buf(P.find("fovT")).ptr;
+  }
+
+  ~Engine() { zgemm_oz_release(&oz); }
+
+  // The iteration of cclr_ccsd evaluates the residual ~100 times on the same integrals: the two contractions with a constant big
+  // A operand -- <ab||ef> tau (the pp ladder) and <ma||ef> tau -- get registered integer slices, the three ring-shaped ones slice
+  // their operands per call (zgemm.cu dispatch).  7 slices (48 bits below the row maxima, ~1e-13 norm-wise) so that the fixed point
+  // of the iteration is the fixed point of the FP64 residual to well below the 1e-10 convergence threshold.  Skipped when the
+  // shapes are not eligible or the slices (7/8 of the operands) do not fit comfortably.
+  void enable_integer_slices() {
+    const long vv = npair(v), oo = npair(o), ov = (long)o * v;
+    if (!zgemm_oz_eligible((int)vv, (int)oo, (int)vv)) return;
+    const size_t need = (size_t)14 * vv * vv + (size_t)14 * ov * vv;
+    size_t free_b = 0, total_b = 0;
+    if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess || free_b < 2 * need) return;
+    oz.slices = 7;
+    check(zgemm_oz_register(st, &oz, (const c128 *)eri->vvvv, vv, vv, vv), "integer slices of <ab||ef>");
+    if (zgemm_oz_eligible((int)ov, (int)oo, (int)vv))
+      check(zgemm_oz_register(st, &oz, (const c128 *)eri->ovvv, vv, ov, vv), "integer slices of <ma||ef>");
+    ws.oz = &oz;
   }
 
   // mode 0: OM = Omega(T) by the direct residual plan
@@ -196,6 +219,7 @@ extern "C" int cclr_ccsd(int o, int v, const cclr_c128 *fock, const cclr_eri_pac
     check(cudaMalloc(&D, (size_t)n * sizeof(double)), "cudaMalloc(D)");
     struct FreeD { double *p; ~FreeD() { cudaFree(p); } } freeD{D};
     check(denominators(st, (const c128 *)fock, o, v, D), "denominators");
+    E.enable_integer_slices();
     check(cudaMemcpyAsync(T.p, t1, (size_t)n1 * sizeof(c128), cudaMemcpyDeviceToDevice, st), "copy t1");
     check(cudaMemcpyAsync(T.p + n1, t2, (size_t)n2 * sizeof(c128), cudaMemcpyDeviceToDevice, st), "copy t2");
 
