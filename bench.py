@@ -218,6 +218,7 @@ def ground_state(cc, torch, synth, o, v, f, eri, cfg, mode):
                 return blob["t1"], blob["t2"], "cclr_ccsd converged (cached; ||Omega|| = %.1e re-evaluated)" % res, blob["info"]
         except Exception:
             pass
+    torch.cuda.empty_cache()      # cclr_ccsd sizes its integer-slice operands from the free device memory
     t1, t2, g = cc.cclr_ccsd(o, v, f, eri, t1, t2, tol=1e-10, maxiter=150)
     info = {"iterations": g.iterations, "residual": g.residual, "energy_re": g.energy_re, "energy_im": g.energy_im, "seconds": g.seconds}
     try:
@@ -414,6 +415,9 @@ def run_ours(args):
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": workload_name(args.config, o, v), "o": o, "v": v, "nvec": nvec, "omega": omega,
+                   "arithmetic": ("complex128 in and out; ladder and ring as integer-slice products on the INT8 tensor path at FP64 accuracy "
+                                  "(6 slices of 7 bits, S32 accumulation, FP64 recombination; sigma parity 1e-10 holds, DESIGN.md 6.1b), "
+                                  "everything else on the FP64 tensor cores" if oz_on else "complex128 on the FP64 tensor cores (DMMA)"),
                    "gamma": gamma, "sigma_V": synth.sigma_v(v), "ground_state": ground_txt, "parallelism": "replicas x%d" % world,
                    "l2": "inputs larger than L2 (W_vvvv %.2f GB streamed every step)" % (npair(v) ** 2 * 16 / 1e9),
                    "flops_per_step": flops_step, "complex_product": args.gemm, "context_bytes": ctx.bytes()},
@@ -436,8 +440,7 @@ def run_ours(args):
         lad_ms = phases["ladder"] / (args.steps * nvec)
         lad_flops8 = 8.0 * cm["T11"]
         traffic, traffic_src = measured_ladder_traffic(args.gemm, args.config)
-        oz_ladder = args.gemm == "oz" and cc.cclr_zgemm_oz_eligible(npair(v), npair(o), npair(v))
-        if oz_ladder:
+        if oz_on:
             # the ladder runs as 21 INT8 slice-pair products (6 slices, t + u <= 5) of the real embedding: 4 real multiply-adds per
             # complex one, 2 ops each -> 21 * 8 vv^2 oo integer ops; peak = measured cuBLAS bf16 (sustained: the kernel is timed inside
             # a long step) x 2, the nominal INT8 : bf16 ratio of the chip (4.5 : 2.25 Pop/s)

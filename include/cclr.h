@@ -63,11 +63,15 @@ typedef struct {
 
 #define CCLR_GEMM_DMMA 32u  /* keep EVERY contraction on the FP64 tensor cores (DMMA).  Default: the two contractions that are 91 % of
                                cclr_sigma -- the pp ladder T11 and the ring T8 -- run on the INT8 tensor path at FP64 accuracy when
-                               their shapes allow (vv >= 512, oo >= 32): the context keeps 6 integer slices of 7 bits of W_vvvv and
+                               their shapes allow (vv >= 512, oo >= 32 and at least 64 output tiles of 256 x 256 reals: configs 3, 4, 5): the context keeps 6 integer slices of 7 bits of W_vvvv and
                                W_ovvo (3/4 of their size) and slices the trial vector per call (cclr_zgemm_oz; csrc/zgemm_oz.cu;
                                DESIGN.md 6.1b).  The slice product holds north_star's 1e-10 on sigma (~1e-11 measured); every
                                other contraction, cclr_create and the left transform are DMMA either way.  CCLR_GEMM_4M implies
                                this flag.  cclr_set_gemm_path switches an existing context. */
+
+#define CCLR_GEMM_INT8_ANY_SIZE 64u /* testing aid: ladder and ring take the INT8 tensor path at ANY size the kernel supports (default: only
+                               where it pays, from 64 output tiles of 256 x 256 reals), so that small inputs can be compared with
+                               the full-tensor oracle through that path */
 
 #define CCLR_SMALL_CHUNKS 2u /* testing aid: run the chunked intermediate builds with chunks of 3 indices so that small
                                inputs exercise several chunks and a ragged last one (results are unchanged) */
@@ -252,7 +256,7 @@ int cclr_zgemm(void *cuda_stream, int M, int N, int K, const cclr_c128 *alpha, c
  * column of B is scaled by a power of two and cut into `slices` (2..8) signed slices of 7 bits; the slices * (slices + 1) / 2
  * integer products with t + u < slices are exact, so the only error is the truncation of the operands 6 + 7 (slices - 1) bits below
  * their row / column maxima (slices = 6: norm-wise ~1e-11 for rows without outliers; it holds north_star's 1e-10 on sigma).
- * Shapes: M >= 512, N >= 32, 512 <= K < 2^17 (else CCLR_EINVAL).  reps >= 1 repeats the product (timing); ms (HOST, may be NULL)
+ * Shapes: M >= 512, N >= 32, 512 <= K < 2^17 and at least 64 output tiles, ceil(M / 256) * ceil(2 N / 256) >= 64 (else CCLR_EINVAL).  reps >= 1 repeats the product (timing); ms (HOST, may be NULL)
  * receives ms[0] = slicing A (done once), ms[1] = one product including the slicing of B, ms[2] = the slicing of B alone
  * (CUDA events on the stream).  bn = 0 picks the tile width and cluster shape; else bn % 1000 forces the width (multiple of 16 in
  * [16, 256]) and (bn / 1000) % 10, bn / 10000 the CTAs of a cluster along N and M (tuning runs).  With beta != 0 use reps = 1. */

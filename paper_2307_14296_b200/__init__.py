@@ -41,6 +41,7 @@ GEMM_4M = 4
 NO_GRAPH = 8
 NO_SUM_PLANES = 16
 GEMM_DMMA = 32
+GEMM_INT8_ANY_SIZE = 64
 
 
 class Context:
@@ -401,7 +402,7 @@ def cclr_zgemm(A, B, C_out, alpha=1.0, beta=0.0, conj_a=False, conj_b=False, b_i
 
 def cclr_zgemm_oz_eligible(M, N, K):
     """Whether the integer-slice product takes this shape (include/cclr.h: cclr_zgemm_oz)."""
-    return M >= 512 and N >= 32 and 512 <= K < (1 << 17)
+    return M >= 512 and N >= 32 and 512 <= K < (1 << 17) and ((M + 255) // 256) * ((2 * N + 255) // 256) >= 64
 
 
 def cclr_zgemm_oz(A, B, C_out, alpha=1.0, beta=0.0, conj_a=False, conj_b=False, b_is_kn=False, slices=6, bn=0, reps=1):

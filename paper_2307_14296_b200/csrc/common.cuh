@@ -66,6 +66,7 @@ struct OzEntry {
 };
 struct OzWorkspace {
   int slices = 0;                             // 0 = off; 2..8 slices of 7 bits (6 + 7(s-1) bits below each row maximum are kept)
+  bool any_size = false;                      // testing aid (CCLR_GEMM_INT8_ANY_SIZE): registered operands use the path at any supported size
   int force_bn = 0, force_cm = 0, force_cn = 0;   // tile width / cluster shape overrides (tuning runs); 0 = chosen per call
   cudaEvent_t ev_b[2] = {nullptr, nullptr};   // when set: recorded around the slicing of B (cclr_zgemm_oz timing)
   std::vector<OzEntry> persist;               // slices of constant A operands (W_vvvv, W_ovvo): made once, see zgemm_oz_register
@@ -75,7 +76,8 @@ struct OzWorkspace {
   double *scale[2] = {nullptr, nullptr};
   size_t scale_bytes[2] = {0, 0};
 };
-bool zgemm_oz_eligible(int M, int N, int K);
+bool zgemm_oz_supported(int M, int N, int K);   // the kernel can run the shape
+bool zgemm_oz_eligible(int M, int N, int K);    // ... and it pays (what the dispatch in zgemm() uses)
 cudaError_t zgemm_oz(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *A, long lda, bool conjA, const c128 *B, long ldb,
                      bool b_is_kn, bool conjB, c128 beta, c128 *C, long ldc, OzWorkspace *ow);
 cudaError_t zgemm_oz_register(cudaStream_t st, OzWorkspace *ow, const c128 *A, long lda, long rows, long K);

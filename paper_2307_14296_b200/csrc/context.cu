@@ -279,9 +279,12 @@ extern "C" int cclr_create(int o, int v, const cclr_c128 *fock, const cclr_eri_p
 
     // integer slices of the two big constant operands of sigma -- the A operands of the ladder and of the ring -- for the INT8
     // tensor path (zgemm_oz.cu), when the shapes are eligible and the slices (3/4 of the operands) fit comfortably
-    if (!(flags & (CCLR_GEMM_DMMA | CCLR_GEMM_4M)) && zgemm_oz_eligible((int)ctx->vv, (int)ctx->oo, (int)ctx->vv)) {
+    const bool any_size = (flags & CCLR_GEMM_INT8_ANY_SIZE) != 0;
+    if (!(flags & (CCLR_GEMM_DMMA | CCLR_GEMM_4M)) &&
+        (any_size ? zgemm_oz_supported((int)ctx->vv, (int)ctx->oo, (int)ctx->vv) : zgemm_oz_eligible((int)ctx->vv, (int)ctx->oo, (int)ctx->vv))) {
       const long ov = (long)o * v;
-      const bool ring_too = zgemm_oz_eligible((int)ov, (int)ov, (int)ov);
+      const bool ring_too = any_size ? zgemm_oz_supported((int)ov, (int)ov, (int)ov) : zgemm_oz_eligible((int)ov, (int)ov, (int)ov);
+      ctx->oz.any_size = any_size;
       const size_t need = (size_t)12 * ctx->vv * ctx->vv + (ring_too ? (size_t)12 * ov * ov : 0);
       size_t free_b = 0, total_b = 0;
       if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess && free_b > need + need / 2) {

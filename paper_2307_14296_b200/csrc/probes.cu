@@ -215,7 +215,7 @@ extern "C" int cclr_zgemm(void *cuda_stream, int M, int N, int K, const cclr_c12
 extern "C" int cclr_zgemm_oz(void *cuda_stream, int M, int N, int K, const cclr_c128 *alpha, const cclr_c128 *A, long lda, int conj_a,
                              const cclr_c128 *B, long ldb, int b_is_kn, int conj_b, const cclr_c128 *beta, cclr_c128 *C, long ldc,
                              int slices, int bn, int reps, double *ms) {
-  if (!alpha || !beta || !A || !B || !C || reps < 1 || slices < 2 || slices > 8 || !zgemm_oz_eligible(M, N, K)) return CCLR_EINVAL;
+  if (!alpha || !beta || !A || !B || !C || reps < 1 || slices < 2 || slices > 8 || !zgemm_oz_supported(M, N, K)) return CCLR_EINVAL;
   if (lda < K || ldc < N || (b_is_kn ? ldb < N : ldb < K)) return CCLR_EINVAL;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   OzWorkspace ow;

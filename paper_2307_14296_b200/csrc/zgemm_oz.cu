@@ -505,9 +505,16 @@ cudaError_t oz_ensure(cudaStream_t st, void **ptr, size_t *have, size_t need) {
 
 }  // namespace
 
+bool zgemm_oz_supported(int M, int N, int K) {
+  // what the kernel can do: 2K * 64^2 must leave room for one slice pair in an S32 accumulator
+  return M >= 1 && N >= 1 && K >= 1 && (long)K < (1L << 17);
+}
+
 bool zgemm_oz_eligible(int M, int N, int K) {
-  // large contractions only; 2K * 64^2 must leave room for at least one pair in an S32 accumulator
-  return M >= 512 && N >= 32 && K >= 512 && (long)K < (1L << 17);
+  // large contractions only: at least 64 output tiles of 256 x 256 reals (below that the 148 SMs are not filled and the DMMA kernels
+  // with their smaller tiles win: config 2's ladder is 13 tiles), and 2K * 64^2 must leave room for one pair in an S32 accumulator
+  if (M < 512 || N < 32 || K < 512 || (long)K >= (1L << 17)) return false;
+  return (long)((M + 255) / 256) * ((2L * N + 255) / 256) >= 64;
 }
 
 void zgemm_oz_release(OzWorkspace *ow) {
@@ -546,7 +553,7 @@ cudaError_t zgemm_oz_register(cudaStream_t st, OzWorkspace *ow, const c128 *A, l
 
 cudaError_t zgemm_oz(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *A, long lda, bool conjA, const c128 *B, long ldb,
                      bool b_is_kn, bool conjB, c128 beta, c128 *C, long ldc, OzWorkspace *ow) {
-  if (!ow || ow->slices < 2 || ow->slices > 8 || !zgemm_oz_eligible(M, N, K)) return cudaErrorInvalidValue;
+  if (!ow || ow->slices < 2 || ow->slices > 8 || !zgemm_oz_supported(M, N, K)) return cudaErrorInvalidValue;
   const int s = ow->slices;
   const long ldp = oz_ldp(K);
   // ---- A: registered slices, else sliced into scratch 0 ----

@@ -255,9 +255,10 @@ def test_create_intermediates_match_oracle(o, v, flags):
 
 
 @pytest.mark.parametrize("o,v,flags,nvec", [(3, 5, 0, 1), (4, 7, 2, 2), (4, 20, 0, 3), (6, 40, 0, 1), (6, 40, 4, 1),
-                                            (9, 34, 0, 2),      # vv = 561, oo = 36: the ladder runs on the INT8 tensor path
-                                            (10, 52, 0, 1),     # ... and the ring (ov = 520)
-                                            (9, 34, 32, 1), (10, 52, 32, 1)])   # CCLR_GEMM_DMMA: the same on the FP64 tensor cores
+                                            # CCLR_GEMM_INT8_ANY_SIZE: ladder and ring on the INT8 tensor path at sizes the
+                                            # full oracle can do (several tile rows, ragged: vv = 561 / 1326, ov = 306 / 520)
+                                            (9, 34, 64, 2), (10, 52, 64, 1), (10, 52, 64 | 2, 1),
+                                            (10, 52, 32, 1)])   # CCLR_GEMM_DMMA: the same on the FP64 tensor cores
 def test_sigma_matches_oracle(o, v, flags, nvec):
     cc = _lib()
     s = make_system(o, v, seed=o * 100 + v + 1)
