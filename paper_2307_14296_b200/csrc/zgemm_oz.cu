@@ -21,12 +21,17 @@
 //     accumulator as long as  pairs * 2K * 64^2 < 2^31  (otherwise the diagonal is split into several accumulation groups);
 //     each group is converted to FP64, scaled (exactly) and added to C in the epilogue -- smallest diagonals last.
 //
-// Kernel: one CTA per 256 x BN output tile (BN <= 256 real columns, chosen per call for the least padded 2N); two 128-row
+// Kernel: one CTA per 256 x BN output tile (BN <= 256 real columns, chosen per call from a port / pipe cost model); two 128-row
 // tcgen05.mma halves with their accumulators side by side in the 512 columns of tensor memory.  warp 0 = TMA producer (3-D
 // maps {k, row, slice} over the INT8 slices, 128 B x rows boxes, SWIZZLE_128B = the canonical K-major layout of the shared-
 // memory matrix descriptors), warp 1 = MMA issue (one lane; 8 MMAs of 128 x BN x 32 per 128-byte k block), warps 2-9 =
-// epilogue (tcgen05.ld 32x32b, S32 -> FP64, read-modify-write of the C tile).  3-stage ring of 64 KB stages with full / empty
-// mbarriers; tcgen05.commit frees a stage and hands the accumulators to the epilogue at the end of each accumulation group.
+// epilogue (tcgen05.ld 32x32b, S32 -> FP64, read-modify-write of the C tile).  Ring of as many (32 KB + BN x 128 B) stages as fit
+// 227 KB (3 or 4) with full / empty mbarriers; tcgen05.commit frees a stage and hands the accumulators to the epilogue at the
+// end of each accumulation group.
+// Clusters: the CTAs of c_m x c_n adjacent tiles form a thread-block cluster and share operand tiles by TMA multicast -- the
+// A tile along a cluster row, the B tile along a cluster column; the CTAs take turns as the loader of a stage and the
+// "slot consumed" commits are multicast to the peers, which keeps a cluster in lock-step.  For the ladder one cluster spans all
+// tile columns of a row panel, so W_vvvv's slices leave HBM once per use (538 GB -> 104 GB per call at config 4, profiles/).
 #include "common.cuh"
 #include <algorithm>
 #include <atomic>
