@@ -237,6 +237,7 @@ def build_workload(cc, torch, synth, cfg, o, v, nvec, seed, ground, gemm="3m", g
     f = synth.fock(o, v, seed=0).to(dev)
     t1, t2, ground_txt, ground_info = ground_state(cc, torch, synth, o, v, f, eri, cfg, ground)
     torch.cuda.synchronize()
+    torch.cuda.empty_cache()      # cclr_create sizes its optional operand copies (sum plane, integer slices) from the free device memory
     l0 = cc.cclr_kernel_launches()
     t0 = time.perf_counter()
     ctx = cc.cclr_create(o, v, f, eri, t1, t2, cc.ERI_INPLACE | (cc.GEMM_4M if gemm == "4m" else 0) | (cc.GEMM_DMMA if gemm == "3m" else 0)

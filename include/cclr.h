@@ -69,6 +69,10 @@ typedef struct {
                                other contraction, cclr_create and the left transform are DMMA either way.  CCLR_GEMM_4M implies
                                this flag.  cclr_set_gemm_path switches an existing context. */
 
+#define CCLR_NO_LEFT_SLICES 128u /* do not keep the integer slices of W_vvvv's transpose (another 3/4 of W_vvvv) that put the transposed
+                               ladder of cclr_sigma_left / cclr_f_transform on the INT8 tensor path as well (default: kept when
+                               the free device memory allows); the left ladder then runs on the FP64 tensor cores */
+
 #define CCLR_GEMM_INT8_ANY_SIZE 64u /* testing aid: ladder and ring take the INT8 tensor path at ANY size the kernel supports (default: only
                                where it pays, from 64 output tiles of 256 x 256 reals), so that small inputs can be compared with
                                the full-tensor oracle through that path */
@@ -258,7 +262,8 @@ int cclr_zgemm(void *cuda_stream, int M, int N, int K, const cclr_c128 *alpha, c
  * their row / column maxima (slices = 6: norm-wise ~1e-11 for rows without outliers; it holds north_star's 1e-10 on sigma).
  * Shapes: M >= 512, N >= 32, 512 <= K < 2^17 and at least 64 output tiles, ceil(M / 256) * ceil(2 N / 256) >= 64 (else CCLR_EINVAL).  reps >= 1 repeats the product (timing); ms (HOST, may be NULL)
  * receives ms[0] = slicing A (done once), ms[1] = one product including the slicing of B, ms[2] = the slicing of B alone
- * (CUDA events on the stream).  bn = 0 picks the tile width and cluster shape; else bn % 1000 forces the width (multiple of 16 in
+ * (CUDA events on the stream).  slices + 100 (b_is_kn only): B is the constant operand -- its TRANSPOSE is sliced once and the
+ * product runs as C^T = B^T A^T with a transposed store (the route of the left transform's ladder).  bn = 0 picks the tile width and cluster shape; else bn % 1000 forces the width (multiple of 16 in
  * [16, 256]) and (bn / 1000) % 10, bn / 10000 the CTAs of a cluster along N and M (tuning runs).  With beta != 0 use reps = 1. */
 int cclr_zgemm_oz(void *cuda_stream, int M, int N, int K, const cclr_c128 *alpha, const cclr_c128 *A, long lda, int conj_a,
                   const cclr_c128 *B, long ldb, int b_is_kn, int conj_b, const cclr_c128 *beta, cclr_c128 *C, long ldc,

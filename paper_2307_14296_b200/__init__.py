@@ -42,6 +42,7 @@ NO_GRAPH = 8
 NO_SUM_PLANES = 16
 GEMM_DMMA = 32
 GEMM_INT8_ANY_SIZE = 64
+NO_LEFT_SLICES = 128
 
 
 class Context:
@@ -405,15 +406,16 @@ def cclr_zgemm_oz_eligible(M, N, K):
     return M >= 512 and N >= 32 and 512 <= K < (1 << 17) and ((M + 255) // 256) * ((2 * N + 255) // 256) >= 64
 
 
-def cclr_zgemm_oz(A, B, C_out, alpha=1.0, beta=0.0, conj_a=False, conj_b=False, b_is_kn=False, slices=6, bn=0, reps=1):
+def cclr_zgemm_oz(A, B, C_out, alpha=1.0, beta=0.0, conj_a=False, conj_b=False, b_is_kn=False, slices=6, bn=0, reps=1, b_side=False):
     """C = alpha opA(A) opB(B) + beta C on 2-D row-major tensors through the integer-slice product on the INT8 tensor path
-    (include/cclr.h: cclr_zgemm_oz).  Returns (C_out, [ms slicing A, ms per product incl. slicing B, ms slicing B])."""
+    (include/cclr.h: cclr_zgemm_oz).  b_side: B ([K][N]) is the constant operand whose transpose is sliced once (C^T = B^T A^T route).
+    Returns (C_out, [ms slicing the constant operand, ms per product incl. slicing the other one, ms of that slicing])."""
     M, K = A.shape
     N = B.shape[1] if b_is_kn else B.shape[0]
     al, be = _lib.Complex(complex(alpha).real, complex(alpha).imag), _lib.Complex(complex(beta).real, complex(beta).imag)
     ms = (C.c_double * 3)()
     rc = _lib.load().cclr_zgemm_oz(_stream(), M, N, K, C.byref(al), _dev(A, "A"), A.shape[1], int(conj_a), _dev(B, "B"), B.shape[1],
-                                   int(b_is_kn), int(conj_b), C.byref(be), _dev(C_out, "C"), C_out.shape[1], slices, bn, reps, ms)
+                                   int(b_is_kn), int(conj_b), C.byref(be), _dev(C_out, "C"), C_out.shape[1], slices + (100 if b_side else 0), bn, reps, ms)
     _lib.check(rc, "cclr_zgemm_oz")
     return C_out, [ms[0], ms[1], ms[2]]
 

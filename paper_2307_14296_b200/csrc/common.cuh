@@ -60,6 +60,7 @@ struct OzEntry {
   const c128 *key = nullptr;   // operand base pointer (A operand, [rows][K], K contiguous, leading dimension ld)
   long ld = 0, rows = 0, K = 0;
   int s = 0;
+  bool transposed = false;     // slices of the operand's TRANSPOSE: key is stored [K][rows] (zgemm_oz_register_t)
   int8_t *slices = nullptr;    // [s][rows][ldp] with ldp = 2K rounded up to 16 bytes
   double *scale = nullptr;     // [rows] powers of two above the row maxima
   size_t bytes = 0;
@@ -81,6 +82,11 @@ bool zgemm_oz_eligible(int M, int N, int K);    // ... and it pays (what the dis
 cudaError_t zgemm_oz(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *A, long lda, bool conjA, const c128 *B, long ldb,
                      bool b_is_kn, bool conjB, c128 beta, c128 *C, long ldc, OzWorkspace *ow);
 cudaError_t zgemm_oz_register(cudaStream_t st, OzWorkspace *ow, const c128 *A, long lda, long rows, long K);
+// the same for a constant B operand stored [K][N]: slices of its transpose, used by zgemm_oz_bt (C^T = B^T A^T, transposed store)
+cudaError_t zgemm_oz_register_t(cudaStream_t st, OzWorkspace *ow, const c128 *B, long ldb, long K, long N);
+bool zgemm_oz_has_bt(const OzWorkspace *ow, const c128 *B, long ldb, int N, int K);
+cudaError_t zgemm_oz_bt(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *A, long lda, bool conjA, const c128 *B, long ldb,
+                        bool conjB, c128 beta, c128 *C, long ldc, OzWorkspace *ow);
 void zgemm_oz_release(OzWorkspace *ow);
 
 // ---- permute.cu: generic index-permutation / pair (un)packing / antisymmetrising gather-scatter kernel ---------

@@ -291,6 +291,12 @@ extern "C" int cclr_create(int o, int v, const cclr_c128 *fock, const cclr_eri_p
         ctx->oz.slices = 6;
         check(zgemm_oz_register(ctx->st, &ctx->oz, P.buf(P.find("Wabef")).ptr, ctx->vv, ctx->vv, ctx->vv), "integer slices of W_vvvv");
         if (ring_too) check(zgemm_oz_register(ctx->st, &ctx->oz, P.buf(P.find("Wring")).ptr, ov, ov, ov), "integer slices of W_ovvo");
+        // ... and of W_vvvv's transpose for the transposed ladder of the left transform (lambda, left response equations, the F
+        // transform), when another 3/4 of W_vvvv still leaves room for the solvers' trial spaces
+        const size_t need_t = (size_t)12 * ctx->vv * ctx->vv;
+        if (!(flags & CCLR_NO_LEFT_SLICES) && cudaMemGetInfo(&free_b, &total_b) == cudaSuccess &&
+            free_b > need_t + std::max<size_t>((size_t)32 << 30, 64 * (size_t)(ctx->n1 + ctx->n2) * sizeof(c128)))
+          check(zgemm_oz_register_t(ctx->st, &ctx->oz, P.buf(P.find("Wabef")).ptr, ctx->vv, ctx->vv, ctx->vv), "integer slices of W_vvvv^T");
         ctx->extra_bytes += ctx->oz.persist_bytes;
         ctx->ws.oz = &ctx->oz;
       }

@@ -215,7 +215,10 @@ extern "C" int cclr_zgemm(void *cuda_stream, int M, int N, int K, const cclr_c12
 extern "C" int cclr_zgemm_oz(void *cuda_stream, int M, int N, int K, const cclr_c128 *alpha, const cclr_c128 *A, long lda, int conj_a,
                              const cclr_c128 *B, long ldb, int b_is_kn, int conj_b, const cclr_c128 *beta, cclr_c128 *C, long ldc,
                              int slices, int bn, int reps, double *ms) {
+  const bool b_side = slices >= 100;      // slices + 100: B ([K][N]) is the constant operand, C^T = B^T A^T route (zgemm_oz_bt)
+  if (b_side) slices -= 100;
   if (!alpha || !beta || !A || !B || !C || reps < 1 || slices < 2 || slices > 8 || !zgemm_oz_supported(M, N, K)) return CCLR_EINVAL;
+  if (b_side && !b_is_kn) return CCLR_EINVAL;
   if (lda < K || ldc < N || (b_is_kn ? ldb < N : ldb < K)) return CCLR_EINVAL;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   OzWorkspace ow;
@@ -227,14 +230,16 @@ extern "C" int cclr_zgemm_oz(void *cuda_stream, int M, int N, int K, const cclr_
   for (auto &e : ev) cudaEventCreate(&e);
   ow.ev_b[0] = ev[4]; ow.ev_b[1] = ev[5];
   cudaEventRecord(ev[0], st);
-  cudaError_t e = zgemm_oz_register(st, &ow, (const c128 *)A, lda, M, K);
+  cudaError_t e = b_side ? zgemm_oz_register_t(st, &ow, (const c128 *)B, ldb, K, N) : zgemm_oz_register(st, &ow, (const c128 *)A, lda, M, K);
   cudaEventRecord(ev[1], st);
   // reps > 1: the first product is an untimed warm-up (it allocates the B scratch); reps == 1 runs exactly one product
   const int first = reps > 1 ? 1 : 0;
   for (int r = 0; r < reps + first && e == cudaSuccess; ++r) {
     if (r == first) cudaEventRecord(ev[2], st);
-    e = zgemm_oz(st, M, N, K, make_double2(alpha->re, alpha->im), (const c128 *)A, lda, conj_a != 0, (const c128 *)B, ldb,
-                 b_is_kn != 0, conj_b != 0, make_double2(beta->re, beta->im), (c128 *)C, ldc, &ow);
+    e = b_side ? zgemm_oz_bt(st, M, N, K, make_double2(alpha->re, alpha->im), (const c128 *)A, lda, conj_a != 0, (const c128 *)B, ldb,
+                             conj_b != 0, make_double2(beta->re, beta->im), (c128 *)C, ldc, &ow)
+               : zgemm_oz(st, M, N, K, make_double2(alpha->re, alpha->im), (const c128 *)A, lda, conj_a != 0, (const c128 *)B, ldb,
+                          b_is_kn != 0, conj_b != 0, make_double2(beta->re, beta->im), (c128 *)C, ldc, &ow);
   }
   cudaEventRecord(ev[3], st);
   const cudaError_t e2 = cudaStreamSynchronize(st);

@@ -769,9 +769,13 @@ cudaError_t zgemm(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *
   // W_vvvv and W_ovvo: ladder and ring of sigma), and ring-shaped ones (N >= 1024: slicing A per call costs < 10 % of the product)
   // as long as the per-call slices stay small (the transposed ladder of the left transform, 48 GB of them, stays on DMMA)
   if (ws && ws->oz && ws->oz->slices > 0 && batch == 1 && zgemm_oz_supported(M, N, K)) {
+    // the big constant operand on the B side (transposed ladder of the left transform): C^T = B^T A^T on the slices of B^T
+    if (b_is_kn && zgemm_oz_has_bt(ws->oz, B, ldb, N, K) && (zgemm_oz_eligible(N, M, K) || ws->oz->any_size) &&
+        (size_t)ws->oz->slices * 4 * (size_t)K * (size_t)M <= ((size_t)6 << 30))
+      return zgemm_oz_bt(st, M, N, K, alpha, A, lda, conjA, B, ldb, conjB, beta, C, ldc, ws->oz);
     bool registered = false;
     for (const OzEntry &e : ws->oz->persist)
-      if (e.key == A && e.ld == lda && e.rows == M && e.K == K) registered = true;
+      if (!e.transposed && e.key == A && e.ld == lda && e.rows == M && e.K == K) registered = true;
     const bool pays = zgemm_oz_eligible(M, N, K);
     const size_t per_call = (size_t)ws->oz->slices * 2 * (size_t)K * ((registered ? 0 : (size_t)M) + 2 * (size_t)N);
     if (((registered && (pays || ws->oz->any_size)) || (pays && N >= 1024)) && per_call <= ((size_t)6 << 30))

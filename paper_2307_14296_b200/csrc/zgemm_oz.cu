@@ -59,7 +59,7 @@ struct OzArgs {
   uint32_t idesc;
   c128 alpha, beta;
   c128 *C;
-  long ldc;
+  long c_rs, c_cs;                                    // element strides of C along the rows (m) / complex columns (n) of this product
   const double *sa, *sb;                              // 2^ea[m] per row of A, 2^eb[n] per complex column of B
 };
 
@@ -251,7 +251,7 @@ zgemm_oz_kernel(const __grid_constant__ CUtensorMap tA, const __grid_constant__ 
     const uint32_t taddr = tmem + ((uint32_t)(q * 32) << 16) + (uint32_t)h * 256u;
     const bool has_beta = a.beta.x != 0.0 || a.beta.y != 0.0;
     const double rs0 = grow < a.M ? a.sa[grow] : 0.0;
-    c128 *crow = a.C + (grow < a.M ? grow : 0) * a.ldc;
+    c128 *crow = a.C + (grow < a.M ? grow : 0) * a.c_rs;   // c_rs = 1, c_cs = ldc: the product is stored transposed (zgemm_oz_bt)
     const int N = a.N2 >> 1;
     for (int g = 0; g < a.ngroups; ++g) {
       mbar_wait(bar_tfull, (uint32_t)g & 1u);
@@ -270,9 +270,10 @@ zgemm_oz_kernel(const __grid_constant__ CUtensorMap tA, const __grid_constant__ 
               const double sc = rs * a.sb[col];
               const c128 pv = make_double2((double)r[2 * j] * sc, (double)r[2 * j + 1] * sc);
               c128 out = cmul(a.alpha, pv);
-              if (g > 0) out = cadd(out, crow[col]);
-              else if (has_beta) out = cadd(out, cmul(a.beta, crow[col]));
-              crow[col] = out;
+              c128 *cp = crow + (long)col * a.c_cs;
+              if (g > 0) out = cadd(out, *cp);
+              else if (has_beta) out = cadd(out, cmul(a.beta, *cp));
+              *cp = out;
             }
           }
         }
@@ -389,6 +390,8 @@ __global__ void __launch_bounds__(256) oz_slice_rows_kernel(const c128 *__restri
 }
 // B operand stored [K][N] (N contiguous): 64 k x 32 n tiles transposed through shared memory into the same two-rows-per-column
 // K-major layout.  256 threads: tx = column in the tile, ty = 0..7 -> k = ty, ty + 8, ...
+// AFMT: the A-operand format instead (ONE row [re, im]_k per column n: the slices of the operand's transpose, zgemm_oz_register_t).
+template <bool AFMT>
 __global__ void __launch_bounds__(256) oz_slice_kn_kernel(const c128 *__restrict__ X, long ld, long krows, long ncols, int s,
                                                           const double *__restrict__ scale, int8_t *__restrict__ out, long ldp,
                                                           size_t slice_stride, int c0, int c1, int c2) {
@@ -413,17 +416,23 @@ __global__ void __launch_bounds__(256) oz_slice_kn_kernel(const c128 *__restrict
       yr[i] = (yr[i] - qr) * 128.0;
       yi[i] = (yi[i] - qi) * 128.0;
       const int ir = (int)qr, ii = (int)qi, kk = 2 * (ty + 8 * i);
-      tile[2 * tx][kk] = (int8_t)ir;
-      tile[2 * tx][kk + 1] = (int8_t)(c0 * ii);
-      tile[2 * tx + 1][kk] = (int8_t)(c1 * ii);
-      tile[2 * tx + 1][kk + 1] = (int8_t)(c2 * ir);
+      if (AFMT) {
+        tile[tx][kk] = (int8_t)ir;
+        tile[tx][kk + 1] = (int8_t)ii;
+      } else {
+        tile[2 * tx][kk] = (int8_t)ir;
+        tile[2 * tx][kk + 1] = (int8_t)(c0 * ii);
+        tile[2 * tx + 1][kk] = (int8_t)(c1 * ii);
+        tile[2 * tx + 1][kk + 1] = (int8_t)(c2 * ir);
+      }
     }
     __syncthreads();
-    // 64 rows x 128 bytes: warp w writes rows w, w + 8, ...; lane = 4 bytes
-    for (int row = ty; row < 64; row += 8) {
-      const long nn = 2 * n0 + row;
+    // 64 (32) rows x 128 bytes: warp w writes rows w, w + 8, ...; lane = 4 bytes
+    const int nrows = AFMT ? 32 : 64;
+    for (int row = ty; row < nrows; row += 8) {
+      const long nn = (AFMT ? n0 : 2 * n0) + row;
       const long kb = 2 * k0 + 4 * tx;
-      if (nn < 2 * ncols && kb < ldp)
+      if (nn < (AFMT ? ncols : 2 * ncols) && kb < ldp)
         *(uint32_t *)(out + (size_t)t * slice_stride + (size_t)nn * ldp + kb) = *(const uint32_t *)&tile[row][4 * tx];
     }
     __syncthreads();
@@ -489,7 +498,7 @@ cudaError_t oz_slice_b(cudaStream_t st, const c128 *B, long ldb, bool b_is_kn, l
     oz_colmax_kernel<<<g1, 256, 0, st>>>(B, ldb, K, N, kslab, (unsigned long long *)scale);
     oz_scale_finalize_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(scale, N);
     dim3 g2((unsigned)((N + 31) / 32), (unsigned)((K + 63) / 64));
-    oz_slice_kn_kernel<<<g2, 256, 0, st>>>(B, ldb, K, N, s, scale, slices, ldp, (size_t)(2 * N) * ldp, c0, c1, c2);
+    oz_slice_kn_kernel<false><<<g2, 256, 0, st>>>(B, ldb, K, N, s, scale, slices, ldp, (size_t)(2 * N) * ldp, c0, c1, c2);
     cclr_count_launch(3);
   }
   return cudaGetLastError();
@@ -556,28 +565,14 @@ cudaError_t zgemm_oz_register(cudaStream_t st, OzWorkspace *ow, const c128 *A, l
   return cudaSuccess;
 }
 
-cudaError_t zgemm_oz(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *A, long lda, bool conjA, const c128 *B, long ldb,
-                     bool b_is_kn, bool conjB, c128 beta, c128 *C, long ldc, OzWorkspace *ow) {
-  if (!ow || ow->slices < 2 || ow->slices > 8 || !zgemm_oz_supported(M, N, K)) return cudaErrorInvalidValue;
+// The product proper: C'[M][N] = alpha * A'[M][K] * opB(B)[K][N] + beta * C' with A' given as slices + scales (the conjugation of A'
+// is folded into the sign pattern of the B slices), C' addressed as C[m * c_rs + n * c_cs].
+static cudaError_t oz_run(cudaStream_t st, int M, int N, int K, c128 alpha, const int8_t *sa_sl, const double *sa_sc, bool conjA,
+                          const c128 *B, long ldb, bool b_is_kn, bool conjB, c128 beta, c128 *C, long c_rs, long c_cs, OzWorkspace *ow) {
   const int s = ow->slices;
   const long ldp = oz_ldp(K);
-  // ---- A: registered slices, else sliced into scratch 0 ----
-  const int8_t *sa_sl = nullptr;
-  const double *sa_sc = nullptr;
-  for (const auto &e : ow->persist)
-    if (e.key == A && e.ld == lda && e.rows == M && e.K == K && e.s == s) { sa_sl = e.slices; sa_sc = e.scale; }
-  cudaError_t err;
-  if (!sa_sl) {
-    err = oz_ensure(st, (void **)&ow->scratch[0], &ow->scratch_bytes[0], (size_t)s * M * ldp);
-    if (err != cudaSuccess) return err;
-    err = oz_ensure(st, (void **)&ow->scale[0], &ow->scale_bytes[0], (size_t)M * sizeof(double));
-    if (err != cudaSuccess) return err;
-    err = oz_slice_a(st, A, lda, M, K, s, ow->scratch[0], ow->scale[0]);
-    if (err != cudaSuccess) return err;
-    sa_sl = ow->scratch[0]; sa_sc = ow->scale[0];
-  }
   // ---- B: always sliced per call (the trial vector side) ----
-  err = oz_ensure(st, (void **)&ow->scratch[1], &ow->scratch_bytes[1], (size_t)s * 2 * N * ldp);
+  cudaError_t err = oz_ensure(st, (void **)&ow->scratch[1], &ow->scratch_bytes[1], (size_t)s * 2 * N * ldp);
   if (err != cudaSuccess) return err;
   err = oz_ensure(st, (void **)&ow->scale[1], &ow->scale_bytes[1], (size_t)N * sizeof(double));
   if (err != cudaSuccess) return err;
@@ -622,7 +617,7 @@ cudaError_t zgemm_oz(cudaStream_t st, int M, int N, int K, c128 alpha, const c12
   a.npairs = np; a.ngroups = ng;
   // instruction descriptor (kind::i8): D = S32, A = B = signed 8 bit, both K-major, M = 128, N = BN
   a.idesc = (2u << 4) | (1u << 7) | (1u << 10) | (((uint32_t)BN >> 3) << 17) | ((128u >> 4) << 24);
-  a.alpha = alpha; a.beta = beta; a.C = C; a.ldc = ldc;
+  a.alpha = alpha; a.beta = beta; a.C = C; a.c_rs = c_rs; a.c_cs = c_cs;
   a.sa = sa_sc; a.sb = ow->scale[1];
   CUtensorMap tA, tB;
   if (!oz_make_map(&tA, sa_sl, 2L * K, M, ldp, s, OZ_BM) || !oz_make_map(&tB, ow->scratch[1], 2L * K, 2L * N, ldp, s, BN))
@@ -694,4 +689,76 @@ cudaError_t zgemm_oz(cudaStream_t st, int M, int N, int K, c128 alpha, const c12
   if (!launched) return err;
   cclr_count_launch();
   return cudaSuccess;
+}
+
+cudaError_t zgemm_oz(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *A, long lda, bool conjA, const c128 *B, long ldb,
+                     bool b_is_kn, bool conjB, c128 beta, c128 *C, long ldc, OzWorkspace *ow) {
+  if (!ow || ow->slices < 2 || ow->slices > 8 || !zgemm_oz_supported(M, N, K)) return cudaErrorInvalidValue;
+  const int s = ow->slices;
+  const long ldp = oz_ldp(K);
+  // ---- A: registered slices, else sliced into scratch 0 ----
+  const int8_t *sa_sl = nullptr;
+  const double *sa_sc = nullptr;
+  for (const auto &e : ow->persist)
+    if (!e.transposed && e.key == A && e.ld == lda && e.rows == M && e.K == K && e.s == s) { sa_sl = e.slices; sa_sc = e.scale; }
+  if (!sa_sl) {
+    cudaError_t err = oz_ensure(st, (void **)&ow->scratch[0], &ow->scratch_bytes[0], (size_t)s * M * ldp);
+    if (err != cudaSuccess) return err;
+    err = oz_ensure(st, (void **)&ow->scale[0], &ow->scale_bytes[0], (size_t)M * sizeof(double));
+    if (err != cudaSuccess) return err;
+    err = oz_slice_a(st, A, lda, M, K, s, ow->scratch[0], ow->scale[0]);
+    if (err != cudaSuccess) return err;
+    sa_sl = ow->scratch[0]; sa_sc = ow->scale[0];
+  }
+  return oz_run(st, M, N, K, alpha, sa_sl, sa_sc, conjA, B, ldb, b_is_kn, conjB, beta, C, ldc, 1, ow);
+}
+
+// Slices of the TRANSPOSE of a constant operand stored [K][N] (N contiguous, leading dimension ldb): rows n = [re, im]_k, scaled
+// by the column maxima.  For products in which the big constant matrix is the B operand (the transposed ladder of the left
+// transform, O2T[(ij);(ef)] = l2T[(ij);(ab)] . W[(ab);(ef)]): zgemm_oz_bt then runs C^T = B^T . A^T with these slices on the A side.
+cudaError_t zgemm_oz_register_t(cudaStream_t st, OzWorkspace *ow, const c128 *B, long ldb, long K, long N) {
+  if (!ow || ow->slices < 2 || ow->slices > 8) return cudaErrorInvalidValue;
+  OzEntry e;
+  e.key = B; e.ld = ldb; e.rows = N; e.K = K; e.s = ow->slices; e.transposed = true;
+  const long ldp = oz_ldp(K);
+  const size_t bytes = (size_t)e.s * (size_t)N * (size_t)ldp;
+  cudaError_t err = cudaMalloc((void **)&e.slices, bytes);
+  if (err != cudaSuccess) return err;
+  err = cudaMalloc((void **)&e.scale, (size_t)N * sizeof(double));
+  if (err != cudaSuccess) { cudaFree(e.slices); return err; }
+  err = cudaMemsetAsync(e.scale, 0, (size_t)N * sizeof(double), st);
+  if (err == cudaSuccess) {
+    const long kslab = 256;
+    dim3 g1((unsigned)((N + 255) / 256), (unsigned)((K + kslab - 1) / kslab));
+    oz_colmax_kernel<<<g1, 256, 0, st>>>(B, ldb, K, N, kslab, (unsigned long long *)e.scale);
+    oz_scale_finalize_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(e.scale, N);
+    dim3 g2((unsigned)((N + 31) / 32), (unsigned)((K + 63) / 64));
+    oz_slice_kn_kernel<true><<<g2, 256, 0, st>>>(B, ldb, K, N, e.s, e.scale, e.slices, ldp, (size_t)N * ldp, 1, 1, 1);
+    cclr_count_launch(3);
+    err = cudaGetLastError();
+  }
+  if (err != cudaSuccess) { cudaFree(e.slices); cudaFree(e.scale); return err; }
+  e.bytes = bytes + (size_t)N * sizeof(double);
+  ow->persist.push_back(e);
+  ow->persist_bytes += e.bytes;
+  return cudaSuccess;
+}
+
+bool zgemm_oz_has_bt(const OzWorkspace *ow, const c128 *B, long ldb, int N, int K) {
+  if (!ow) return false;
+  for (const auto &e : ow->persist)
+    if (e.transposed && e.key == B && e.ld == ldb && e.rows == N && e.K == K && e.s == ow->slices) return true;
+  return false;
+}
+
+// C[M][N] = alpha opA(A)[M][K] opB(B)[K][N] + beta C with B stored [K][N] and registered by zgemm_oz_register_t: computed as
+// C^T = opB(B)^T . opA(A)^T -- B's transposed slices are the A side, A ([M][K], K contiguous) is the per-call side, and the
+// epilogue stores transposed (consecutive lanes = consecutive n: coalesced).
+cudaError_t zgemm_oz_bt(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *A, long lda, bool conjA, const c128 *B, long ldb,
+                        bool conjB, c128 beta, c128 *C, long ldc, OzWorkspace *ow) {
+  if (!ow || ow->slices < 2 || ow->slices > 8 || !zgemm_oz_supported(N, M, K)) return cudaErrorInvalidValue;
+  for (const auto &e : ow->persist)
+    if (e.transposed && e.key == B && e.ld == ldb && e.rows == N && e.K == K && e.s == ow->slices)
+      return oz_run(st, N, M, K, alpha, e.slices, e.scale, conjB, A, lda, false, conjA, beta, C, 1, ldc, ow);
+  return cudaErrorInvalidValue;
 }
