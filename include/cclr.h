@@ -273,6 +273,11 @@ int cclr_zgemm_oz(void *cuda_stream, int M, int N, int K, const cclr_c128 *alpha
  * i.e. was created without CCLR_GEMM_DMMA / CCLR_GEMM_4M at an eligible size) and DMMA (path = 0).  Returns the path now in use. */
 int cclr_set_gemm_path(cclr_ctx *ctx, int path);
 
+/* Number of integer slices per operand the context's INT8 tensor path works with (6 for integrals without outliers inside their
+ * rows; 7 or 8 when cclr_create found a wider range, from the rms over the rows of (power-of-two row scale / row rms) of W_vvvv and
+ * W_ovvo, so that 2^(-7 s) rho^2 <= 3e-11), or 0 when ladder and ring run on the FP64 tensor cores. */
+int cclr_gemm_slices(const cclr_ctx *ctx);
+
 /* The particle-particle ladder alone (term T11 of S-Eq. 12):
  * out2[k][ab][ij] = sum_{e<f} W_vvvv[ab][ef] x2[k][ef][ij] for nvec vectors (no shift, no other term). */
 int cclr_ladder(cclr_ctx *ctx, const cclr_c128 *x2, int nvec, cclr_c128 *out2);

@@ -97,6 +97,10 @@ class Context:
         Returns the path now in use."""
         return int(_lib.load().cclr_set_gemm_path(self.handle, int(path)))
 
+    def gemm_slices(self):
+        """Integer slices per operand of the INT8 tensor path in use (0: ladder and ring on the FP64 tensor cores)."""
+        return int(_lib.load().cclr_gemm_slices(self.handle))
+
     def set_profiling(self, on):
         _lib.check(_lib.load().cclr_set_profiling(self.handle, int(bool(on))), "cclr_set_profiling")
 

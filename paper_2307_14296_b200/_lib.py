@@ -73,6 +73,7 @@ SIGNATURES = {
                              c128_p, C.c_long, C.c_int, C.c_int, C.POINTER(Complex), c128_p, C.c_long, C.c_int,
                              C.c_long, C.c_long, C.c_long, C.c_int]),
     "cclr_set_gemm_path": (C.c_int, [C.c_void_p, C.c_int]),
+    "cclr_gemm_slices": (C.c_int, [C.c_void_p]),
     "cclr_zgemm_oz": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.POINTER(Complex), c128_p, C.c_long, C.c_int,
                                 c128_p, C.c_long, C.c_int, C.c_int, C.POINTER(Complex), c128_p, C.c_long, C.c_int, C.c_int,
                                 C.c_int, C.POINTER(C.c_double)]),

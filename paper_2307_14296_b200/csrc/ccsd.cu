@@ -108,7 +108,10 @@ struct Engine {
     const size_t need = (size_t)14 * vv * vv + (size_t)14 * ov * vv;
     size_t free_b = 0, total_b = 0;
     if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess || free_b < 2 * need) return;
-    oz.slices = 7;
+    int s_need = 0;      // one slice more than the range inside the rows asks for (zgemm_oz_suggest_slices: 6 for this task's integrals)
+    check(zgemm_oz_suggest_slices(st, (const c128 *)eri->vvvv, vv, vv, vv, &s_need, nullptr), "row statistics of <ab||ef>");
+    if (s_need == 0 || s_need + 1 > 8) return;
+    oz.slices = s_need + 1;
     check(zgemm_oz_register(st, &oz, (const c128 *)eri->vvvv, vv, vv, vv), "integer slices of <ab||ef>");
     if (zgemm_oz_eligible((int)ov, (int)oo, (int)vv))
       check(zgemm_oz_register(st, &oz, (const c128 *)eri->ovvv, vv, ov, vv), "integer slices of <ma||ef>");

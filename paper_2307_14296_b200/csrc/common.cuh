@@ -81,6 +81,8 @@ bool zgemm_oz_supported(int M, int N, int K);   // the kernel can run the shape
 bool zgemm_oz_eligible(int M, int N, int K);    // ... and it pays (what the dispatch in zgemm() uses)
 cudaError_t zgemm_oz(cudaStream_t st, int M, int N, int K, c128 alpha, const c128 *A, long lda, bool conjA, const c128 *B, long ldb,
                      bool b_is_kn, bool conjB, c128 beta, c128 *C, long ldc, OzWorkspace *ow);
+// slice count (6..8) that holds ~3e-11 norm-wise for an operand with this range inside its rows, 0 if none does (zgemm_oz.cu)
+cudaError_t zgemm_oz_suggest_slices(cudaStream_t st, const c128 *A, long lda, long rows, long K, int *slices, double *rho_out);
 cudaError_t zgemm_oz_register(cudaStream_t st, OzWorkspace *ow, const c128 *A, long lda, long rows, long K);
 // the same for a constant B operand stored [K][N]: slices of its transpose, used by zgemm_oz_bt (C^T = B^T A^T, transposed store)
 cudaError_t zgemm_oz_register_t(cudaStream_t st, OzWorkspace *ow, const c128 *B, long ldb, long K, long N);

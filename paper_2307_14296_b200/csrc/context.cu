@@ -287,13 +287,19 @@ extern "C" int cclr_create(int o, int v, const cclr_c128 *fock, const cclr_eri_p
       ctx->oz.any_size = any_size;
       const size_t need = (size_t)12 * ctx->vv * ctx->vv + (ring_too ? (size_t)12 * ov * ov : 0);
       size_t free_b = 0, total_b = 0;
-      if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess && free_b > need + need / 2) {
-        ctx->oz.slices = 6;
+      // slice count from the range inside the rows of the two operands (6 for integrals without outliers; more slices are more
+      // products: 7 -> 28 pairs instead of 21; beyond 8 the contractions stay on the FP64 tensor cores)
+      int s_lad = 0, s_ring = 0;
+      check(zgemm_oz_suggest_slices(ctx->st, P.buf(P.find("Wabef")).ptr, ctx->vv, ctx->vv, ctx->vv, &s_lad, nullptr), "row statistics of W_vvvv");
+      if (ring_too) check(zgemm_oz_suggest_slices(ctx->st, P.buf(P.find("Wring")).ptr, ov, ov, ov, &s_ring, nullptr), "row statistics of W_ovvo");
+      const int s_need = (s_lad == 0 || (ring_too && s_ring == 0)) ? 0 : std::max(s_lad, s_ring);
+      if (s_need > 0 && cudaMemGetInfo(&free_b, &total_b) == cudaSuccess && free_b > need * s_need / 6 + need / 2) {
+        ctx->oz.slices = s_need;
         check(zgemm_oz_register(ctx->st, &ctx->oz, P.buf(P.find("Wabef")).ptr, ctx->vv, ctx->vv, ctx->vv), "integer slices of W_vvvv");
         if (ring_too) check(zgemm_oz_register(ctx->st, &ctx->oz, P.buf(P.find("Wring")).ptr, ov, ov, ov), "integer slices of W_ovvo");
         // ... and of W_vvvv's transpose for the transposed ladder of the left transform (lambda, left response equations, the F
         // transform), when another 3/4 of W_vvvv still leaves room for the solvers' trial spaces
-        const size_t need_t = (size_t)12 * ctx->vv * ctx->vv;
+        const size_t need_t = (size_t)2 * s_need * ctx->vv * ctx->vv;
         if (!(flags & CCLR_NO_LEFT_SLICES) && cudaMemGetInfo(&free_b, &total_b) == cudaSuccess &&
             free_b > need_t + std::max<size_t>((size_t)32 << 30, 64 * (size_t)(ctx->n1 + ctx->n2) * sizeof(c128)))
           check(zgemm_oz_register_t(ctx->st, &ctx->oz, P.buf(P.find("Wabef")).ptr, ctx->vv, ctx->vv, ctx->vv), "integer slices of W_vvvv^T");
@@ -349,6 +355,8 @@ extern "C" int cclr_create(int o, int v, const cclr_c128 *fock, const cclr_eri_p
 }
 
 extern "C" void cclr_destroy(cclr_ctx *ctx) { destroy(ctx); }
+
+extern "C" int cclr_gemm_slices(const cclr_ctx *ctx) { return (ctx && ctx->ws.oz) ? ctx->oz.slices : 0; }
 
 extern "C" int cclr_set_gemm_path(cclr_ctx *ctx, int path) {
   if (!ctx) return CCLR_EINVAL;

@@ -318,6 +318,35 @@ __global__ void __launch_bounds__(256) oz_rowmax_kernel(const c128 *__restrict__
     __syncthreads();
   }
 }
+// acc[0] += sum over rows of (2^E_r)^2 / mean(x^2 over the row), acc[1] += number of non-zero rows: the dynamic range the slicing
+// has to cover (zgemm_oz_suggest_slices)
+__global__ void __launch_bounds__(256) oz_rowstats_kernel(const c128 *__restrict__ X, long ld, long rows, long cols, double *acc) {
+  __shared__ double redm[8], reds[8];
+  for (long r = blockIdx.x; r < rows; r += gridDim.x) {
+    const c128 *x = X + r * ld;
+    double mx = 0.0, ss = 0.0;
+    for (long c = threadIdx.x; c < cols; c += 256) {
+      const c128 v = x[c];
+      mx = fmax(mx, fmax(fabs(v.x), fabs(v.y)));
+      ss += v.x * v.x + v.y * v.y;
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+      mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+      ss += __shfl_xor_sync(0xffffffffu, ss, o);
+    }
+    if ((threadIdx.x & 31) == 0) { redm[threadIdx.x >> 5] = mx; reds[threadIdx.x >> 5] = ss; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      for (int w = 1; w < 8; ++w) { mx = fmax(mx, redm[w]); ss += reds[w]; }
+      if (mx > 0.0 && ss > 0.0) {
+        const double sc = pow2_above(mx);
+        atomicAdd(acc, sc * sc * (2.0 * (double)cols) / ss);
+        atomicAdd(acc + 1, 1.0);
+      }
+    }
+    __syncthreads();
+  }
+}
 // column maxima of X [krows][ncols] (N contiguous): bit patterns of |x| through atomicMax, then 2^E in place
 __global__ void __launch_bounds__(256) oz_colmax_kernel(const c128 *__restrict__ X, long ld, long krows, long ncols, long kslab,
                                                         unsigned long long *__restrict__ mxbits) {
@@ -529,6 +558,31 @@ bool zgemm_oz_eligible(int M, int N, int K) {
   // with their smaller tiles win: config 2's ladder is 13 tiles), and 2K * 64^2 must leave room for one pair in an S32 accumulator
   if (M < 512 || N < 32 || K < 512 || (long)K >= (1L << 17)) return false;
   return (long)((M + 255) / 256) * ((2L * N + 255) / 256) >= 64;
+}
+
+// How many slices a constant operand needs.  The error of the product is ~ 2^(-7s) rho_A rho_B with rho = (power-of-two row scale) /
+// (row rms), taken as the rms over the rows (rows without outliers: rho = 4.5 ... 9 for Gaussian entries; measured 1e-11 at s = 6).
+// Assuming the other operand is no worse, s is the smallest count with 2^(-7s) rho^2 <= 3e-11 -- 6 for the integrals of this task, 7
+// or 8 for operands with a wider range inside their rows, 0 (do not use the integer path) beyond that.
+cudaError_t zgemm_oz_suggest_slices(cudaStream_t st, const c128 *A, long lda, long rows, long K, int *slices, double *rho_out) {
+  *slices = 0;
+  double *acc = nullptr, h[2] = {0.0, 0.0};
+  cudaError_t err = cudaMalloc((void **)&acc, 2 * sizeof(double));
+  if (err != cudaSuccess) return err;
+  err = cudaMemsetAsync(acc, 0, 2 * sizeof(double), st);
+  if (err == cudaSuccess) {
+    oz_rowstats_kernel<<<(unsigned)std::min<long>(rows, 148 * 16), 256, 0, st>>>(A, lda, rows, K, acc);
+    cclr_count_launch();
+    err = cudaMemcpyAsync(h, acc, 2 * sizeof(double), cudaMemcpyDeviceToHost, st);
+  }
+  if (err == cudaSuccess) err = cudaStreamSynchronize(st);
+  cudaFree(acc);
+  if (err != cudaSuccess) return err;
+  const double rho2 = h[1] > 0.0 ? h[0] / h[1] : 1.0;
+  if (rho_out) *rho_out = std::sqrt(rho2);
+  for (int s = 6; s <= 8; ++s)
+    if (std::ldexp(rho2, -7 * s) <= 3e-11) { *slices = s; break; }
+  return cudaSuccess;
 }
 
 void zgemm_oz_release(OzWorkspace *ow) {

@@ -300,6 +300,34 @@ def test_sigma_matches_oracle(o, v, flags, nvec):
     ctx.close()
 
 
+def test_slice_count_follows_the_range_inside_the_rows():
+    """cclr_create picks the slice count of the INT8 tensor path from the data (include/cclr.h: cclr_gemm_slices): 6 for the synthetic
+    integrals; with the diagonal of <ab||ef> scaled by 1000 (still Hermitian) every row has one element far above the rest, six slices
+    would lose ~3 digits, and the context takes 8 -- sigma keeps north_star's 1e-10 against the oracle on the same integrals."""
+    cc = _lib()
+    o, v = 9, 34
+    s = make_system(o, v, seed=77)
+    ctx = gpu_context(s, cc.GEMM_INT8_ANY_SIZE)
+    assert ctx.gemm_slices() == 6
+    ctx.close()
+    vv = v * (v - 1) // 2
+    idx = torch.arange(vv)
+    s["eri"]["vvvv"] = s["eri"]["vvvv"].clone()
+    s["eri"]["vvvv"].view(vv, vv)[idx, idx] *= 1000.0
+    full = packing.unpack_eri(o, v, {k: x.numpy() for k, x in s["eri"].items()})
+    ints = ccsd.Integrals(o, v, s["fock"].numpy(), **full)
+    ctx = gpu_context(s, cc.GEMM_INT8_ANY_SIZE)
+    assert ctx.gemm_slices() in (7, 8)
+    c = cclr.CCLR(ints, s["t1f"], s["t2f"])
+    x1, x2 = synth.amplitudes(o, v, seed=3, cls1="x1", cls2="x2")
+    o1, o2 = cc.cclr_sigma(ctx, x1.cuda(), x2.cuda(), 0.0773, 0.0045)
+    torch.cuda.synchronize()
+    r1, r2 = c.sigma(*packing.unpack_amplitudes(x1[0].numpy(), x2[0].numpy(), o, v), z=0.0773 + 0.0045j)
+    r1p, r2p = packing.pack_amplitudes(r1, r2)
+    assert rel(o1[0].cpu().numpy(), r1p.reshape(-1)) < 1e-10 and rel(o2[0].cpu().numpy(), r2p.reshape(-1)) < 1e-10
+    ctx.close()
+
+
 def test_ladder_and_ring_terms_match_oracle():
     cc = _lib()
     o, v = 4, 20
