@@ -90,12 +90,19 @@ struct Engine {
     t1_id = P.find("t1");
     t2_id = P.find("t2");
     P.execute(PLAN_OMEGA0);
+    // split-K workspace of the GEMM engine: the one-index intermediates of the residual are M, N <= v contractions over K = v oo
+    // ... o vv (1 - 25 output tiles); without the K split each of them runs on a handful of SMs (130 ms each at config 4)
+    ws.elems = (size_t)8 << 20;
+    if (cudaMalloc(&ws.buf, ws.elems * sizeof(c128)) != cudaSuccess) { cudaGetLastError(); ws.buf = nullptr; ws.elems = 0; }
     P.set_workspace(&ws);
     W0 = P.buf(P.find("W0")).ptr;
     fovT = P.buf(P.find("fovT")).ptr;
   }
 
-  ~Engine() { zgemm_oz_release(&oz); }
+  ~Engine() {
+    zgemm_oz_release(&oz);
+    if (ws.buf) cudaFree(ws.buf);
+  }
 
   // The iteration of cclr_ccsd evaluates the residual ~100 times on the same integrals: the two contractions with a constant big
   // A operand -- <ab||ef> tau (the pp ladder) and <ma||ef> tau -- get registered integer slices, the three ring-shaped ones slice
