@@ -140,6 +140,7 @@ def test_zgemm_3m_component_accuracy_when_one_part_is_tiny():
 
 
 @pytest.mark.parametrize("M,N,K,kn,ca,cb,beta,slices", [
+    (66, 6, 66, True, False, False, 0.0, 6), (3, 5, 7, False, True, False, 1.0, 6),      # far below one tile
     (512, 32, 512, False, False, False, 0.0, 6), (700, 77, 1000, True, False, False, 0.0, 6),
     (515, 130, 777, False, True, False, 1.0, 6), (515, 130, 777, True, False, True, -0.5, 6),
     (1300, 561, 1000, True, True, True, 0.0, 6), (1024, 300, 2048, False, False, False, 1.0, 7),
