@@ -67,6 +67,8 @@ struct OzEntry {
 };
 struct OzWorkspace {
   int slices = 0;                             // 0 = off; 2..8 slices of 7 bits (6 + 7(s-1) bits below each row maximum are kept)
+  int active = 0;                             // 0 = all slices; 2 .. slices - 1: the next products use only the leading `active` slices of every
+                                              // operand (precision on demand: the response solver lowers it as its residual falls)
   bool any_size = false;                      // testing aid (CCLR_GEMM_INT8_ANY_SIZE): registered operands use the path at any supported size
   int force_bn = 0, force_cm = 0, force_cn = 0;   // tile width / cluster shape overrides (tuning runs); 0 = chosen per call
   cudaEvent_t ev_b[2] = {nullptr, nullptr};   // when set: recorded around the slicing of B (cclr_zgemm_oz timing)
@@ -151,6 +153,8 @@ cudaError_t block_lincomb(cudaStream_t st, int R, c128 *Y, long ldy, const c128 
 // y[i] = alpha * x[i] / (z - D[i])      (orbital-energy preconditioner)
 cudaError_t precondition(cudaStream_t st, c128 *y, const c128 *x, const double *D, c128 z, c128 alpha, long n);
 cudaError_t scale_vec(cudaStream_t st, c128 *y, c128 alpha, long n);
+// out[0] += sum_i |s[i] - D[i] b[i]|^2 (device double, zeroed by the caller)
+cudaError_t offdiag_norm2(cudaStream_t st, const c128 *s, const c128 *b, const double *D, long n, double *out);
 // out[i] = src[i] + alpha * x[i]
 cudaError_t shifted_copy(cudaStream_t st, c128 *out, const c128 *src, c128 alpha, const c128 *x, long n);
 // D1[a,i] = eps_a - eps_i, D2[(ab),(ij)] = eps_a + eps_b - eps_i - eps_j from the diagonal of fock ([n][n])

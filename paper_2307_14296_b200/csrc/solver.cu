@@ -15,6 +15,7 @@
 // many simultaneous systems, the residual block R = xi + beta^T [sigma; -z b] as two DMMA GEMMs.
 #include "subspace.cuh"
 #include <chrono>
+#include <cstdlib>
 
 namespace {
 
@@ -170,9 +171,17 @@ static int solve_impl(cclr_ctx *ctx, const cclr_c128 *xi1, const cclr_c128 *xi2,
       int iter = 0;
       bool all_done = std::all_of(done.begin(), done.end(), [](int d) { return d != 0; });
 
+      // precision on demand (subspace.cuh): on the integer-slice path the sigma vectors of late trial vectors use fewer slices
+      S.adapt_tol = getenv("CCLR_SOLVER_ALL_SLICES") ? 0.0 : tol;
       while (!all_done) {
         ++iter;
         // ---- step 2: sigma vectors of the new trial vectors, reduced matrix (Eq. 29) ----
+        S.adapt_relres = 1.0;
+        if (iter > 1) {
+          S.adapt_relres = 0.0;
+          for (int sidx = 0; sidx < nsys; ++sidx)
+            if (!done[sidx]) S.adapt_relres = std::max(S.adapt_relres, relres[sidx]);
+        }
         S.extend(L0);
         L0 = S.L;
         const int L = S.L;
@@ -258,6 +267,23 @@ static int solve_impl(cclr_ctx *ctx, const cclr_c128 *xi1, const cclr_c128 *xi2,
         }
         // ---- convergence and step 5: solutions t = sum_j beta_j b_j of the converged systems ----
         const bool last = iter >= maxiter;
+        // a system whose recurrence residual has converged is accepted only if the estimated contribution of the reduced-precision
+        // sigma vectors to its TRUE residual, 3 sqrt(sum_j |beta_j|^2 err_j^2), stays below tol / 2; otherwise every sigma vector of the space is
+        // formed again with all slices and the iteration goes on at full precision
+        if (S.adapt_tol > 0.0 && !S.sig_err.empty()) {
+          bool redo = false;
+          for (int sidx : active) {
+            if (relres[sidx] > tol) continue;
+            double e2 = 0.0;      // independent errors add in quadrature; factor 3 for what the error model does not know
+            for (int j = 0; j < L; ++j) e2 += std::norm(beta[(size_t)sidx * maxdim + j]) * S.sig_err[j] * S.sig_err[j];
+            if (3.0 * std::sqrt(e2) > 0.5 * tol * norm_xi[sidx / nomega]) redo = true;
+          }
+          if (redo && !last) {
+            S.adapt_tol = 0.0;
+            L0 = 0;
+            continue;
+          }
+        }
         {
           std::vector<int> wr;
           for (int sidx : active)
@@ -356,6 +382,12 @@ static int solve_impl(cclr_ctx *ctx, const cclr_c128 *xi1, const cclr_c128 *xi2,
             for (int a = 0; a < m; ++a)
               for (int j = 0; j < L; ++j) g[a] += std::conj(Cc[a][j]) * beta[(size_t)sidx * maxdim + j];
             for (int j = 0; j < maxdim; ++j) beta[(size_t)sidx * maxdim + j] = j < m ? g[j] : cplx(0.0);
+          }
+          if (!S.sig_err.empty()) {      // error estimates of the collapsed sigma vectors sigma' = S C
+            std::vector<double> en(maxdim, 0.0);
+            for (int a = 0; a < m; ++a)
+              for (int j = 0; j < L; ++j) en[a] += std::abs(Cc[a][j]) * S.sig_err[j];
+            S.sig_err = en;
           }
           std::fill(S.G.begin(), S.G.end(), cplx(0.0));
           std::fill(S.c.begin(), S.c.end(), cplx(0.0));

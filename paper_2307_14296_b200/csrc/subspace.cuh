@@ -31,6 +31,27 @@ struct Space {
   std::vector<cplx> G;        // maxdim x maxdim, row-major: G[i][j] = b_i^H sigma_j
   int sigma_calls = 0;
   bool left = false;          // sigma_j = A^T b_j (left transform) instead of A b_j
+  // Precision on demand (solver.cu; contexts whose ladder / ring run as integer-slice products, zgemm_oz.cu): a trial vector
+  // added when the residuals have fallen to relres enters the solutions with coefficients of that size, so its sigma vector may
+  // carry a relative error ~ tol / relres without moving the converged residual (inexact-Krylov argument) -- sigma_j is then
+  // formed with fewer slices (15, 10, 6 pair products instead of 21).  adapt_tol = 0: always all slices.
+  double adapt_tol = 0.0, adapt_relres = 1.0;
+  std::vector<double> sig_err;   // per basis vector: estimated 2-norm error of sigma_j from the dropped slices (0 with all slices)
+  int reduced_sigma = 0;         // how many sigma vectors were formed with fewer slices
+
+  double offdiag_max = 1.0;      // largest || sigma_j - D b_j || seen so far (unit b_j): the size of the contractions' contribution
+
+  // slices for the next sigma vectors.  The vector enters the solutions with |beta_j| ~ relres ||xi||; its sigma error
+  // eps_j ||sigma_j - D b_j|| (only the contractions are inexact, the diagonal part is FP64) is to stay a small part of the budget
+  // tol ||xi|| / 2 shared by ~50 such vectors adding in quadrature with a safety factor 3: eps_j <= tol / (50 w relres),
+  // w = offdiag_max, eps(s) = 16 * 2^(-7 s) (the measured size of the truncation error of an s-slice product).
+  int slices_for_next() const {
+    const OzWorkspace *oz = ctx->ws.oz;
+    if (!oz || !(adapt_tol > 0.0) || (ctx->graph_enabled && !ctx->graph_failed)) return 0;   // a replayed graph has its slices baked in
+    int se = oz->slices;
+    while (se > 2 && std::ldexp(16.0, -7 * (se - 1)) * 50.0 * offdiag_max * std::max(adapt_relres, 1e-300) <= adapt_tol) --se;
+    return se < oz->slices ? se : 0;
+  }
 
   c128 *b(int j) { return Bm.p + (size_t)j * n; }
   c128 *s(int j) { return Sm.p + (size_t)j * n; }
@@ -112,12 +133,39 @@ struct Space {
 
   // sigma_j = A b_j for j in [L0, L) and the new rows / columns of G
   void extend_sigma(int L0) {
-    for (int j = L0; j < L; ++j) {
-      cclr_sigma_one(ctx, b(j), b(j) + n1, make_double2(0.0, 0.0), s(j), s(j) + n1, false, left);
-      ++sigma_calls;
+    const int se = slices_for_next();
+    if (se) ctx->ws.oz->active = se;
+    try {
+      for (int j = L0; j < L; ++j) {
+        cclr_sigma_one(ctx, b(j), b(j) + n1, make_double2(0.0, 0.0), s(j), s(j) + n1, false, left);
+        ++sigma_calls;
+      }
+    } catch (...) {
+      if (se) ctx->ws.oz->active = 0;
+      throw;
     }
+    if (se) ctx->ws.oz->active = 0;
     const int nn = L - L0;
     if (nn == 0) return;
+    if ((int)sig_err.size() < maxdim) sig_err.resize(maxdim, 0.0);
+    if (ctx->ws.oz && adapt_tol > 0.0 && ctx->D) {
+      // || sigma_j - D b_j || of the new vectors (one pass each), through the dot scratch of the context
+      cclr_ensure_dot_scratch(ctx, nn);
+      double *acc = (double *)ctx->dot_out;
+      check(cudaMemsetAsync(acc, 0, (size_t)nn * sizeof(double), st), "memset");
+      for (int j = 0; j < nn; ++j) check(offdiag_norm2(st, s(L0 + j), b(L0 + j), ctx->D, n, acc + j), "offdiag_norm2");
+      std::vector<double> w(nn);
+      check(cudaMemcpyAsync(w.data(), acc, (size_t)nn * sizeof(double), cudaMemcpyDeviceToHost, st), "D2H norms");
+      check(cudaStreamSynchronize(st), "sync norms");
+      for (int j = 0; j < nn; ++j) {
+        const double wj = std::sqrt(std::max(0.0, w[j]));
+        offdiag_max = std::max(offdiag_max, wj);
+        sig_err[L0 + j] = se ? std::ldexp(16.0, -7 * se) * wj : 0.0;
+      }
+      if (se) reduced_sigma += nn;
+    } else {
+      for (int j = 0; j < nn; ++j) sig_err[L0 + j] = 0.0;
+    }
     std::vector<cplx> cols = dots(Bm.p, L, s(L0), nn);           // G[0:L, L0:L]
     for (int i = 0; i < L; ++i)
       for (int j = 0; j < nn; ++j) G[(size_t)i * maxdim + L0 + j] = cols[(size_t)i * nn + j];

@@ -295,6 +295,32 @@ cudaError_t precondition(cudaStream_t st, c128 *y, const c128 *x, const double *
   return cudaGetLastError();
 }
 
+// out[0] += sum_i |s_i - D_i b_i|^2 : the part of a sigma vector that does not come from the orbital-energy diagonal (what the
+// contractions contribute; the solver scales its error estimate of reduced-precision sigma vectors with it).  out zeroed by the caller.
+__global__ void __launch_bounds__(256) offdiag_norm2_kernel(const c128 *__restrict__ s, const c128 *__restrict__ b,
+                                                            const double *__restrict__ D, long n, double *out) {
+  double acc = 0.0;
+  for (long i = (long)blockIdx.x * 256 + threadIdx.x; i < n; i += (long)gridDim.x * 256) {
+    const c128 sv = s[i], bv = b[i];
+    const double d = D[i], re = sv.x - d * bv.x, im = sv.y - d * bv.y;
+    acc += re * re + im * im;
+  }
+  for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+  __shared__ double red[8];
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = acc;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < 8; ++w) acc += red[w];
+    atomicAdd(out, acc);
+  }
+}
+cudaError_t offdiag_norm2(cudaStream_t st, const c128 *s, const c128 *b, const double *D, long n, double *out) {
+  if (n <= 0) return cudaSuccess;
+  offdiag_norm2_kernel<<<stream_grid(n), 256, 0, st>>>(s, b, D, n, out);
+  cclr_count_launch();
+  return cudaGetLastError();
+}
+
 cudaError_t scale_vec(cudaStream_t st, c128 *y, c128 alpha, long n) {
   if (n <= 0) return cudaSuccess;
   scale_kernel<<<stream_grid(n), 256, 0, st>>>(y, alpha, n);

@@ -623,10 +623,13 @@ cudaError_t zgemm_oz_register(cudaStream_t st, OzWorkspace *ow, const c128 *A, l
 // is folded into the sign pattern of the B slices), C' addressed as C[m * c_rs + n * c_cs].
 static cudaError_t oz_run(cudaStream_t st, int M, int N, int K, c128 alpha, const int8_t *sa_sl, const double *sa_sc, bool conjA,
                           const c128 *B, long ldb, bool b_is_kn, bool conjB, c128 beta, c128 *C, long c_rs, long c_cs, OzWorkspace *ow) {
-  const int s = ow->slices;
+  const int s_all = ow->slices;
+  // the leading slices of a decomposition are the decomposition with fewer slices (the slicing is sequential), so a product at
+  // reduced precision reads the first `active` slices of the registered operands and slices the per-call side that far only
+  const int s = (ow->active >= 2 && ow->active < s_all) ? ow->active : s_all;
   const long ldp = oz_ldp(K);
   // ---- B: always sliced per call (the trial vector side) ----
-  cudaError_t err = oz_ensure(st, (void **)&ow->scratch[1], &ow->scratch_bytes[1], (size_t)s * 2 * N * ldp);
+  cudaError_t err = oz_ensure(st, (void **)&ow->scratch[1], &ow->scratch_bytes[1], (size_t)s_all * 2 * N * ldp);
   if (err != cudaSuccess) return err;
   err = oz_ensure(st, (void **)&ow->scale[1], &ow->scale_bytes[1], (size_t)N * sizeof(double));
   if (err != cudaSuccess) return err;

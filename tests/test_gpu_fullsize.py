@@ -212,3 +212,35 @@ def test_properties_at_full_size_with_T(cfg):
         assert rel(q2, o2 - zz * x2) < 1e-14 and rel(q1, o1 - zz * x1) < 1e-14
     ctx.close()
     torch.cuda.empty_cache()
+
+
+@pytest.mark.parametrize("cfg", [3])
+def test_precision_on_demand_keeps_the_true_residual(cfg):
+    """cclr_solve on the integer-slice path forms the sigma vectors of late trial vectors with fewer slices (subspace.cuh: their
+    coefficients in the solutions are of the size of the residual at the time they were added).  The converged solutions are
+    checked here with the OTHER arithmetic: the residual (A - z) t + xi recomputed whole-vector by cclr_sigma on the FP64 tensor
+    cores (cclr_set_gemm_path 0) must sit at the solver's tolerance, for a real and a damped shift pair, and for the left solver."""
+    import paper_2307_14296_b200 as cc
+    o, v = synth.CONFIGS[cfg]["o"], synth.CONFIGS[cfg]["v"]
+    eri = {k: synth.eri_class(k, o, v, seed=0, device="cuda") for k in ("oooo", "ooov", "oovv", "ovvo", "ovvv", "vvvv")}
+    f = synth.fock(o, v, seed=0).cuda()
+    t1, t2 = synth.first_order_amplitudes(o, v, f, eri["oovv"])      # a well-conditioned Jacobian (random T is not, at this size)
+    ctx = cc.cclr_create(o, v, f, eri, t1, t2, cc.ERI_INPLACE)
+    del eri
+    assert ctx.gemm_slices() == 6
+    xi1, xi2 = synth.amplitudes(o, v, seed=21, cls1="x1", cls2="x2", device="cuda", nvec=1)
+    tol = 1e-10
+    nxi = float(torch.sqrt(xi1.abs().pow(2).sum() + xi2.abs().pow(2).sum()))
+    for gamma, solve, sig in ((0.0, cc.cclr_solve, cc.cclr_sigma), (0.0045, cc.cclr_solve, cc.cclr_sigma),
+                              (0.0, cc.cclr_solve_left, cc.cclr_sigma_left)):
+        omegas = [0.0773, -0.0773]
+        s1, s2, info = solve(ctx, xi1, xi2, omegas, gamma, tol=tol, maxiter=200)
+        assert info.converged == 1
+        assert ctx.set_gemm_path(0) == 0
+        for k, w in enumerate(omegas):
+            q1, q2 = sig(ctx, s1[0, k][None].contiguous(), s2[0, k][None].contiguous(), w, gamma)
+            r = float(torch.sqrt((q1[0] + xi1[0]).abs().pow(2).sum() + (q2[0] + xi2[0]).abs().pow(2).sum()))
+            assert r <= 1.2 * tol * nxi, (gamma, w, r / nxi)
+        assert ctx.set_gemm_path(1) == 1
+    ctx.close()
+    torch.cuda.empty_cache()
