@@ -245,14 +245,37 @@ extern "C" int cclr_ccsd(int o, int v, const cclr_c128 *fock, const cclr_eri_pac
       check(cudaStreamSynchronize(st), "sync coef");
     };
     int nhist = 0;
-    for (int it = 0; it < maxiter; ++it) {
-      res.iterations = it;
-      E.direct(T.p, OM.p);
+    // Precision on demand on the integer-slice path: a residual of size r only has to be known to a fraction of r, so the
+    // contractions of an evaluation use the fewest slices with 16 * 2^(-7 s) * 10 <= r_prev / 100 (10 = a bound on the size of the
+    // contracted terms); 2 slices at the start, all of them near convergence.  A residual that meets tol with fewer than all
+    // slices is evaluated again with all of them before it is accepted.
+    double prev_res = 1.0;
+    auto evaluate = [&](int active) {
+      E.oz.active = active;
+      try {
+        E.direct(T.p, OM.p);
+      } catch (...) {
+        E.oz.active = 0;
+        throw;
+      }
+      E.oz.active = 0;
       ++res.sigma_calls;     // (residual evaluations)
-      // ---- convergence on the full-tensor 2-norm: ||Omega1||^2 + 4 ||Omega2 (unique)||^2 ----
+      // ---- the full-tensor 2-norm: ||Omega1||^2 + 4 ||Omega2 (unique)||^2 ----
       const double d1 = host_dots(OM.p, n, 1, OM.p, n, 1, n1, true)[0].real();
       const double d2 = host_dots(OM.p + n1, n, 1, OM.p + n1, n, 1, n2, true)[0].real();
       res.residual = std::sqrt(std::max(0.0, d1 + 4.0 * d2));
+    };
+    for (int it = 0; it < maxiter; ++it) {
+      res.iterations = it;
+      int active = 0;
+      if (E.ws.oz && E.oz.slices > 2) {
+        int se = 2;
+        while (se < E.oz.slices && std::ldexp(160.0, -7 * se) > 0.01 * prev_res) ++se;
+        active = se < E.oz.slices ? se : 0;
+      }
+      evaluate(active);
+      if (active && std::isfinite(res.residual) && res.residual <= tol) evaluate(0);
+      prev_res = std::isfinite(res.residual) ? std::max(res.residual, 1e-300) : 1.0;
       if (!std::isfinite(res.residual) || res.residual > 1e6) break;
       if (res.residual <= tol) { res.converged = 1; rc = CCLR_OK; break; }
       if (it == maxiter - 1) { res.iterations = maxiter; break; }
