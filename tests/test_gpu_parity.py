@@ -329,6 +329,28 @@ def test_slice_count_follows_the_range_inside_the_rows():
     ctx.close()
 
 
+def test_solver_with_precision_on_demand_is_certified_by_the_oracle_residual():
+    """cclr_solve on the integer-slice path (forced at a size the full oracle can do; CCLR_NO_GRAPH so that the slice count can
+    follow the residual, subspace.cuh) -- the solutions are certified by the ORACLE's sigma: ||(A - z) t + xi|| <= 2 tol ||xi||."""
+    cc = _lib()
+    o, v = 9, 34
+    s = make_system(o, v, seed=91, t_scale=0.01, diag_fock=True, eri_scale=0.01)     # weakly coupled: a well-conditioned Jacobian
+    ctx = gpu_context(s, cc.GEMM_INT8_ANY_SIZE | cc.NO_GRAPH)
+    assert ctx.gemm_slices() == 6
+    c = cclr.CCLR(s["ints"], s["t1f"], s["t2f"])
+    xi1, xi2 = synth.amplitudes(o, v, seed=92, cls1="x1", cls2="x2")
+    gamma, omegas, tol = 0.0045, [0.0773, -0.0773], 1e-10
+    t1s, t2s, info = cc.cclr_solve(ctx, xi1.cuda(), xi2.cuda(), omegas, gamma, tol=tol, maxiter=300)
+    assert info.converged == 1
+    xi = np.concatenate([xi1[0].numpy(), xi2[0].numpy()])
+    for k, w in enumerate(omegas):
+        g1, g2 = packing.unpack_amplitudes(t1s[0, k].cpu().numpy(), t2s[0, k].cpu().numpy(), o, v)
+        q1, q2 = c.sigma(g1, g2, z=w + 1j * gamma)
+        res = packing.flat(q1, q2) + xi
+        assert np.linalg.norm(res) <= 2 * tol * np.linalg.norm(xi), (w, np.linalg.norm(res) / np.linalg.norm(xi))
+    ctx.close()
+
+
 def test_ladder_and_ring_terms_match_oracle():
     cc = _lib()
     o, v = 4, 20
