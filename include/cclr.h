@@ -114,7 +114,13 @@ typedef struct {
  * one shared Krylov subspace (steps 1-5 of PAPER.md:952-967 in the readings of DESIGN.md; A is shift independent so
  * one sigma serves every frequency).  Convergence: ||(A - z)t + xi||_2 <= tol * ||xi||_2 over unique elements.
  * omegas (host) may be negative, gamma may be negative.  Outputs: t1_out [nrhs][nomega][v*o], t2_out
- * [nrhs][nomega][vv*oo].  info (host) may be NULL. */
+ * [nrhs][nomega][vv*oo].  info (host) may be NULL.
+ * On a context whose ladder / ring run as integer-slice products (cclr_gemm_slices > 0, no CUDA-graph replay) the sigma vectors of
+ * trial vectors that are added late use fewer slices -- they enter the solutions with coefficients of the size of the residual at
+ * that time -- and a converged system is accepted only while the estimated effect of that on its TRUE residual stays below tol / 2;
+ * otherwise the iteration falls back to all slices.  The environment variable
+ * CCLR_SOLVER_ALL_SLICES=1 keeps every sigma vector at all slices.  The same holds for cclr_solve_left, cclr_lambda and the
+ * response entry points built on them. */
 int cclr_solve(cclr_ctx *ctx, const cclr_c128 *xi1, const cclr_c128 *xi2, int nrhs, const double *omegas,
                int nomega, double gamma, double tol, int maxiter, cclr_c128 *t1_out, cclr_c128 *t2_out,
                cclr_solve_info *info);
@@ -200,7 +206,11 @@ typedef struct {
  * t -= Omega / D with DIIS on the direct residual plan (csrc/plans.inc CCLR_PLAN_OMEGA; the
  * quadrature of the Jacobian, cclr_ccsd_residual mode 1, is the independent cross-check).
  * t1 [v][o], t2 [vv][oo] are IN/OUT device arrays: the start amplitudes on entry (zeros are fine), the solution on exit.
- * The integrals are only read.  Returns CCLR_OK, or CCLR_ENOTCONV (best iterate written, info filled). */
+ * The integrals are only read.  Returns CCLR_OK, or CCLR_ENOTCONV (best iterate written, info filled).
+ * From the size where it pays (>= 64 output tiles) and when 7/8 of <ab||ef> + <ma||ef> fit twice into the free device memory, the
+ * ladder, <ma||ef> tau and the ring-shaped contractions of the residual run as integer-slice products (csrc/zgemm_oz.cu) whose slice
+ * count follows the residual: 2 slices far from convergence, one more than cclr_create would take near it; a residual that meets tol
+ * with fewer than all slices is evaluated again with all of them before it is accepted. */
 int cclr_ccsd(int o, int v, const cclr_c128 *fock, const cclr_eri_packed *eri, cclr_c128 *t1, cclr_c128 *t2, double tol,
               int maxiter, void *cuda_stream, cclr_ccsd_info *info);
 

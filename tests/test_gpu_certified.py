@@ -58,15 +58,28 @@ def _rms(x):
 def _certify_residual(what, r1, r2, rhs1, rhs2):
     """r1, r2 = sampled residual elements (singles, doubles); rhs = the whole right-hand side.  The solver's criterion is
     ||r||_2 <= TOL ||rhs||_2 over unique elements, so (rigorously) no element of a converged residual exceeds TOL ||rhs||_2,
-    and the stratified estimate n1 <|r1|^2> + n2 <|r2|^2> of ||r||^2 must come out at that level too (factor 5 for the
-    sampling noise); a wrong solution shows elements of the size of the right-hand side's, ten orders of magnitude above."""
+    and the stratified estimate n1 <|r1|^2> + n2 <|r2|^2> of ||r||^2 must come out at that level too (factor 10 for the
+    sampling noise: 15 + 30 elements of a residual whose element sizes span orders of magnitude -- a draw of 5.4 came up at
+    config 5 for a solution whose whole-vector residual, recomputed with both tensor paths, is 0.97 TOL); a wrong solution shows
+    elements of the size of the right-hand side's, ten orders of magnitude above.  The whole-vector statement is made by
+    _whole_vector_residual below."""
     n1, n2 = np.size(rhs1), np.size(rhs2)
     norm = float(np.sqrt(np.sum(np.abs(rhs1) ** 2) + np.sum(np.abs(rhs2) ** 2)))
     r = np.concatenate([r1, r2])
     assert np.abs(r).max() <= 2 * TOL * norm, (what, "max sampled residual", np.abs(r).max(), TOL * norm)
     est = float(np.sqrt(n1 * np.mean(np.abs(r1) ** 2) + n2 * np.mean(np.abs(r2) ** 2)))
-    assert est <= 5 * TOL * norm, (what, "estimated ||r||", est, TOL * norm)
+    assert est <= 10 * TOL * norm, (what, "estimated ||r||", est, TOL * norm)
     return est / norm
+
+
+def _whole_vector_residual(cc, ctx, t1, t2, xi1, xi2, omega, gamma):
+    """||(A - z) t + xi|| / ||xi|| over the WHOLE vectors with sigma recomputed on the FP64 tensor cores (cclr_set_gemm_path 0) --
+    the other arithmetic than the solver's integer-slice path; complements the oracle's sampled elements."""
+    was = ctx.set_gemm_path(0)
+    q1, q2 = cc.cclr_sigma(ctx, t1[None].contiguous(), t2[None].contiguous(), omega, gamma)
+    ctx.set_gemm_path(1)
+    r = torch.sqrt((q1[0] + xi1).abs().pow(2).sum() + (q2[0] + xi2).abs().pow(2).sum())
+    return float(r / torch.sqrt(xi1.abs().pow(2).sum() + xi2.abs().pow(2).sum()))
 
 
 def _udot(u, w):
@@ -150,6 +163,8 @@ def test_workflow_certified_by_the_sampled_oracle(cfg):
             s1, s2 = S.sigma_elements(h[0], h[1], singles, doubles, z=zz)
             x1, x2 = _pick(*vecs[op]["hxi"], o, v, singles, doubles)
             report[key] = _certify_residual(key, np.array(s1) + x1, np.array(s2) + x2, *vecs[op]["hxi"])
+            whole = _whole_vector_residual(cc, ctx, a1, a2, vecs[op]["xi"][0], vecs[op]["xi"][1], zz.real, zz.imag)
+            assert whole <= 1.2 * TOL, (key, "whole-vector residual on the FP64 tensor cores", whole)
         # ---- step 4: the response function assembled by the oracle from the certified vectors vs the library, 1e-8 ----
         want = occlr.cc_ci_from_vectors(_udot, vecs["X"]["heta"], vecs["Y"]["heta"], hl, vecs["X"]["hxi"], vecs["Y"]["hxi"],
                                         hs["tY_z"], hs["tX_mz"], hs["tY_zc"], hs["tX_mzc"])
@@ -176,5 +191,7 @@ def test_workflow_certified_by_the_sampled_oracle(cfg):
             for k in (0, 21, 42, 63):
                 g1, g2 = S.sigma_elements(_np(s1[r, k]), _np(s2[r, k]), singles, doubles, z=complex(omegas[k], 0.0045))
                 _certify_residual(("sweep", r, k), np.array(g1) + x1, np.array(g2) + x2, *hxi)
+                whole = _whole_vector_residual(cc, ctx, s1[r, k], s2[r, k], xi1[r], xi2[r], omegas[k], 0.0045)
+                assert whole <= 1.2 * TOL, ("sweep", r, k, "whole-vector residual on the FP64 tensor cores", whole)
     ctx.close()
     torch.cuda.empty_cache()
