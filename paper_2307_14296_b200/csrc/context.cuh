@@ -26,6 +26,9 @@ struct cclr_ctx {
   std::vector<double> op_ms;      // per operation of the sigma plan, summed over the vectors of the last call
   std::vector<cudaEvent_t> events;
   // staging buffers of cclr_sigma_host
+  cudaStream_t copy_stream = nullptr;   // cclr_sigma_host: x2 goes to the device here while the x1-only statements of the plan run
+  cudaEvent_t copy_done = nullptr;
+  int first_x2_op = 0;                  // index of the first statement of the sigma plan that reads x2
   c128 *host_stage = nullptr;
   size_t host_stage_elems = 0;
   c128 *lambda = nullptr;         // ground-state multipliers [n1 + n2], solved on first use by cclr_response_ci

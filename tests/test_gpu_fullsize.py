@@ -210,6 +210,10 @@ def test_properties_at_full_size_with_T(cfg):
         zz = 0.0773 + 0.0045j
         q1, q2 = cc.cclr_sigma(ctx, x1, x2, zz.real, zz.imag)
         assert rel(q2, o2 - zz * x2) < 1e-14 and rel(q1, o1 - zz * x1) < 1e-14
+        # the host-buffer entry (x2 copied on a second stream under the x1-only statements at this size) returns the same bits
+        h1, h2 = torch.empty_like(x1, device="cpu").pin_memory(), torch.empty_like(x2, device="cpu").pin_memory()
+        cc.cclr_sigma_host(ctx, x1.cpu().pin_memory(), x2.cpu().pin_memory(), zz.real, zz.imag, h1, h2)
+        assert torch.equal(h1, q1.cpu()) and torch.equal(h2, q2.cpu())
     ctx.close()
     torch.cuda.empty_cache()
 

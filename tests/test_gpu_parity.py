@@ -372,12 +372,13 @@ def test_ladder_and_ring_terms_match_oracle():
     ctx.close()
 
 
-def test_sigma_host_entry_point_and_inplace_vvvv():
+@pytest.mark.parametrize("flags", [0, 8])     # 8 = CCLR_NO_GRAPH: the host entry copies x2 on a second stream while the x1-only
+def test_sigma_host_entry_point_and_inplace_vvvv(flags):     # statements of the plan run
     cc = _lib()
     o, v = 4, 20
     s = make_system(o, v, seed=12)
     dev = {k: x.cuda() for k, x in s["eri"].items()}
-    ctx = cc.cclr_create(o, v, s["fock"].contiguous().cuda(), dev, s["t1"].cuda(), s["t2"].cuda(), cc.ERI_INPLACE)
+    ctx = cc.cclr_create(o, v, s["fock"].contiguous().cuda(), dev, s["t1"].cuda(), s["t2"].cuda(), cc.ERI_INPLACE | flags)
     c = cclr.CCLR(s["ints"], s["t1f"], s["t2f"])
     x1, x2 = synth.amplitudes(o, v, seed=5, cls1="x1", cls2="x2", nvec=2)
     o1, o2 = torch.empty_like(x1), torch.empty_like(x2)
