@@ -37,7 +37,6 @@
 #include <atomic>
 #include <mutex>
 #include <cmath>
-#include <cstdlib>
 
 namespace {
 
@@ -653,7 +652,6 @@ static cudaError_t oz_run(cudaStream_t st, int M, int N, int K, c128 alpha, cons
   a.BN = BN;
   a.stage_bytes = OZ_A_BYTES + BN * OZ_BK;
   a.nstages = std::min(OZ_MAX_STAGES, (OZ_MAX_SMEM - 1024 - 256) / a.stage_bytes);
-  if (const char *e = getenv("CCLR_OZ_STAGES")) a.nstages = std::max(2, std::min(a.nstages, atoi(e)));     // tuning runs
 
   const int smem_bytes = 1024 + a.nstages * a.stage_bytes + 256;
   const int tiles_n = (a.N2 + BN - 1) / BN, tiles_m = (M + OZ_BM - 1) / OZ_BM;
