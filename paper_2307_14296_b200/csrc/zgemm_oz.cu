@@ -688,18 +688,20 @@ static cudaError_t oz_run(cudaStream_t st, int M, int N, int K, c128 alpha, cons
   }
   // cluster shape c_m x c_n (tiles along M x along N that share their operand tiles by multicast): up to 8 tile columns can form
   // ONE cluster row (the A panel then leaves HBM exactly once -- without it the tile columns of a panel drift apart in time and
-  // re-read it: 538 GB instead of 104 GB at config 4, profiles/r02_oz_*); otherwise 4 x 2.  Clusters must fit the GPCs (6-CTA
-  // clusters keep 132 of 148 SMs busy, which still beats unclustered CTAs by 2x); a shape the device cannot co-schedule on at
-  // least 3/4 of its SMs gives way to the next smaller one
+  // re-read it: 538 GB instead of 104 GB at config 4, profiles/r02_oz_*); more tile columns are covered by c_m x 1 or 4 x 2
+  // clusters.  Clusters must fit the GPCs (8-, 6-, 5-CTA clusters keep 120, 132, 130 of the 148 SMs busy), and every cluster takes
+  // the same time, so the shape is picked by the number of WAVES ceil(clusters / resident clusters) -- at the mid-size configs the
+  // last partial wave is what differs (ring of config 5: 3 waves of 4 x 2 clusters, 2 waves of 6 x 1: 2.7 -> 1.9 ms); ties go
+  // to the shape listed first
   struct Shape { int cm, cn; };
-  Shape cand[8];
+  Shape cand[12];
   int ncand = 0;
   if (ow->force_cm >= 1 && ow->force_cn >= 1 && ow->force_cm * ow->force_cn <= 8) cand[ncand++] = {ow->force_cm, ow->force_cn};
   else if (tiles_n <= 8) {
     for (int d = tiles_n; d >= 1; --d)
       if (tiles_n % d == 0) cand[ncand++] = {1, d};
   } else {
-    const Shape all[6] = {{4, 2}, {2, 2}, {2, 4}, {1, 4}, {1, 2}, {1, 1}};
+    const Shape all[10] = {{5, 1}, {4, 2}, {6, 1}, {4, 1}, {8, 1}, {3, 1}, {2, 2}, {2, 1}, {1, 2}, {1, 1}};
     for (const Shape &c : all)
       if (c.cm <= tiles_m || c.cm == 1) cand[ncand++] = c;
   }
@@ -718,7 +720,8 @@ static cudaError_t oz_run(cudaStream_t st, int M, int N, int K, c128 alpha, cons
     cfg.numAttrs = c.cm * c.cn > 1 ? 1 : 0;
     return ct_n;
   };
-  int resident[8];
+  int resident[12];
+  long waves[12];
   const int sms = zgemm_num_sms();
   for (int i = 0; i < ncand; ++i) {
     cudaLaunchConfig_t cfg;
@@ -728,12 +731,21 @@ static cudaError_t oz_run(cudaStream_t st, int M, int N, int K, c128 alpha, cons
     if (cand[i].cm * cand[i].cn == 1) active = sms;
     else if (cudaOccupancyMaxActiveClusters(&active, (const void *)zgemm_oz_kernel, &cfg) != cudaSuccess) { cudaGetLastError(); active = 0; }
     resident[i] = std::min(active * cand[i].cm * cand[i].cn, sms);
+    const long ncl = (long)((tiles_m + cand[i].cm - 1) / cand[i].cm) * ((tiles_n + cand[i].cn - 1) / cand[i].cn);
+    const long res_cl = std::max(1, resident[i] / (cand[i].cm * cand[i].cn));
+    waves[i] = resident[i] >= 1 ? (ncl + res_cl - 1) / res_cl : (1L << 60);
+    // unclustered CTAs re-read their operands from HBM (see above): only when nothing else can be scheduled
+    if (cand[i].cm * cand[i].cn == 1 && ncand > 1 && tiles_n > 1) waves[i] = (1L << 59);
   }
+  int order[12];
+  for (int i = 0; i < ncand; ++i) order[i] = i;
+  std::stable_sort(order, order + ncand, [&](int x, int y) { return waves[x] < waves[y]; });
   err = cudaErrorLaunchFailure;
   bool launched = false;
-  for (int pass = 0; pass < 2 && !launched; ++pass)          // pass 0: shapes resident on >= 3/4 of the SMs; pass 1: any
-    for (int i = 0; i < ncand && !launched; ++i) {
-      if (resident[i] < 1 || (pass == 0 && resident[i] * 4 < sms * 3)) continue;
+  for (int q = 0; q < ncand && !launched; ++q) {
+    {
+      const int i = order[q];
+      if (resident[i] < 1) continue;
       cudaLaunchConfig_t cfg;
       cudaLaunchAttribute attr[1];
       a.c_m = cand[i].cm; a.c_n = cand[i].cn;
@@ -741,6 +753,7 @@ static cudaError_t oz_run(cudaStream_t st, int M, int N, int K, c128 alpha, cons
       err = cudaLaunchKernelEx(&cfg, zgemm_oz_kernel, tA, tB, a);
       if (err == cudaSuccess) launched = true; else cudaGetLastError();
     }
+  }
   if (!launched) return err;
   cclr_count_launch();
   return cudaSuccess;
