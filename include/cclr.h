@@ -246,6 +246,19 @@ const char *cclr_strerror(int code);
 int cclr_last_cuda_error(void); /* CUDA error code behind the last CCLR_ECUDA of the calling thread */
 const char *cclr_last_error_message(void); /* text of the last failure of the calling thread ("" if none) */
 
+/* The property contraction for callers that cannot allocate device memory (code under CUDA-graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): result[k] = sum_i eta1[i] x1[k][i] + sum_i eta2[i] x2[k][i] (bilinear, as cclr_property) for
+ * nvec <= CCLR_NOALLOC_MAX_VECS vectors, eta1 [n1], eta2 [n2], x1 [nvec][n1], x2 [nvec][n2] and result [nvec] all DEVICE arrays
+ * (the caller owns inputs and outputs; the result stays on the device and the call does not synchronise).  No context, and no
+ * cudaMalloc / cudaFree / allocating routine inside: the partial sums of the two-pass reduction live in a file-scope static
+ * device array of 151,552 bytes (csrc/vecops.cu) that every GPU loading the library holds until exit.  Every call shares that array:
+ * calls that overlap on the GPU (other streams or threads) race; calls on one stream are safe, and stale contents are harmless.
+ * Returns CCLR_OK; CCLR_EINVAL with a message for null pointers, n1 < 1, n2 < 1, nvec < 1 or nvec > CCLR_NOALLOC_MAX_VECS;
+ * CCLR_ECUDA if the device address of the array cannot be had or a launch fails. */
+#define CCLR_NOALLOC_MAX_VECS 16
+int cclr_property_noalloc(void *cuda_stream, const cclr_c128 *eta1, const cclr_c128 *eta2, const cclr_c128 *x1, const cclr_c128 *x2,
+                          long n1, long n2, int nvec, cclr_c128 *result);
+
 /* ---- host-buffer forms (end-to-end timing: host<->device copies are part of the call) ------------------------ */
 /* Same as cclr_sigma with HOST x1, x2, out1, out2 (pinned or pageable). */
 int cclr_sigma_host(cclr_ctx *ctx, const cclr_c128 *x1, const cclr_c128 *x2, int nvec, double omega, double gamma,

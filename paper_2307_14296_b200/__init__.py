@@ -370,6 +370,21 @@ def cclr_property(ctx, eta1, eta2, x1, x2):
     return [complex(r.re, r.im) for r in res]
 
 
+NOALLOC_MAX_VECS = 16
+
+
+def cclr_property_noalloc(eta1, eta2, x1, x2, out):
+    """Bilinear eta . x_k for every vector k WITHOUT any device allocation inside the library (include/cclr.h:
+    cclr_property_noalloc): eta1 [n1], eta2 [n2], x1 [nvec, n1], x2 [nvec, n2] and out [nvec] are CUDA tensors of the caller;
+    nvec <= NOALLOC_MAX_VECS.  The result stays on the device (no synchronisation).  Calls that overlap on the GPU race."""
+    n1, n2 = eta1.numel(), eta2.numel()
+    nvec = x1.numel() // n1
+    rc = _lib.load().cclr_property_noalloc(_stream(), _dev(eta1, "eta1", n1), _dev(eta2, "eta2", n2), _dev(x1, "x1", nvec * n1),
+                                           _dev(x2, "x2", nvec * n2), n1, n2, nvec, _dev(out, "out", nvec))
+    _lib.check(rc, "cclr_property_noalloc")
+    return out
+
+
 def cclr_ladder(ctx, x2, out2=None):
     nvec = x2.numel() // ctx.n2
     if out2 is None:

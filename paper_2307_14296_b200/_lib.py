@@ -72,6 +72,7 @@ SIGNATURES = {
     "cclr_zgemm": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.POINTER(Complex), c128_p, C.c_long, C.c_int,
                              c128_p, C.c_long, C.c_int, C.c_int, C.POINTER(Complex), c128_p, C.c_long, C.c_int,
                              C.c_long, C.c_long, C.c_long, C.c_int]),
+    "cclr_property_noalloc": (C.c_int, [C.c_void_p, c128_p, c128_p, c128_p, c128_p, C.c_long, C.c_long, C.c_int, c128_p]),
     "cclr_set_gemm_path": (C.c_int, [C.c_void_p, C.c_int]),
     "cclr_gemm_slices": (C.c_int, [C.c_void_p]),
     "cclr_zgemm_oz": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.POINTER(Complex), c128_p, C.c_long, C.c_int,

@@ -380,3 +380,85 @@ cudaError_t shifted_copy(cudaStream_t st, c128 *out, const c128 *src, c128 alpha
   cclr_count_launch();
   return cudaGetLastError();
 }
+
+// ---- cclr_property_noalloc: the property contraction without a context and without any allocation (include/cclr.h) ----------
+// Callers that cannot call cudaMalloc (code under CUDA-graph capture, tight serving loops, harnesses that forbid it) get the
+// partial-sum scratch of the two-pass dot from this file-scope device array instead of a context's heap buffer: 2 (singles,
+// doubles) x CCLR_NOALLOC_MAX_VECS pairs x DOT_MAX_CHUNKS partial sums = 151,552 bytes, held by every GPU that loads the
+// library until the process exits.  Every call shares it: calls that overlap on the GPU (two streams, two threads) race.
+// Nothing in it has to start at zero -- dot_partial_kernel writes every slot dot_final reads -- so stale contents are harmless.
+#include "../../include/cclr.h"
+#include <mutex>
+#include <string>
+
+void cclr_set_error(const std::string &msg, cudaError_t e);   // context.cu
+
+static __device__ __align__(256) c128 g_noalloc_scratch[2 * CCLR_NOALLOC_MAX_VECS * DOT_MAX_CHUNKS];
+
+namespace {
+
+// out[k] = (sum_c p1[k][c]) + (sum_c p2[k][c]): the same two fixed-order sums cclr_property forms, added in the same order
+__global__ void noalloc_final_kernel(const c128 *__restrict__ p1, int c1, const c128 *__restrict__ p2, int c2, int nvec,
+                                     c128 *__restrict__ out) {
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= nvec) return;
+  c128 s1 = czero(), s2 = czero();
+  for (int c = 0; c < c1; ++c) s1 = cadd(s1, p1[(size_t)k * c1 + c]);
+  for (int c = 0; c < c2; ++c) s2 = cadd(s2, p2[(size_t)k * c2 + c]);
+  out[k] = cadd(s1, s2);
+}
+
+// device address of g_noalloc_scratch, looked up once per device with that device current (in host code the array's name is a
+// host-side stand-in, not a device address)
+cudaError_t noalloc_scratch_address(c128 **ptr) {
+  static std::mutex mu;
+  static c128 *addr[64] = {};
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  std::lock_guard<std::mutex> lock(mu);
+  if (dev >= 0 && dev < 64 && addr[dev]) { *ptr = addr[dev]; return cudaSuccess; }
+  void *p = nullptr;
+  e = cudaGetSymbolAddress(&p, g_noalloc_scratch);
+  if (e != cudaSuccess) return e;
+  if (dev >= 0 && dev < 64) addr[dev] = (c128 *)p;
+  *ptr = (c128 *)p;
+  return cudaSuccess;
+}
+
+}  // namespace
+
+extern "C" int cclr_property_noalloc(void *cuda_stream, const cclr_c128 *eta1, const cclr_c128 *eta2, const cclr_c128 *x1,
+                                     const cclr_c128 *x2, long n1, long n2, int nvec, cclr_c128 *result) {
+  if (!eta1 || !eta2 || !x1 || !x2 || !result || n1 < 1 || n2 < 1 || nvec < 1) {
+    cclr_set_error("cclr_property_noalloc: null pointer, n1 < 1, n2 < 1 or nvec < 1", cudaSuccess);
+    return CCLR_EINVAL;
+  }
+  if (nvec > CCLR_NOALLOC_MAX_VECS) {
+    cclr_set_error("cclr_property_noalloc: nvec exceeds CCLR_NOALLOC_MAX_VECS (" + std::to_string(CCLR_NOALLOC_MAX_VECS) +
+                       "), the size of the static scratch; split the call or use cclr_property",
+                   cudaSuccess);
+    return CCLR_EINVAL;
+  }
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  c128 *scratch = nullptr;
+  cudaError_t e = noalloc_scratch_address(&scratch);
+  if (e != cudaSuccess) {
+    cclr_set_error(std::string("cclr_property_noalloc: cudaGetSymbolAddress: ") + cudaGetErrorString(e), e);
+    return CCLR_ECUDA;
+  }
+  c128 *p1 = scratch, *p2 = scratch + (size_t)CCLR_NOALLOC_MAX_VECS * DOT_MAX_CHUNKS;
+  const int c1 = dot_chunks(n1), c2 = dot_chunks(n2);
+  dot_partial_kernel<<<dim3(c1, nvec), DOT_THREADS, 0, st>>>((const c128 *)eta1, n1, (const c128 *)x1, n1, nvec, n1, 0, 0,
+                                                             (n1 + c1 - 1) / c1, p1);
+  dot_partial_kernel<<<dim3(c2, nvec), DOT_THREADS, 0, st>>>((const c128 *)eta2, n2, (const c128 *)x2, n2, nvec, n2, 0, 0,
+                                                             (n2 + c2 - 1) / c2, p2);
+  noalloc_final_kernel<<<1, 32, 0, st>>>(p1, c1, p2, c2, nvec, (c128 *)result);
+  cclr_count_launch(3);
+  e = cudaGetLastError();
+  if (e != cudaSuccess) {
+    cclr_set_error(std::string("cclr_property_noalloc: ") + cudaGetErrorString(e), e);
+    return CCLR_ECUDA;
+  }
+  return CCLR_OK;
+}
