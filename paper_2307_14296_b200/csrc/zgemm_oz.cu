@@ -690,9 +690,9 @@ static cudaError_t oz_run(cudaStream_t st, int M, int N, int K, c128 alpha, cons
   // ONE cluster row (the A panel then leaves HBM exactly once -- without it the tile columns of a panel drift apart in time and
   // re-read it: 538 GB instead of 104 GB at config 4, profiles/r02_oz_*); more tile columns are covered by c_m x 1 or 4 x 2
   // clusters.  Clusters must fit the GPCs (8-, 6-, 5-CTA clusters keep 120, 132, 130 of the 148 SMs busy), and every cluster takes
-  // the same time, so the shape is picked by the number of WAVES ceil(clusters / resident clusters) -- at the mid-size configs the
-  // last partial wave is what differs (ring of config 5: 3 waves of 4 x 2 clusters, 2 waves of 6 x 1: 2.7 -> 1.9 ms); ties go
-  // to the shape listed first
+  // the same time, so at the mid-size configs the shape is picked by the number of WAVES ceil(clusters / resident clusters) -- the
+  // last partial wave is what differs (ring of config 5: 3 waves of 4 x 2 clusters, 2 waves of 6 x 1: 2.7 -> 1.9 ms) -- and at
+  // large sizes by the operand traffic (below)
   struct Shape { int cm, cn; };
   Shape cand[12];
   int ncand = 0;
@@ -721,7 +721,7 @@ static cudaError_t oz_run(cudaStream_t st, int M, int N, int K, c128 alpha, cons
     return ct_n;
   };
   int resident[12];
-  long waves[12];
+  double waves[12], traffic[12];
   const int sms = zgemm_num_sms();
   for (int i = 0; i < ncand; ++i) {
     cudaLaunchConfig_t cfg;
@@ -733,9 +733,25 @@ static cudaError_t oz_run(cudaStream_t st, int M, int N, int K, c128 alpha, cons
     resident[i] = std::min(active * cand[i].cm * cand[i].cn, sms);
     const long ncl = (long)((tiles_m + cand[i].cm - 1) / cand[i].cm) * ((tiles_n + cand[i].cn - 1) / cand[i].cn);
     const long res_cl = std::max(1, resident[i] / (cand[i].cm * cand[i].cn));
-    waves[i] = resident[i] >= 1 ? (ncl + res_cl - 1) / res_cl : (1L << 60);
+    waves[i] = resident[i] >= 1 ? (double)((ncl + res_cl - 1) / res_cl) : 1e30;
+    // operand bytes a tile pulls through L2 / HBM per k block ~ 1 / c_n (its A tile is shared by c_n CTAs) + 1 / c_m (B tile)
+    traffic[i] = 1.0 / cand[i].cn + 1.0 / cand[i].cm;
     // unclustered CTAs re-read their operands from HBM (see above): only when nothing else can be scheduled
-    if (cand[i].cm * cand[i].cn == 1 && ncand > 1 && tiles_n > 1) waves[i] = (1L << 59);
+    if (cand[i].cm * cand[i].cn == 1 && ncand > 1 && tiles_n > 1) waves[i] = 1e29;
+  }
+  // Few waves (mid-size products): the last partial wave decides -- fewest waves wins, ties to the shape that shares more.
+  // Many waves (>= 16 for every shape: config 4): the chip runs at its power cap and the total rate is the same for every shape
+  // that fills 3/4 of the SMs (ring of config 4: 78-80 ms for 4 x 2, 5 x 1, 6 x 1, 8 x 1), falling with the operand traffic
+  // (2 x 2: 84 ms, 1 x 2: 92 ms) -- and a shape that reads twice the bytes (5 x 1: 233 GB per call against 124 GB for 4 x 2)
+  // takes power from the kernels around it (the ladder after it: 78 -> 86 ms) -- so the shape that shares most wins.
+  double minw = 1e30;
+  for (int i = 0; i < ncand; ++i) minw = std::min(minw, waves[i]);
+  if (minw >= 16.0 && ncand > 1 && !(ow->force_cm >= 1 && ow->force_cn >= 1)) {
+    for (int i = 0; i < ncand; ++i)
+      waves[i] = (waves[i] < 1e29 && resident[i] * 4 >= sms * 3) ? traffic[i] + 1e-3 * waves[i] : 1e28 + waves[i];
+  } else {
+    for (int i = 0; i < ncand; ++i)
+      if (waves[i] < 1e29) waves[i] += 1e-3 * traffic[i];
   }
   int order[12];
   for (int i = 0; i < ncand; ++i) order[i] = i;
